@@ -1,0 +1,158 @@
+/*
+ * ants_recon.h -- C ABI of the B200-native statistical event reconstruction
+ * (contracting grids over B-spline LRFs) of the ANTS2 paper, arXiv:1602.07247.
+ *
+ * Problem statement (section 5.1.2): "For each event, statistical
+ * methods search for the position (and, optionally, the event energy) which
+ * results in the best match between the ... photosensor signals and those
+ * provided by a mathematical model of the detector ... constructed using the
+ * light response functions of the photosensors."
+ *
+ * Method (section 5.1.2.2 "Contracting Grids"): a regular grid of
+ * nodes centred at the start position (the centroid); at every
+ * node each sensor's LRF gives the expected signal, the energy is "the ratio
+ * of two sums over all photosensors: the sum of the photosensor signals and
+ * that of the LRF values", the match is Maximum Likelihood or Least Squares
+ * (PAPER.md:316); the best node becomes the centre of a finer grid with the
+ * same number of nodes; repeated a preconfigured number of iterations.
+ * LRFs are cubic B-splines (section 6): axial L(r)
+ * or axial+z L(r,z), one shared profile scaled
+ * by relative gains or one table per sensor (section 6.2).
+ *
+ * Every step runs in hand-written sm_100a CUDA kernels; there is no CPU
+ * fallback.  All functions return an ants_status code (0 = OK) and never throw.
+ * Points on which the paper is silent follow DESIGN.md "Readings" (R1..R18).
+ */
+#ifndef ANTS_RECON_H
+#define ANTS_RECON_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum ants_status {
+    ANTS_OK = 0,
+    ANTS_ERR_INVALID = -1,     /* NULL pointer, N < 1, bad knots/dims, G < 2, factor not in (0,1), K < 1, ... */
+    ANTS_ERR_UNSUPPORTED = -2, /* valid request outside the compiled limits (see ants_reconstruct) */
+    ANTS_ERR_CUDA = -3,        /* a CUDA runtime call failed (no device, launch error, ...) */
+    ANTS_ERR_NOMEM = -4        /* host or device allocation failed */
+};
+
+enum ants_method {
+    ANTS_POISSON_ML = 0,  /* A = sum S / sum L; score = Poisson deviance 2 sum[mu - S + S ln(S/mu)], mu = A L (R2) */
+    ANTS_CHI_SQUARE = 1   /* w = 1/max(S,1); A = sum w S L / sum w L^2; score = sum w (S - A L)^2 (R3, R4) */
+};
+
+/* Opaque LRF model living in device memory; immutable after create. */
+typedef struct ants_lrf ants_lrf_t;
+
+typedef struct {
+    int32_t n_sensors; /* N >= 1 */
+    int32_t n_lrf;     /* 1 = one shared profile, L_i = gains[i] * s(.); N = one table per sensor, L_i = s_i(.) */
+    int32_t lrf_dim;   /* 1 = axial s(r); 2 = axial+z s(r,z) tensor product */
+    int32_t n_int_r;   /* uniform intervals in r: n_int_r + 3 coefficients */
+    int32_t n_int_z;   /* uniform intervals in z (ignored when lrf_dim == 1) */
+} ants_lrf_dims_t;
+
+/*
+ * ants_lrf_create -- build the device-resident LRF model (step a0).
+ *   sensor_xy HOST [N][2] float, sensor axis positions in mm.
+ *   gains     HOST [N] float, all > 0; NULL means all 1.  Used in the centroid
+ *              and, when n_lrf == 1, as the profile scale.
+ *   knots     HOST {r_lo, r_hi} (lrf_dim 1) or {r_lo, r_hi, z_lo, z_hi} (lrf_dim 2);
+ *             breakpoints are uniform inside; requires 0 <= r_lo < r_hi, z_lo < z_hi.
+ *   coeffs    HOST [n_lrf][n_int_z + 3 (or 1)][n_int_r + 3] float, r fastest: uniform
+ *             cubic B-spline coefficients, no end conditions (R7).  r outside
+ *             [r_lo, r_hi] is clamped (R5); z outside [z_lo, z_hi] makes a node invalid (R6).
+ *   out       receives the handle; the library owns device copies of everything,
+ *             the caller may free its arrays on return.
+ * The model is created on the current CUDA device and must be used there.
+ * Errors: ANTS_ERR_INVALID, ANTS_ERR_UNSUPPORTED (lrf_dim 2 with n_lrf != 1;
+ * tables larger than the shared-memory budget), ANTS_ERR_CUDA, ANTS_ERR_NOMEM.
+ */
+int ants_lrf_create(const float *sensor_xy, const float *gains, const float *knots,
+                    const float *coeffs, const ants_lrf_dims_t *dims, ants_lrf_t **out);
+
+typedef struct {
+    int32_t dim;            /* 2 = search (x,y); 3 = search (x,y,z), requires lrf_dim == 2 */
+    int32_t nodes_per_axis; /* G >= 2; the grid has G^dim nodes */
+    float step0_xy;         /* first-iteration node spacing in x and y, mm, > 0 */
+    float step0_z;          /* first-iteration node spacing in z, mm (dim == 3), > 0 */
+    float factor;           /* contraction factor in (0,1): h_k = h_0 * factor^k (R1) */
+    int32_t n_iter;         /* K >= 1 iterations */
+    int32_t seed_mode;      /* 0 = centroid start (the only mode on the hot path, R12) */
+    float z_seed;           /* start z (dim 3) or fixed z (dim 2 with lrf_dim 2); NaN = (z_lo+z_hi)/2 (R10) */
+} ants_grid_params_t;
+
+/*
+ * ants_reconstruct -- steps a1..a6 for a batch of events, ONE kernel launch,
+ * asynchronous on `cuda_stream`, no allocation, no host synchronisation.
+ *   signals   DEVICE [n_events][N] float row-major, caller-owned, read-only.
+ *   out_xyzA  DEVICE [n_events][4] float: x, y, z (0 for axial LRFs), energy A
+ *             at the last best node (R11).
+ *   out_score DEVICE [n_events] float: the score at that node (deviance or chi-square).
+ *   cuda_stream  a cudaStream_t (NULL = default stream).
+ * Node order: linear index (iz*G + iy)*G + ix, x fastest; the first strict
+ * minimum in that order wins (R9); a node is invalid if z is outside the LRF
+ * range, if sum L <= 0 or (Poisson) some L_i <= 0 with S_i > 0.  Poisson ML
+ * clips negative signals to 0 first (R18).
+ * Per-event failure does not fail the call: an event with a non-finite signal,
+ * sum S <= 0 or sum S/g <= 0 gets x = y = z = A = NaN and score = +inf.
+ * Errors: ANTS_ERR_INVALID (NULL pointers with n_events > 0, bad grid values,
+ * dim 3 with an axial LRF, method not 0/1), ANTS_ERR_UNSUPPORTED (G^dim above
+ * the compiled limit: 256 nodes in 2-D, 512 in 3-D), ANTS_ERR_CUDA.
+ * n_events == 0 is a valid no-op.
+ */
+int ants_reconstruct(const ants_lrf_t *lrf, const float *signals, int64_t n_events,
+                     const ants_grid_params_t *grid, int32_t method,
+                     float *out_xyzA, float *out_score, void *cuda_stream);
+
+/*
+ * ants_reconstruct_trace -- ants_reconstruct plus, for the parity tests,
+ * out_path DEVICE [n_events][K] uint16: the winning linear node index of every
+ * iteration (0xFFFF when no node was valid or the event failed).
+ */
+int ants_reconstruct_trace(const ants_lrf_t *lrf, const float *signals, int64_t n_events,
+                           const ants_grid_params_t *grid, int32_t method,
+                           float *out_xyzA, float *out_score, uint16_t *out_path,
+                           void *cuda_stream);
+
+/*
+ * ants_reconstruct_host -- the same reconstruction for HOST buffers: signals,
+ * out_xyzA, out_score are host arrays (pinned memory makes the copies
+ * asynchronous).  The events are cut into chunks of `chunk_events` (<= 0: 2^20)
+ * which are copied in, reconstructed and copied back on a ring of three CUDA
+ * streams so that transfers overlap the kernels (BASELINE.json config 5:
+ * "processed in 8 streamed batches").  Returns after all results are in host
+ * memory.  Errors as ants_reconstruct, plus ANTS_ERR_NOMEM.
+ */
+int ants_reconstruct_host(const ants_lrf_t *lrf, const float *signals_host, int64_t n_events,
+                          const ants_grid_params_t *grid, int32_t method,
+                          float *out_xyzA_host, float *out_score_host, int64_t chunk_events);
+
+/* Release the model and its device memory.  NULL is a no-op. */
+void ants_destroy(ants_lrf_t *lrf);
+
+/* Static, NUL-terminated description of a status code. */
+const char *ants_strerror(int status);
+
+/* Number of reconstruction kernels this library has launched in this process
+ * (bench.py reports it as gpu_launches). */
+int64_t ants_launch_count(void);
+
+/*
+ * ants_plan_info -- host-only introspection of how a call would run (no GPU
+ * work): first iteration index that uses the differential score (K if none),
+ * nodes handled per lane, warps per CTA, CTAs per SM and dynamic shared-memory
+ * bytes per CTA.  Any output pointer may be NULL.  Errors as ants_reconstruct.
+ */
+int ants_plan_info(const ants_lrf_t *lrf, const ants_grid_params_t *grid, int32_t method,
+                   int32_t *first_diff_iter, int32_t *nodes_per_lane, int32_t *warps_per_cta,
+                   int32_t *ctas_per_sm, int32_t *smem_bytes);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ANTS_RECON_H */

@@ -326,3 +326,15 @@ int oracle_reconstruct(const oracle_model_t *m, const float *signals, int64_t n_
     }
     return 0;
 }
+
+/* score_at for many events: pos [E][3] double, A_out/score_out [E] (interface
+ * helper for the parity tests; the arithmetic is oracle_score_at's). */
+int oracle_score_at_many(const oracle_model_t *m, const float *signals, int64_t n_events, int method,
+                         const double *pos, double *A_out, double *score_out)
+{
+    if (!m || !signals || !pos || !A_out || !score_out || n_events < 0) return -1;
+    for (int64_t e = 0; e < n_events; ++e)
+        oracle_score_at(m, signals + e * m->n_sensors, method, pos[3 * e], pos[3 * e + 1], pos[3 * e + 2],
+                        A_out + e, score_out + e);
+    return 0;
+}

@@ -55,6 +55,9 @@ def _load():
         lib.oracle_score_at.restype = C.c_int
         lib.oracle_score_at.argtypes = [C.POINTER(_Model), C.c_void_p, C.c_int, C.c_double, C.c_double,
                                         C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        lib.oracle_score_at_many.restype = C.c_int
+        lib.oracle_score_at_many.argtypes = [C.POINTER(_Model), C.c_void_p, C.c_int64, C.c_int,
+                                             C.c_void_p, C.c_void_p, C.c_void_p]
         lib.oracle_threads.restype = C.c_int
         lib.oracle_threads.argtypes = [C.c_int]
         lib.oracle_reconstruct.restype = C.c_int
@@ -122,6 +125,19 @@ class Model:
         _load().oracle_score_at(C.byref(self.c), s.ctypes.data, int(method), float(x), float(y),
                                 float(z), C.byref(A), C.byref(sc))
         return A.value, sc.value
+
+
+def score_at_many(model: Model, signals, method: int, pos):
+    """(A [E], score [E]) of each event's signals at its own position pos [E][3]."""
+    s = _f32(signals).reshape(-1, model.n_sensors)
+    p = np.ascontiguousarray(np.asarray(pos, dtype=np.float64)).reshape(-1, 3)
+    assert p.shape[0] == s.shape[0]
+    A, sc = np.zeros(s.shape[0]), np.zeros(s.shape[0])
+    rc = _load().oracle_score_at_many(C.byref(model.c), s.ctypes.data, s.shape[0], int(method),
+                                      p.ctypes.data, A.ctypes.data, sc.ctypes.data)
+    if rc != 0:
+        raise ValueError("oracle_score_at_many: invalid argument")
+    return A, sc
 
 
 def grid_params(dim, nodes_per_axis, step0_xy, step0_z, factor, n_iter, z_seed=float("nan")):

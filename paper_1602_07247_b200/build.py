@@ -1,0 +1,38 @@
+"""Build the C-ABI CUDA library in-tree: paper_1602_07247_b200/libants_recon.so.
+
+nvcc cross-compiles for sm_100a without a GPU; cudart is linked statically so the
+library loads (and its symbols can be listed) on a CPU-only box.
+"""
+from __future__ import annotations
+
+import os
+import subprocess
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+SRC = os.path.join(_HERE, "csrc", "ants_recon.cu")
+DEPS = [os.path.join(_HERE, "csrc", f) for f in ("ants_recon.cu", "recon_common.cuh", "recon2d.cuh", "recon3d.cuh")]
+DEPS.append(os.path.join(os.path.dirname(_HERE), "include", "ants_recon.h"))
+LIB = os.path.join(_HERE, "libants_recon.so")
+
+NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
+              "-Xcompiler", "-fPIC", "-shared"]
+
+
+def nvcc() -> str:
+    cand = os.path.join(os.environ.get("CUDA_HOME", "/usr/local/cuda"), "bin", "nvcc")
+    return cand if os.path.exists(cand) else "nvcc"
+
+
+def build(force: bool = False, verbose: bool = False) -> str:
+    """Compile if the library is missing or older than its sources; returns its path."""
+    stale = force or not os.path.exists(LIB) or any(
+        os.path.getmtime(d) > os.path.getmtime(LIB) for d in DEPS if os.path.exists(d))
+    if stale:
+        cmd = [nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB, SRC]
+        subprocess.check_call(cmd)
+    return LIB
+
+
+if __name__ == "__main__":
+    import sys
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

@@ -1,0 +1,467 @@
+// ants_recon.cu -- C ABI (include/ants_recon.h) and host logic of the B200
+// contracting-grid reconstruction: table build (step a0), launch planning,
+// kernel dispatch, the streamed host-buffer pipeline.  No CPU fallback: every
+// reconstruction step runs in the kernels of recon2d.cuh / recon3d.cuh.
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <atomic>
+#include <mutex>
+#include <new>
+#include <vector>
+
+#include "../../include/ants_recon.h"
+#include "recon2d.cuh"
+#include "recon3d.cuh"
+
+using namespace ants;
+
+// ---------------------------------------------------------------------------
+// the opaque handle
+// ---------------------------------------------------------------------------
+struct ants_lrf {
+    ModelDev dev{};          // device pointers + scalars, passed by value to the kernels
+    int device = 0;
+    int sm_count = 0;
+    bool positive = false;   // every spline strictly positive on its domain
+    double max_dlog = 0.0;   // max |d ln s / dr| over the domain, 1/mm (only if positive)
+    double knot_r = 0.0, knot_z = 0.0;   // knot spacing, mm
+    void *d_sens = nullptr, *d_poly = nullptr, *d_polyd = nullptr;
+    // scratch of ants_reconstruct_host (lazily allocated, reused, guarded)
+    std::mutex host_mu;
+    int64_t scratch_events = 0;
+    float *d_sig[3] = {nullptr, nullptr, nullptr};
+    float *d_xyzA[3] = {nullptr, nullptr, nullptr};
+    float *d_score[3] = {nullptr, nullptr, nullptr};
+    cudaStream_t streams[3] = {nullptr, nullptr, nullptr};
+};
+
+static std::atomic<int64_t> g_launches{0};
+
+// ---------------------------------------------------------------------------
+// step a0: B-spline coefficients -> per-interval cubics
+// ---------------------------------------------------------------------------
+// Uniform cubic B-spline on interval k with local u in [0,1] (R7), power basis:
+//   s = p0 + p1 u + p2 u^2 + p3 u^3 from the four coefficients c[k..k+3].
+static void interval_power(const float *c, double p[4]) {
+    const double c0 = c[0], c1 = c[1], c2 = c[2], c3 = c[3];
+    p[0] = (c0 + 4.0 * c1 + c2) / 6.0;
+    p[1] = (c2 - c0) / 2.0;
+    p[2] = (c0 - 2.0 * c1 + c2) / 2.0;
+    p[3] = (c3 - c0 + 3.0 * (c1 - c2)) / 6.0;
+}
+
+// minimum of the cubic on [0,1] (end points and interior critical points)
+static double cubic_min01(const double p[4]) {
+    auto f = [&](double u) { return p[0] + u * (p[1] + u * (p[2] + u * p[3])); };
+    double mn = std::fmin(f(0.0), f(1.0));
+    const double a = 3.0 * p[3], b = 2.0 * p[2], c = p[1];
+    if (std::fabs(a) > 0.0) {
+        double disc = b * b - 4.0 * a * c;
+        if (disc >= 0.0) {
+            double sq = std::sqrt(disc);
+            for (double u : {(-b + sq) / (2.0 * a), (-b - sq) / (2.0 * a)})
+                if (u > 0.0 && u < 1.0) mn = std::fmin(mn, f(u));
+        }
+    } else if (std::fabs(b) > 0.0) {
+        double u = -c / b;
+        if (u > 0.0 && u < 1.0) mn = std::fmin(mn, f(u));
+    }
+    return mn;
+}
+
+// one r-spline (n_r + 3 coefficients) -> fp32 centred rows [n_r + 1] and fp64 rows [n_r][4];
+// updates positivity and the log-derivative bound
+static void build_rows(const float *c, int n_r, double sc_r, float4 *rows32, double *rows64,
+                       bool &positive, double &max_dlog) {
+    double last[4] = {0, 0, 0, 0};
+    for (int k = 0; k < n_r; ++k) {
+        double p[4];
+        interval_power(c + k, p);
+        for (int a = 0; a < 4; ++a) rows64[4 * k + a] = p[a];
+        // re-centre to v = u - 1/2
+        rows32[k] = make_float4((float)(p[0] + 0.5 * p[1] + 0.25 * p[2] + 0.125 * p[3]),
+                                (float)(p[1] + p[2] + 0.75 * p[3]), (float)(p[2] + 1.5 * p[3]), (float)p[3]);
+        if (!(cubic_min01(p) > 0.0)) positive = false;
+        for (int s = 0; s <= 16; ++s) {
+            double u = s / 16.0;
+            double f = p[0] + u * (p[1] + u * (p[2] + u * p[3]));
+            double d = p[1] + u * (2.0 * p[2] + 3.0 * u * p[3]);
+            if (f > 0.0) max_dlog = std::fmax(max_dlog, std::fabs(d) * sc_r / f);
+        }
+        for (int a = 0; a < 4; ++a) last[a] = p[a];
+    }
+    // row n_r: constant extension s(r_hi) (R5)
+    rows32[n_r] = make_float4((float)(last[0] + last[1] + last[2] + last[3]), 0.f, 0.f, 0.f);
+}
+
+static bool finite_f(float v) { return std::isfinite(v); }
+
+extern "C" int ants_lrf_create(const float *sensor_xy, const float *gains, const float *knots,
+                               const float *coeffs, const ants_lrf_dims_t *dims, ants_lrf_t **out) {
+    if (!out) return ANTS_ERR_INVALID;
+    *out = nullptr;
+    if (!sensor_xy || !knots || !coeffs || !dims) return ANTS_ERR_INVALID;
+    const int N = dims->n_sensors, n_lrf = dims->n_lrf, dim = dims->lrf_dim, n_r = dims->n_int_r;
+    const int n_z = dim == 2 ? dims->n_int_z : 0;
+    if (N < 1 || N > 65535 || (dim != 1 && dim != 2) || n_r < 1 || n_r > 4096) return ANTS_ERR_INVALID;
+    if (n_lrf != 1 && n_lrf != N) return ANTS_ERR_INVALID;
+    if (dim == 2 && (n_z < 1 || n_z > 1024)) return ANTS_ERR_INVALID;
+    const float r_lo = knots[0], r_hi = knots[1];
+    if (!finite_f(r_lo) || !finite_f(r_hi) || !(r_lo >= 0.f) || !(r_hi > r_lo)) return ANTS_ERR_INVALID;
+    float z_lo = 0.f, z_hi = 1.f;
+    if (dim == 2) {
+        z_lo = knots[2];
+        z_hi = knots[3];
+        if (!finite_f(z_lo) || !finite_f(z_hi) || !(z_hi > z_lo)) return ANTS_ERR_INVALID;
+    }
+    for (int i = 0; i < N; ++i) {
+        if (!finite_f(sensor_xy[2 * i]) || !finite_f(sensor_xy[2 * i + 1])) return ANTS_ERR_INVALID;
+        if (gains && !(gains[i] > 0.f && finite_f(gains[i]))) return ANTS_ERR_INVALID;
+    }
+    const int n_rows_z = dim == 2 ? n_z + 3 : 1;
+    const size_t n_coef = (size_t)n_lrf * n_rows_z * (n_r + 3);
+    for (size_t j = 0; j < n_coef; ++j)
+        if (!finite_f(coeffs[j])) return ANTS_ERR_INVALID;
+    if (dim == 2 && n_lrf != 1) return ANTS_ERR_UNSUPPORTED;
+
+    ants_lrf *h = new (std::nothrow) ants_lrf;
+    if (!h) return ANTS_ERR_NOMEM;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&h->device) != cudaSuccess ||
+        cudaGetDeviceProperties(&prop, h->device) != cudaSuccess) {
+        delete h;
+        return ANTS_ERR_CUDA;
+    }
+    h->sm_count = prop.multiProcessorCount;
+
+    const size_t n_spl = (size_t)n_lrf * n_rows_z;   // r-splines in the table
+    std::vector<float4> sens(N), rows32(n_spl * (n_r + 1));
+    std::vector<double> rows64(n_spl * n_r * 4);
+    for (int i = 0; i < N; ++i) {
+        float g = gains ? gains[i] : 1.f;
+        sens[i] = make_float4(sensor_xy[2 * i], sensor_xy[2 * i + 1], g, 1.f / g);
+    }
+    const double sc_r = (double)n_r / ((double)r_hi - (double)r_lo);
+    bool positive = true;
+    double max_dlog = 0.0;
+    for (size_t s = 0; s < n_spl; ++s)
+        build_rows(coeffs + s * (n_r + 3), n_r, sc_r, rows32.data() + s * (n_r + 1),
+                   rows64.data() + s * n_r * 4, positive, max_dlog);
+    if (dim == 2) {
+        // positivity / slope of the tensor product: sufficient test on the coefficients
+        // (all > 0 => s > 0 by the convex-hull property); the differential 3-D score needs it
+        positive = true;
+        for (size_t j = 0; j < n_coef; ++j)
+            if (!(coeffs[j] > 0.f)) positive = false;
+    }
+    h->positive = positive;
+    h->max_dlog = max_dlog;
+    h->knot_r = 1.0 / sc_r;
+    h->knot_z = dim == 2 ? ((double)z_hi - (double)z_lo) / n_z : 0.0;
+
+    cudaError_t e1 = cudaMalloc(&h->d_sens, sens.size() * sizeof(float4));
+    cudaError_t e2 = cudaMalloc(&h->d_poly, rows32.size() * sizeof(float4));
+    cudaError_t e3 = cudaMalloc(&h->d_polyd, rows64.size() * sizeof(double));
+    if (e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess) {
+        cudaGetLastError();
+        ants_destroy(h);
+        return (e1 == cudaErrorMemoryAllocation || e2 == cudaErrorMemoryAllocation ||
+                e3 == cudaErrorMemoryAllocation) ? ANTS_ERR_NOMEM : ANTS_ERR_CUDA;
+    }
+    if (cudaMemcpy(h->d_sens, sens.data(), sens.size() * sizeof(float4), cudaMemcpyHostToDevice) != cudaSuccess ||
+        cudaMemcpy(h->d_poly, rows32.data(), rows32.size() * sizeof(float4), cudaMemcpyHostToDevice) != cudaSuccess ||
+        cudaMemcpy(h->d_polyd, rows64.data(), rows64.size() * sizeof(double), cudaMemcpyHostToDevice) != cudaSuccess) {
+        cudaGetLastError();
+        ants_destroy(h);
+        return ANTS_ERR_CUDA;
+    }
+    ModelDev &m = h->dev;
+    m.sens = (const float4 *)h->d_sens;
+    m.poly = (const float4 *)h->d_poly;
+    m.polyd = (const double *)h->d_polyd;
+    m.N = N;
+    m.n_lrf = n_lrf;
+    m.n_r = n_r;
+    m.n_z = n_z;
+    m.r_lo = r_lo;
+    m.r_hi = r_hi;
+    m.sc = (float)sc_r;
+    m.of = (float)(-(double)r_lo * sc_r - 0.5);
+    m.tmax = (float)n_r - 0.5f;
+    m.z_lo = z_lo;
+    m.z_hi = z_hi;
+    m.scz = dim == 2 ? (float)((double)n_z / ((double)z_hi - (double)z_lo)) : 0.f;
+    *out = h;
+    return ANTS_OK;
+}
+
+extern "C" void ants_destroy(ants_lrf_t *h) {
+    if (!h) return;
+    cudaFree(h->d_sens);
+    cudaFree(h->d_poly);
+    cudaFree(h->d_polyd);
+    for (int s = 0; s < 3; ++s) {
+        cudaFree(h->d_sig[s]);
+        cudaFree(h->d_xyzA[s]);
+        cudaFree(h->d_score[s]);
+        if (h->streams[s]) cudaStreamDestroy(h->streams[s]);
+    }
+    cudaGetLastError();
+    delete h;
+}
+
+extern "C" const char *ants_strerror(int status) {
+    switch (status) {
+        case ANTS_OK: return "ok";
+        case ANTS_ERR_INVALID: return "invalid argument";
+        case ANTS_ERR_UNSUPPORTED: return "unsupported combination or size";
+        case ANTS_ERR_CUDA: return "CUDA runtime error";
+        case ANTS_ERR_NOMEM: return "out of memory";
+        default: return "unknown status";
+    }
+}
+
+extern "C" int64_t ants_launch_count(void) { return g_launches.load(); }
+
+// ---------------------------------------------------------------------------
+// launch planning
+// ---------------------------------------------------------------------------
+struct Plan {
+    int npt = 0;             // nodes per lane (template instantiation)
+    int warps = 0;           // warps per CTA
+    int ctas_per_sm = 0;
+    size_t smem = 0;         // dynamic shared memory per CTA
+    int k_diff = 0;          // first differential iteration (K = never)
+    const void *kernel = nullptr;
+};
+
+static const int kNpt2D[] = {1, 2, 3, 4, 8};
+static const double kQSeries = 0.1;   // |dL/L0| bound under which the degree-6 log1p series is used
+
+template <int METHOD, bool POS>
+static const void *pick2d(int npt) {
+    switch (npt) {
+        case 1: return (const void *)recon2d_kernel<1, METHOD, POS>;
+        case 2: return (const void *)recon2d_kernel<2, METHOD, POS>;
+        case 3: return (const void *)recon2d_kernel<3, METHOD, POS>;
+        case 4: return (const void *)recon2d_kernel<4, METHOD, POS>;
+        case 8: return (const void *)recon2d_kernel<8, METHOD, POS>;
+    }
+    return nullptr;
+}
+
+static int validate_grid(const ants_lrf *h, const ants_grid_params_t *g, int32_t method) {
+    if (!h || !g) return ANTS_ERR_INVALID;
+    if (method != ANTS_POISSON_ML && method != ANTS_CHI_SQUARE) return ANTS_ERR_INVALID;
+    if (g->dim != 2 && g->dim != 3) return ANTS_ERR_INVALID;
+    if (g->nodes_per_axis < 2 || g->n_iter < 1 || g->n_iter > 4096) return ANTS_ERR_INVALID;
+    if (!(g->factor > 0.f && g->factor < 1.f)) return ANTS_ERR_INVALID;
+    if (!(g->step0_xy > 0.f) || !std::isfinite(g->step0_xy)) return ANTS_ERR_INVALID;
+    if (g->seed_mode != 0) return ANTS_ERR_INVALID;
+    const bool lrf3 = h->dev.n_z > 0;
+    if (g->dim == 3) {
+        if (!lrf3) return ANTS_ERR_INVALID;
+        if (!(g->step0_z > 0.f) || !std::isfinite(g->step0_z)) return ANTS_ERR_INVALID;
+    }
+    if (lrf3 && !std::isnan(g->z_seed) && !std::isfinite(g->z_seed)) return ANTS_ERR_INVALID;
+    return ANTS_OK;
+}
+
+// first iteration k whose grid is small enough for the differential score:
+// every node within one knot interval of the centre (at most one knot crossed per
+// axis) and, for Poisson, |dL/L0| <= exp(max|dlnL/dr| reach) - 1 <= kQSeries.
+static int first_diff_iter(const ants_lrf *h, const ants_grid_params_t *g, int32_t method) {
+    if (!h->positive) return g->n_iter;
+    const double half = 0.5 * (g->nodes_per_axis - 1);
+    double hxy = g->step0_xy, hz = g->step0_z;
+    for (int k = 0; k < g->n_iter; ++k, hxy *= (double)g->factor, hz *= (double)g->factor) {
+        double reach = std::sqrt(2.0) * half * hxy * 1.001;
+        bool ok = reach <= 0.9 * h->knot_r;
+        if (g->dim == 3) ok = ok && (half * hz * 1.001 <= 0.9 * h->knot_z);
+        if (method == ANTS_POISSON_ML) {
+            double bound = std::expm1(h->max_dlog * reach);
+            if (g->dim == 3) bound = 1e9;   // 3-D decides by its own rule in make_plan3d
+            ok = ok && (bound <= kQSeries || g->dim == 3);
+        }
+        if (ok) return k;
+    }
+    return g->n_iter;
+}
+
+static int make_plan(const ants_lrf *h, const ants_grid_params_t *g, int32_t method, Plan &pl) {
+    int rc = validate_grid(h, g, method);
+    if (rc != ANTS_OK) return rc;
+    const ModelDev &m = h->dev;
+    if (g->dim == 3 || m.n_z > 0) return make_plan3d(h->positive, h->knot_r, h->knot_z, h->max_dlog, m, g, method,
+                                                    pl.npt, pl.warps, pl.ctas_per_sm, pl.smem, pl.k_diff, pl.kernel);
+    const long long nodes = (long long)g->nodes_per_axis * g->nodes_per_axis;
+    if (nodes > 256) return ANTS_ERR_UNSUPPORTED;
+    int need = (int)((nodes + 31) / 32);
+    pl.npt = 0;
+    for (int c : kNpt2D)
+        if (c >= need) { pl.npt = c; break; }
+    if (!pl.npt) return ANTS_ERR_UNSUPPORTED;
+    if (method == ANTS_POISSON_ML)
+        pl.kernel = h->positive ? pick2d<0, true>(pl.npt) : pick2d<0, false>(pl.npt);
+    else
+        pl.kernel = h->positive ? pick2d<1, true>(pl.npt) : pick2d<1, false>(pl.npt);
+    pl.k_diff = first_diff_iter(h, g, method);
+    const size_t tables = (size_t)(m.N + m.n_lrf * (m.n_r + 1)) * 16;
+    const size_t per_warp = warp_smem_bytes_2d(m.N);
+    const size_t budget = 227 * 1024;
+    pl.warps = 8;
+    while (pl.warps > 1 && tables + pl.warps * per_warp > budget / 2) pl.warps >>= 1;
+    pl.smem = tables + pl.warps * per_warp;
+    if (pl.smem > budget) return ANTS_ERR_UNSUPPORTED;
+    pl.ctas_per_sm = (int)std::min<size_t>(budget / (pl.smem + 1024), (size_t)(2048 / (pl.warps * 32)));
+    if (pl.ctas_per_sm < 1) pl.ctas_per_sm = 1;
+    return ANTS_OK;
+}
+
+extern "C" int ants_plan_info(const ants_lrf_t *lrf, const ants_grid_params_t *grid, int32_t method,
+                              int32_t *first_diff, int32_t *nodes_per_lane, int32_t *warps_per_cta,
+                              int32_t *ctas_per_sm, int32_t *smem_bytes) {
+    Plan pl;
+    int rc = make_plan(lrf, grid, method, pl);
+    if (rc != ANTS_OK) return rc;
+    if (first_diff) *first_diff = pl.k_diff;
+    if (nodes_per_lane) *nodes_per_lane = pl.npt;
+    if (warps_per_cta) *warps_per_cta = pl.warps;
+    if (ctas_per_sm) *ctas_per_sm = pl.ctas_per_sm;
+    if (smem_bytes) *smem_bytes = (int32_t)pl.smem;
+    return ANTS_OK;
+}
+
+// ---------------------------------------------------------------------------
+// dispatch: one kernel launch per call
+// ---------------------------------------------------------------------------
+static int launch(const ants_lrf *h, const float *signals, int64_t n_events, const ants_grid_params_t *g,
+                  int32_t method, float *out_xyzA, float *out_score, uint16_t *out_path, cudaStream_t stream) {
+    Plan pl;
+    int rc = make_plan(h, g, method, pl);
+    if (rc != ANTS_OK) return rc;
+    if (n_events < 0) return ANTS_ERR_INVALID;
+    if (n_events == 0) return ANTS_OK;
+    if (!signals || !out_xyzA || !out_score) return ANTS_ERR_INVALID;
+    if (g->n_iter > 65535) return ANTS_ERR_INVALID;
+
+    Params p{};
+    p.m = h->dev;
+    p.signals = signals;
+    p.n_events = n_events;
+    p.out_xyzA = out_xyzA;
+    p.out_score = out_score;
+    p.out_path = out_path;
+    p.G = g->nodes_per_axis;
+    p.K = g->n_iter;
+    p.nodes = g->dim == 3 ? p.G * p.G * p.G : p.G * p.G;
+    p.k_diff = pl.k_diff;
+    p.h0_xy = g->step0_xy;
+    p.h0_z = g->dim == 3 ? g->step0_z : 0.f;
+    p.factor = g->factor;
+    p.z_seed = g->z_seed;
+    p.dim = g->dim;
+    p.warps_per_cta = pl.warps;
+    p.tile_events = pl.warps;
+
+    if (cudaFuncSetAttribute(pl.kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem) != cudaSuccess) {
+        cudaGetLastError();
+        return ANTS_ERR_CUDA;
+    }
+    int occ = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pl.kernel, pl.warps * 32, pl.smem) != cudaSuccess ||
+        occ < 1) {
+        cudaGetLastError();
+        return ANTS_ERR_CUDA;
+    }
+    long long want = (n_events + pl.warps - 1) / pl.warps;
+    long long cap = (long long)h->sm_count * occ;
+    int grid = (int)std::min(want, cap);
+    void *args[] = {&p};
+    if (cudaLaunchKernel(pl.kernel, dim3(grid), dim3(pl.warps * 32), args, pl.smem, stream) != cudaSuccess) {
+        cudaGetLastError();
+        return ANTS_ERR_CUDA;
+    }
+    g_launches.fetch_add(1);
+    return ANTS_OK;
+}
+
+extern "C" int ants_reconstruct(const ants_lrf_t *lrf, const float *signals, int64_t n_events,
+                                const ants_grid_params_t *grid, int32_t method, float *out_xyzA,
+                                float *out_score, void *cuda_stream) {
+    return launch(lrf, signals, n_events, grid, method, out_xyzA, out_score, nullptr, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int ants_reconstruct_trace(const ants_lrf_t *lrf, const float *signals, int64_t n_events,
+                                      const ants_grid_params_t *grid, int32_t method, float *out_xyzA,
+                                      float *out_score, uint16_t *out_path, void *cuda_stream) {
+    if (n_events > 0 && !out_path) return ANTS_ERR_INVALID;
+    return launch(lrf, signals, n_events, grid, method, out_xyzA, out_score, out_path, (cudaStream_t)cuda_stream);
+}
+
+// ---------------------------------------------------------------------------
+// host-buffer pipeline: chunks on a ring of three streams (H2D, kernel, D2H overlap)
+// ---------------------------------------------------------------------------
+static int ensure_scratch(ants_lrf *h, int64_t chunk) {
+    if (h->scratch_events >= chunk) return ANTS_OK;
+    const int N = h->dev.N;
+    for (int s = 0; s < 3; ++s) {
+        cudaFree(h->d_sig[s]);
+        cudaFree(h->d_xyzA[s]);
+        cudaFree(h->d_score[s]);
+        h->d_sig[s] = h->d_xyzA[s] = h->d_score[s] = nullptr;
+    }
+    h->scratch_events = 0;
+    for (int s = 0; s < 3; ++s) {
+        if (!h->streams[s] && cudaStreamCreateWithFlags(&h->streams[s], cudaStreamNonBlocking) != cudaSuccess) {
+            cudaGetLastError();
+            return ANTS_ERR_CUDA;
+        }
+        if (cudaMalloc(&h->d_sig[s], (size_t)chunk * N * sizeof(float)) != cudaSuccess ||
+            cudaMalloc(&h->d_xyzA[s], (size_t)chunk * 4 * sizeof(float)) != cudaSuccess ||
+            cudaMalloc(&h->d_score[s], (size_t)chunk * sizeof(float)) != cudaSuccess) {
+            cudaGetLastError();
+            return ANTS_ERR_NOMEM;
+        }
+    }
+    h->scratch_events = chunk;
+    return ANTS_OK;
+}
+
+extern "C" int ants_reconstruct_host(const ants_lrf_t *lrf, const float *signals_host, int64_t n_events,
+                                     const ants_grid_params_t *grid, int32_t method, float *out_xyzA_host,
+                                     float *out_score_host, int64_t chunk_events) {
+    Plan pl;
+    int rc = make_plan(lrf, grid, method, pl);
+    if (rc != ANTS_OK) return rc;
+    if (n_events < 0) return ANTS_ERR_INVALID;
+    if (n_events == 0) return ANTS_OK;
+    if (!signals_host || !out_xyzA_host || !out_score_host) return ANTS_ERR_INVALID;
+    ants_lrf *h = const_cast<ants_lrf *>(lrf);
+    std::lock_guard<std::mutex> lock(h->host_mu);
+    int64_t chunk = chunk_events > 0 ? chunk_events : (int64_t)1 << 20;
+    chunk = std::min(chunk, n_events);
+    rc = ensure_scratch(h, chunk);
+    if (rc != ANTS_OK) return rc;
+    const int N = h->dev.N;
+    int slot = 0;
+    for (int64_t a = 0; a < n_events; a += chunk, slot = (slot + 1) % 3) {
+        const int64_t n = std::min(chunk, n_events - a);
+        cudaStream_t st = h->streams[slot];
+        // the stream order makes the slot's buffers safe to reuse: the previous
+        // occupant's D2H copy is ahead of this H2D copy on the same stream
+        if (cudaMemcpyAsync(h->d_sig[slot], signals_host + a * N, (size_t)n * N * sizeof(float),
+                            cudaMemcpyHostToDevice, st) != cudaSuccess) { cudaGetLastError(); return ANTS_ERR_CUDA; }
+        rc = launch(h, h->d_sig[slot], n, grid, method, h->d_xyzA[slot], h->d_score[slot], nullptr, st);
+        if (rc != ANTS_OK) return rc;
+        if (cudaMemcpyAsync(out_xyzA_host + a * 4, h->d_xyzA[slot], (size_t)n * 4 * sizeof(float),
+                            cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+            cudaMemcpyAsync(out_score_host + a, h->d_score[slot], (size_t)n * sizeof(float),
+                            cudaMemcpyDeviceToHost, st) != cudaSuccess) { cudaGetLastError(); return ANTS_ERR_CUDA; }
+    }
+    for (int s = 0; s < 3; ++s)
+        if (cudaStreamSynchronize(h->streams[s]) != cudaSuccess) { cudaGetLastError(); return ANTS_ERR_CUDA; }
+    return ANTS_OK;
+}

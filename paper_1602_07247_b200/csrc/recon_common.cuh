@@ -1,0 +1,93 @@
+// recon_common.cuh -- device-side parameter blocks and small helpers shared by
+// the 2-D and 3-D contracting-grid kernels (section 5.1.2.2).
+// Product code: shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace ants {
+
+constexpr unsigned kFull = 0xffffffffu;
+constexpr float kMagic = 12582912.0f;     // 1.5 * 2^23: (t + kMagic) rounds t to the nearest integer
+constexpr int kMagicBits = 0x4B400000;    // bit pattern of kMagic; low bits of (t + kMagic) hold round(t)
+#define kInf (__int_as_float(0x7f800000))
+
+// LRF model as the kernels see it (device pointers; built once in ants_lrf_create, step a0).
+struct ModelDev {
+    const float4 *sens;     // [N] {X, Y, g, 1/g}
+    const float4 *poly;     // axial: [n_lrf][n_r + 1] rows {q0,q1,q2,q3}: s = q0 + v(q1 + v(q2 + v q3)),
+                            //   v = t - round(t - 0.5) - 0.5 in [-0.5, 0.5], t = (r - r_lo) * sc;
+                            //   row n_r is the constant extension s(r_hi).
+                            // axial+z: [n_z + 3][n_r + 1] such rows, one r-spline per z coefficient row
+    const double *polyd;    // axial: [n_lrf][n_r][4] power basis in u = t - k in [0,1] (final score, FP64)
+                            // axial+z: [n_z + 3][n_r][4]
+    int N, n_lrf, n_r, n_z;
+    float r_lo, r_hi, sc, of, tmax;   // sc = n_r/(r_hi - r_lo); of = -r_lo*sc - 0.5; tmax = n_r - 0.5
+    float z_lo, z_hi, scz;            // scz = n_z/(z_hi - z_lo)
+};
+
+struct Params {
+    ModelDev m;
+    const float *signals;   // [E][N]
+    long long n_events;
+    float *out_xyzA;        // [E][4]
+    float *out_score;       // [E]
+    uint16_t *out_path;     // [E][K] or nullptr
+    int G, K, nodes, dim;   // nodes = G^dim
+    int k_diff;             // first iteration scored differentially (K = never)
+    float h0_xy, h0_z, factor, z_seed;
+    int warps_per_cta;
+    int tile_events;        // events staged per CTA tile (= warps_per_cta)
+};
+
+__device__ __forceinline__ float sqrt_approx(float x) {
+    float y;
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float rcp_approx(float x) {
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float lg2_approx(float x) {
+    float y;
+    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
+    return v;
+}
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
+    return v;
+}
+
+// argmin over the warp of (score, index); ties go to the lower index (R9).  All lanes get the result.
+__device__ __forceinline__ void warp_argmin(float &s, int &idx) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        float os = __shfl_xor_sync(kFull, s, o);
+        int oi = __shfl_xor_sync(kFull, idx, o);
+        bool take = (os < s) || (os == s && oi < idx);
+        s = take ? os : s;
+        idx = take ? oi : idx;
+    }
+}
+
+// round-to-nearest interval index k and centred local coordinate v of t in [-0.5, tmax]
+__device__ __forceinline__ void split_t(float t, int &k, float &v) {
+    float tm = t + kMagic;
+    k = __float_as_int(tm) - kMagicBits;
+    v = t - (tm - kMagic);
+}
+
+__device__ __forceinline__ float horner(const float4 p, float v) {
+    return fmaf(fmaf(fmaf(p.w, v, p.z), v, p.y), v, p.x);
+}
+
+}  // namespace ants

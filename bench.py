@@ -1,0 +1,355 @@
+#!/usr/bin/env python
+"""bench.py -- events/s of the contracting-grid reconstruction on B200 (BASELINE.json metric).
+
+One "step" = one pass of the whole hot path (load, centroid seed,
+K grid iterations of LRF evaluation + energy + score + argmin, store) over one batch of seeded
+synthetic flood-field events = ONE kernel launch through the C ABI (ants_reconstruct).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl ours|reference]
+
+Prints ONE JSON line (rank 0).  `value` is device-resident throughput (CUDA events on the
+launching stream, L2 flushed between steps, max over ranks); `e2e` is the same metric through
+ants_reconstruct_host with pinned HOST buffers (H2D and D2H inside the timed region);
+`roofline` is the FP32-ALU roofline of the one kernel; `cpu_baseline` is the double-precision
+oracle (oracle/, test infrastructure) timed on this box's host cores on a bounded sample.
+`--impl reference` times that oracle as the reference arm (there is no reference code: the
+paper ships none).
+
+Multi-GPU (torchrun, one process per GPU): events are independent and the path has no exchange
+step, so every rank reconstructs its own seeded batch -- replicas, weak scaling, no collective
+on the data path; only the timing is reduced (max over ranks).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "events/sec reconstructed on 1 B200; achieved % of FP32 peak"
+UNIT = "events/s"
+
+# nominal algorithmic flop per (node, sensor) pair:
+# FMA = 2, sqrt / log / div = 1; every one of the K * G^d * N evaluations counts.
+FLOP_PER_PAIR = {"axial_poisson": 20.0, "axial_chi2": 25.0, "axialz_poisson": 35.0}
+FP32_LANES_PER_SM = 128          # B200 SM: 4 sub-partitions x 32 FP32 lanes, 1 FMA/lane/clk
+
+
+def flop_per_pair(cfg) -> float:
+    if cfg.lrf_dim == 2:
+        return FLOP_PER_PAIR["axialz_poisson"]
+    return FLOP_PER_PAIR["axial_chi2" if cfg.method == 1 else "axial_poisson"]
+
+
+# ---------------------------------------------------------------------------
+# clocks during the timed region (NVML; the recipe's clocks line)
+# ---------------------------------------------------------------------------
+class ClockSampler:
+    REASONS = {0x1: "gpu_idle", 0x2: "applications_clocks_setting", 0x4: "sw_power_cap", 0x8: "hw_slowdown",
+               0x10: "sync_boost", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+               0x80: "hw_power_brake_slowdown", 0x100: "display_clock_setting"}
+
+    def __init__(self, index: int, period: float = 0.05):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thr = None
+        self.period = period
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            phys = index
+            if vis:
+                try:
+                    phys = int(vis.split(",")[index])
+                except (ValueError, IndexError):
+                    phys = index
+            self.nv, self.h = pynvml, pynvml.nvmlDeviceGetHandleByIndex(phys)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self.nv = None
+
+    def _loop(self):
+        while not self._stop.is_set():
+            try:
+                self.samples.append(float(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM)))
+                mask = int(self.nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                for bit, name in self.REASONS.items():
+                    if mask & bit and name != "gpu_idle":
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            self._stop.wait(self.period)
+
+    def __enter__(self):
+        if self.nv is not None:
+            self._thr = threading.Thread(target=self._loop, daemon=True)
+            self._thr.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._thr is not None:
+            self._thr.join()
+
+    def summary(self) -> dict:
+        med = statistics.median(self.samples) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+# ---------------------------------------------------------------------------
+# helpers shared by the arms (host logic; covered by the gloo test)
+# ---------------------------------------------------------------------------
+def dist_env():
+    return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+
+
+def rank_batch(rank: int, step: int, n_resident: int) -> int:
+    """Which resident batch a rank reconstructs at a step (rotates so that inputs exceed L2)."""
+    return (step + rank) % max(n_resident, 1)
+
+
+def rank_seed_batch(rank: int, j: int, n_resident: int) -> int:
+    """Sub-stream id of resident batch j on a rank: ranks never share events (replicas of the
+    path, distinct data)."""
+    return rank * n_resident + j
+
+
+def max_over_ranks(local_ms: float, dist, device) -> float:
+    """Timing reduction: the slowest rank defines the job's time."""
+    import torch
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return float(local_ms)
+    t = torch.tensor([local_ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def sum_over_ranks(v: float, dist, device) -> float:
+    import torch
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return float(v)
+    t = torch.tensor([v], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    return float(t.item())
+
+
+def oracle_rate(cfg, signals_np, budget_s: float, threads: int = 0):
+    """Time the oracle, as it stands, on a bounded sample: calibrate on a small slice, then run
+    as many of the leading events as fit in ~budget_s.  Returns (events/s, n_events, threads)."""
+    from oracle import oracle
+    model = oracle.Model.from_config(cfg)
+    grid = oracle.grid_from_config(cfg)
+    used = oracle.n_threads(threads)
+    n0 = min(len(signals_np), max(64, 8 * used))
+    t0 = time.perf_counter()
+    oracle.reconstruct(model, signals_np[:n0], grid, cfg.method, threads=threads)
+    t1 = time.perf_counter() - t0
+    n = int(min(len(signals_np), max(n0, n0 * budget_s / max(t1, 1e-6))))
+    t0 = time.perf_counter()
+    oracle.reconstruct(model, signals_np[:n], grid, cfg.method, threads=threads)
+    dt = time.perf_counter() - t0
+    return n / dt, n, used
+
+
+# ---------------------------------------------------------------------------
+# reference arm = the oracle on host cores (rank 0 only)
+# ---------------------------------------------------------------------------
+def run_reference(args):
+    rank, _, world = dist_env()
+    if rank != 0:
+        return 0
+    from paper_1602_07247_b200 import synth
+    cfg = synth.make_config(args.config)
+    from oracle import oracle
+    model = oracle.Model.from_config(cfg)
+    grid = oracle.grid_from_config(cfg)
+    used = oracle.n_threads(0)
+    # bounded sample per step: sized from a calibration slice so that one step takes ~step_s
+    pool = synth.generate_events(cfg, min(cfg.n_events // cfg.n_batches, 262_144), device="cpu")["signals"].numpy()
+    n0 = max(64, 8 * used)
+    t0 = time.perf_counter()
+    oracle.reconstruct(model, pool[:n0], grid, cfg.method)
+    per_ev = (time.perf_counter() - t0) / n0
+    n = int(max(n0, min(len(pool), args.ref_step_seconds / per_ev)))
+    for _ in range(args.warmup):
+        oracle.reconstruct(model, pool[:n], grid, cfg.method)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.reconstruct(model, pool[:n], grid, cfg.method)
+    dt = time.perf_counter() - t0
+    value = n * args.steps / dt
+    sample = f"first {n} events of the seeded {cfg.name} flood field per step, {args.steps} steps"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": workload_config(cfg, n, 1),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": used, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def workload_config(cfg, events_per_step: int, n_gpus: int) -> dict:
+    return {"workload": cfg.name, "events_per_step_per_gpu": int(events_per_step), "n_sensors": cfg.n_sensors,
+            "grid": "x".join([str(cfg.nodes_per_axis)] * cfg.dim), "n_iter": cfg.n_iter,
+            "method": "poisson_ml" if cfg.method == 0 else "chi_square",
+            "pairs_per_event": cfg.pairs_per_event, "parallelism": f"replicas x{n_gpus} (no collective)",
+            "l2": "256 MiB scratch write between timed steps; resident batches rotate"}
+
+
+# ---------------------------------------------------------------------------
+# our arm
+# ---------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    rank, local_rank, world = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    device = torch.device("cuda", local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=device)
+    from paper_1602_07247_b200 import recon, synth
+    recon.load()
+
+    cfg = synth.make_config(args.config)
+    E = cfg.n_events // cfg.n_batches if args.events is None else args.events
+    cfg_run = cfg
+    n_resident = max(2, cfg.n_batches) if args.resident is None else args.resident
+    r = recon.Reconstructor(cfg_run)
+    sigs = [synth.generate_events(cfg, E, device=device, batch=rank_seed_batch(rank, j, n_resident))["signals"]
+            for j in range(n_resident)]
+    xyzA = torch.empty((E, 4), dtype=torch.float32, device=device)
+    score = torch.empty((E,), dtype=torch.float32, device=device)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=device)
+    stream = torch.cuda.current_stream()
+
+    def one(step):
+        recon.ants_reconstruct(r.handle, sigs[rank_batch(rank, step, n_resident)], r.grid, r.method, xyzA, score,
+                               stream.cuda_stream)
+
+    for s in range(args.warmup):
+        one(s)
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    launches0 = recon.launch_count()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    sampler = ClockSampler(local_rank)
+    torch.cuda.synchronize()
+    with sampler:
+        for s in range(args.steps):
+            flush.fill_(s & 0xFF)                 # evict L2 (126 MB) between timed steps
+            ev[s][0].record(stream)
+            one(args.warmup + s)
+            ev[s][1].record(stream)
+        torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    gpu_launches = recon.launch_count() - launches0
+    local_ms = sum(step_ms)
+    total_ms = max_over_ranks(local_ms, dist, device)
+    total_events = sum_over_ranks(float(E * args.steps), dist, device)
+    value = total_events / (total_ms * 1e-3)
+
+    # ---- end to end: pinned host buffers through ants_reconstruct_host -----------------------
+    sig_h = sigs[0].cpu().pin_memory()
+    xyzA_h = torch.empty((E, 4), dtype=torch.float32).pin_memory()
+    score_h = torch.empty((E,), dtype=torch.float32).pin_memory()
+    chunk = max(1, min(E, args.e2e_chunk))
+    for _ in range(2):
+        recon.ants_reconstruct_host(r.handle, sig_h, r.grid, r.method, xyzA_h, score_h, chunk)
+    if dist is not None:
+        dist.barrier()
+    e2e_steps = max(1, min(args.steps, 5))
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        recon.ants_reconstruct_host(r.handle, sig_h, r.grid, r.method, xyzA_h, score_h, chunk)
+    e2e_ms = (time.perf_counter() - t0) * 1e3
+    e2e_ms = max_over_ranks(e2e_ms, dist, device)
+    e2e_value = sum_over_ranks(float(E * e2e_steps), dist, device) / (e2e_ms * 1e-3)
+    assert torch.equal(xyzA_h[:1024].to(device), r(sigs[0][:1024].contiguous())[0])   # same kernel, same bits
+
+    # ---- roofline of the one kernel (FP32 ALU bound) --------------------
+    prop = torch.cuda.get_device_properties(device)
+    clocks = sampler.summary()
+    max_mhz = clocks["sm_max_mhz"] or 1965.0
+    peak_tflops = prop.multi_processor_count * FP32_LANES_PER_SM * 2 * max_mhz * 1e6 / 1e12
+    launch_ms = local_ms / max(gpu_launches, 1)
+    flops_per_launch = flop_per_pair(cfg) * cfg.pairs_per_event * E
+    achieved = flops_per_launch / (launch_ms * 1e-3) / 1e12
+    roofline = {"bound": "alu", "kernel": "ants::recon%dd_kernel" % cfg.dim, "achieved": achieved, "peak": peak_tflops,
+                "unit": "TFLOP/s", "frac": achieved / peak_tflops, "traffic": TRAFFIC_BYTES.get(cfg.name),
+                "peak_source": "derived: SMs x 128 FP32 lanes x 2 x clocks.max.sm (MEASURED_PEAKS.json has no FP32 entry)",
+                "flop_per_pair_nominal": flop_per_pair(cfg), "pairs_per_s": cfg.pairs_per_event * E / (launch_ms * 1e-3),
+                "algorithmic_bytes_per_launch": E * (4 * cfg.n_sensors + 20),
+                "hbm_gbs_signal_stream": E * (4 * cfg.n_sensors + 20) / (launch_ms * 1e-3) / 1e9,
+                "launch_ms": launch_ms}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": workload_config(cfg, E, world), "clocks": clocks,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": E * cfg.n_sensors * 4,
+                    "d2h_bytes_per_step": E * 20, "steps": e2e_steps, "chunk_events": chunk,
+                    "api": "ants_reconstruct_host (pinned host buffers, 3-stream ring)"},
+            "gpu_launches": int(gpu_launches), "roofline": roofline, "step_ms": step_ms,
+            "plan": r.plan()}
+
+    # ---- oracle beside it (rank 0, N = 1) -------------------------------------------------------
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        n_pool = min(E, 262_144)
+        rate, n, used = oracle_rate(cfg, sig_h[:n_pool].numpy(), args.cpu_seconds)
+        line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": used, "kind": "oracle",
+                                "sample": f"first {n} events of the same {cfg.name} batch, one pass, "
+                                          f"double precision, OpenMP over events"}
+    r.close()
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the `ncu --set full` capture of the
+# bench command (profiles/; null until captured for that workload)
+TRAFFIC_BYTES: dict = {}
+
+
+def main(argv=None):
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config 1..5 (default 2 = configs[1])")
+    ap.add_argument("--events", type=int, default=None, help="events per step per GPU (default: the config's batch)")
+    ap.add_argument("--resident", type=int, default=None, help="distinct resident batches to rotate through")
+    ap.add_argument("--e2e-chunk", type=int, default=1 << 18)
+    ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    ap.add_argument("--ref-step-seconds", type=float, default=4.0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args(argv)
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = max(args.warmup, 1)
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

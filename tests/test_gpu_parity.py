@@ -1,0 +1,241 @@
+"""GPU-vs-oracle parity through the C ABI (include/ants_recon.h), -m gpu.
+
+Rules (BASELINE.json north_star; tests/parity_rules.py): score at the returned
+node within 1e-5 relative of the oracle's score there, position within one
+final grid step for >= 99.9 % of events, identical winning node wherever the
+oracle's best-to-second gap exceeds 1e-4 relative, energy to 1e-5.
+
+Sizes: subsets the oracle finishes in seconds (several CTA tiles plus a ragged
+tail), and the full BASELINE.json sizes in the launch configuration bench.py
+times, checked on sampled events (events are independent, so the oracle can
+reconstruct any sample one by one).
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+from oracle import oracle                                      # noqa: E402
+from paper_1602_07247_b200 import recon, synth                 # noqa: E402
+import parity_rules                                            # noqa: E402
+
+FULL = os.environ.get("ANTS_TEST_FULL", "1") != "0"
+
+
+def _run(cfg, sig_dev, trace=True):
+    r = recon.Reconstructor(cfg)
+    try:
+        out = r(sig_dev, trace=trace)
+        torch.cuda.synchronize()
+        return [None if t is None else t.cpu().numpy() for t in out]
+    finally:
+        r.close()
+
+
+# subset sizes: ~3e8 (node, sensor) pairs each for the oracle; none a multiple of the CTA tile
+SUBSETS = {1: 10_000, 2: 20_011, 3: 4_003, 4: 2_501, 5: 2_503}
+
+
+@pytest.mark.parametrize("idx", [1, 2, 3, 4, 5])
+def test_parity_subset(idx):
+    cfg = synth.make_config(idx)
+    ev = synth.generate_events(cfg, SUBSETS[idx], device="cuda")
+    sig = ev["signals"]
+    xyzA, score, path = _run(cfg, sig)
+    res = parity_rules.compare(cfg, sig.cpu().numpy(), xyzA, score, path)
+    parity_rules.assert_parity(res, cfg.name)
+    # sanity: the reconstruction is near the truth (not parity, catches a broken generator)
+    err = np.hypot(xyzA[:, 0] - ev["true_xyz"][:, 0].cpu().numpy(), xyzA[:, 1] - ev["true_xyz"][:, 1].cpu().numpy())
+    assert np.nanmedian(err) < 6.0
+
+
+@pytest.mark.parametrize("idx", [2, 3, 4])
+def test_parity_full_size_sampled(idx):
+    """BASELINE.json's full event count in one launch (bench.py's configuration);
+    2000 sampled events are reconstructed one by one by the oracle."""
+    if not FULL:
+        pytest.skip("ANTS_TEST_FULL=0")
+    cfg = synth.make_config(idx)
+    E = cfg.n_events // cfg.n_batches
+    ev = synth.generate_events(cfg, E, device="cuda")
+    sig = ev["signals"]
+    r = recon.Reconstructor(cfg)
+    try:
+        xyzA, score = r(sig)
+        torch.cuda.synchronize()
+    finally:
+        r.close()
+    rng = np.random.default_rng(7)
+    n_s = 2000 if idx != 4 else 1000
+    pick = np.sort(rng.choice(E, n_s, replace=False))
+    pick[0], pick[-1] = 0, E - 1
+    pt = torch.from_numpy(pick).cuda()
+    res = parity_rules.compare(cfg, sig[pt].cpu().numpy(), xyzA[pt].cpu().numpy(), score[pt].cpu().numpy(), None)
+    parity_rules.assert_parity(res, cfg.name + " full")
+    # properties that hold at any size: every event produced a finite result inside the search reach
+    assert bool(torch.isfinite(xyzA).all()) and bool(torch.isfinite(score).all())
+    assert float(score.min()) >= -1e-3
+    reach = cfg.step0_xy * (cfg.nodes_per_axis - 1) / 2 * 2.0 + 1.0
+    lim = float(np.abs(cfg.sensor_xy).max()) + reach
+    assert float(xyzA[:, :2].abs().max()) <= lim
+
+
+def test_parity_cfg5_batch_sampled():
+    """One of config 5's eight 2M-event batches, through the streamed host-buffer entry point
+    (ants_reconstruct_host, pinned memory), sampled against the oracle."""
+    if not FULL:
+        pytest.skip("ANTS_TEST_FULL=0")
+    cfg = synth.make_config(5)
+    E = 400_000
+    ev = synth.generate_events(cfg, E, device="cuda", batch=3)
+    sig_h = ev["signals"].cpu().pin_memory()
+    xyzA = torch.empty((E, 4), dtype=torch.float32).pin_memory()
+    score = torch.empty((E,), dtype=torch.float32).pin_memory()
+    r = recon.Reconstructor(cfg)
+    try:
+        recon.ants_reconstruct_host(r.handle, sig_h, r.grid, r.method, xyzA, score, chunk_events=100_003)
+        d_xyzA, d_score = r(ev["signals"])
+        torch.cuda.synchronize()
+    finally:
+        r.close()
+    # host path == device path, bit for bit (same kernel, chunking must not matter)
+    assert torch.equal(xyzA, d_xyzA.cpu()) and torch.equal(score, d_score.cpu())
+    pick = np.sort(np.random.default_rng(11).choice(E, 1000, replace=False))
+    res = parity_rules.compare(cfg, sig_h.numpy()[pick], xyzA.numpy()[pick], score.numpy()[pick], None)
+    parity_rules.assert_parity(res, "cfg5 host-streamed")
+
+
+# ---------------------------------------------------------------------------
+# edge cases
+# ---------------------------------------------------------------------------
+def test_empty_and_tiny_batches():
+    cfg = synth.make_config(1)
+    r = recon.Reconstructor(cfg)
+    try:
+        xyzA, score = r(torch.empty((0, cfg.n_sensors), device="cuda"))
+        assert xyzA.shape == (0, 4) and score.shape == (0,)
+        ev = synth.generate_events(cfg, 37, device="cuda")
+        full = r(ev["signals"])
+        for n in (1, 2, 9, 33):
+            part = r(ev["signals"][:n].contiguous())
+            torch.cuda.synchronize()
+            assert torch.equal(part[0], full[0][:n]) and torch.equal(part[1], full[1][:n])
+    finally:
+        r.close()
+
+
+def test_failed_events_and_negative_signals():
+    cfg = synth.make_config(2)
+    ev = synth.generate_events(cfg, 64, device="cuda")
+    sig = ev["signals"].clone()
+    sig[3] = 0.0                         # sum S = 0 -> failed event
+    sig[5, 2] = float("nan")             # non-finite -> failed event
+    sig[7, 1] = float("inf")
+    sig[9] = -sig[9]                     # all negative: Poisson clips to 0 -> failed
+    sig[11, 0] = -3.0                    # one negative: clipped, event fine (R18)
+    xyzA, score, path = _run(cfg, sig)
+    for e in (3, 5, 7, 9):
+        assert np.isnan(xyzA[e]).all() and np.isposinf(score[e])
+        assert ((path[e].astype(np.int64) & 0xFFFF) == 0xFFFF).all()
+    res = parity_rules.compare(cfg, sig.cpu().numpy(), xyzA, score, path)
+    parity_rules.assert_parity(res, "failed events")
+    assert np.isfinite(xyzA[11]).all()
+
+
+@pytest.mark.parametrize("G,method", [(2, 0), (4, 1), (16, 0), (5, 1)])
+def test_grid_sizes_2d(G, method):
+    """Even and odd G, the smallest grid and the compiled maximum (16 x 16 = 256 nodes)."""
+    cfg = synth.make_config(2 if method == 0 else 3)
+    cfg.nodes_per_axis, cfg.method = G, method
+    cfg.step0_xy = 40.0 / G if method == 0 else 8.0 / G
+    cfg.n_iter = 9
+    ev = synth.generate_events(cfg, 1501, device="cuda")
+    xyzA, score, path = _run(cfg, ev["signals"])
+    res = parity_rules.compare(cfg, ev["signals"].cpu().numpy(), xyzA, score, path)
+    parity_rules.assert_parity(res, f"G={G} method={method}")
+
+
+def test_chi_square_on_shared_profile_and_poisson_on_individual():
+    """Method x LRF-sharing combinations the five configs do not use."""
+    for idx, method in ((2, 1), (3, 0)):
+        cfg = synth.make_config(idx)
+        cfg.method = method
+        ev = synth.generate_events(cfg, 3001, device="cuda")
+        xyzA, score, path = _run(cfg, ev["signals"])
+        res = parity_rules.compare(cfg, ev["signals"].cpu().numpy(), xyzA, score, path)
+        parity_rules.assert_parity(res, f"cfg{idx} method={method}")
+
+
+def test_non_positive_spline_uses_validity_rules():
+    """An LRF that goes negative far out: the library must fall back to the per-pair validity
+    rule (a node with L_i <= 0 where S_i > 0 is invalid) and still match the oracle."""
+    cfg = synth.make_config(2)
+    c = cfg.coeffs.copy()
+    c[0, 0, -4:] = -0.002                # negative tail beyond ~75 mm
+    cfg.coeffs = c
+    ev = synth.generate_events(synth.make_config(2), 2001, device="cuda")
+    xyzA, score, path = _run(cfg, ev["signals"])
+    res = parity_rules.compare(cfg, ev["signals"].cpu().numpy(), xyzA, score, path)
+    parity_rules.assert_parity(res, "negative tail")
+
+
+def test_noise_free_recovery_gpu():
+    """Noise-free signals: the GPU result is within one final step of the truth and the deviance ~ 0."""
+    for idx in (1, 2, 5):
+        cfg = synth.make_config(idx)
+        ev = synth.generate_events(cfg, 512, device="cuda", noise_free=True)
+        xyzA, score, path = _run(cfg, ev["signals"])
+        res = parity_rules.compare(cfg, ev["signals"].cpu().numpy(), xyzA, score, path, score_floor=1e-6)
+        assert res["fail_mismatch"] == 0 and res["score_viol"] == 0 and res["pos_frac_within"] >= 0.999, res
+
+
+def test_mirror_symmetry_gpu():
+    """Negating every sensor x negates the reconstructed x and leaves y, A, score bit-identical."""
+    cfg = synth.make_config(2)
+    ev = synth.generate_events(cfg, 4096, device="cuda")
+    a = _run(cfg, ev["signals"], trace=False)
+    cfg_m = synth.make_config(2)
+    cfg_m.sensor_xy = cfg.sensor_xy * np.array([-1.0, 1.0], np.float32)
+    b = _run(cfg_m, ev["signals"], trace=False)
+    same = (a[0][:, 0] == -b[0][:, 0]) & (a[0][:, 1] == b[0][:, 1])
+    assert same.mean() > 0.995                      # exact ties may break differently
+    assert np.array_equal(a[1][same], b[1][same])
+
+
+def test_status_codes():
+    cfg = synth.make_config(1)
+    r = recon.Reconstructor(cfg)
+    try:
+        sig = torch.ones((4, cfg.n_sensors), device="cuda")
+        xyzA = torch.empty((4, 4), device="cuda")
+        score = torch.empty((4,), device="cuda")
+
+        def status(**kw):
+            g = recon.GridParams(cfg.dim, cfg.nodes_per_axis, cfg.step0_xy, cfg.step0_z, cfg.factor,
+                                 cfg.n_iter, 0, cfg.z_seed)
+            for k, v in kw.items():
+                setattr(g, k, v)
+            try:
+                recon.ants_reconstruct(r.handle, sig, g, kw.get("_method", 0), xyzA, score)
+            except recon.AntsError as e:
+                return e.status
+            return 0
+
+        assert status() == 0
+        assert status(nodes_per_axis=1) == -1
+        assert status(factor=1.0) == -1
+        assert status(n_iter=0) == -1
+        assert status(step0_xy=0.0) == -1
+        assert status(dim=3) == -1                      # 3-D search over an axial LRF
+        assert status(nodes_per_axis=17) == -2          # 289 nodes > compiled limit
+        assert status(seed_mode=1) == -1
+    finally:
+        r.close()
+    with pytest.raises(recon.AntsError):
+        recon.ants_lrf_create(cfg.sensor_xy, cfg.gains, np.array([5.0, 1.0], np.float32), cfg.coeffs,
+                              recon.LrfDims(cfg.n_sensors, 1, 1, 16, 0))

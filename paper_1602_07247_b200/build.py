@@ -10,7 +10,7 @@ import subprocess
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(_HERE, "csrc", "ants_recon.cu")
-DEPS = [os.path.join(_HERE, "csrc", f) for f in ("ants_recon.cu", "recon_common.cuh", "recon2d.cuh", "recon3d.cuh")]
+DEPS = [os.path.join(_HERE, "csrc", f) for f in sorted(os.listdir(os.path.join(_HERE, "csrc")))]
 DEPS.append(os.path.join(os.path.dirname(_HERE), "include", "ants_recon.h"))
 LIB = os.path.join(_HERE, "libants_recon.so")
 

@@ -26,6 +26,7 @@ struct ants_lrf {
     int sm_count = 0;
     bool positive = false;   // every spline strictly positive on its domain
     double max_dlog = 0.0;   // max |d ln s / dr| over the domain, 1/mm (only if positive)
+    double max_dlog_z = 0.0; // axial+z: max |d ln s / dz|, 1/mm
     double knot_r = 0.0, knot_z = 0.0;   // knot spacing, mm
     void *d_sens = nullptr, *d_poly = nullptr, *d_polyd = nullptr;
     // scratch of ants_reconstruct_host (lazily allocated, reused, guarded)
@@ -96,6 +97,85 @@ static void build_rows(const float *c, int n_r, double sc_r, float4 *rows32, dou
     rows32[n_r] = make_float4((float)(last[0] + last[1] + last[2] + last[3]), 0.f, 0.f, 0.f);
 }
 
+// bicubic Bezier patch, positivity by recursive de Casteljau subdivision: positive if every control
+// point is > 0 (convex hull); not positive if a corner (a true surface value) is <= 0; otherwise
+// split in four.  Depth-limited: undecided counts as not positive (conservative).
+struct Patch { double p[4][4]; };
+static void split_cubic(const double in[4], double lo[4], double hi[4]) {
+    const double m01 = 0.5 * (in[0] + in[1]), m12 = 0.5 * (in[1] + in[2]), m23 = 0.5 * (in[2] + in[3]);
+    const double m012 = 0.5 * (m01 + m12), m123 = 0.5 * (m12 + m23), mid = 0.5 * (m012 + m123);
+    lo[0] = in[0]; lo[1] = m01; lo[2] = m012; lo[3] = mid;
+    hi[0] = mid; hi[1] = m123; hi[2] = m23; hi[3] = in[3];
+}
+static bool patch_positive(const Patch &P, int depth) {
+    double mn = P.p[0][0];
+    for (int a = 0; a < 4; ++a)
+        for (int b = 0; b < 4; ++b) mn = std::fmin(mn, P.p[a][b]);
+    if (mn > 0.0) return true;
+    if (!(P.p[0][0] > 0.0) || !(P.p[0][3] > 0.0) || !(P.p[3][0] > 0.0) || !(P.p[3][3] > 0.0)) return false;
+    if (depth >= 10) return false;
+    Patch rl, rh;     // split along the second index
+    for (int a = 0; a < 4; ++a) split_cubic(P.p[a], rl.p[a], rh.p[a]);
+    for (const Patch *half : {&rl, &rh}) {
+        Patch zl, zh; // split along the first index
+        for (int b = 0; b < 4; ++b) {
+            double in[4] = {half->p[0][b], half->p[1][b], half->p[2][b], half->p[3][b]}, lo[4], hi[4];
+            split_cubic(in, lo, hi);
+            for (int a = 0; a < 4; ++a) { zl.p[a][b] = lo[a]; zh.p[a][b] = hi[a]; }
+        }
+        if (!patch_positive(zl, depth + 1) || !patch_positive(zh, depth + 1)) return false;
+    }
+    return true;
+}
+
+// axial+z: positivity and log-slopes of the tensor-product spline s(r, z).
+// Positivity: Bezier control nets of every bicubic patch, subdivided until decided (patch_positive).
+// Slopes: max |ds/dr|/s and |ds/dz|/s on a 9 x 9 sample of every patch (sizes the log1p series range).
+static void tensor_analysis(const float *c, const double *rows64, int n_r, int n_z, double sc_r, double sc_z,
+                            bool &positive, double &dlog_r, double &dlog_z) {
+    static const double M[4][4] = {{1 / 6.0, 4 / 6.0, 1 / 6.0, 0}, {0, 4 / 6.0, 2 / 6.0, 0},
+                                   {0, 2 / 6.0, 4 / 6.0, 0}, {0, 1 / 6.0, 4 / 6.0, 1 / 6.0}};
+    positive = true;
+    dlog_r = dlog_z = 0.0;
+    const int nc = n_r + 3;
+    for (int kz = 0; kz < n_z; ++kz)
+        for (int kr = 0; kr < n_r; ++kr) {
+            Patch P;
+            for (int a = 0; a < 4; ++a)
+                for (int b = 0; b < 4; ++b) {
+                    double v = 0.0;
+                    for (int i = 0; i < 4; ++i)
+                        for (int j = 0; j < 4; ++j) v += M[a][i] * M[b][j] * (double)c[(kz + i) * nc + kr + j];
+                    P.p[a][b] = v;
+                }
+            if (!patch_positive(P, 0)) positive = false;
+            for (int iz = 0; iz <= 8; ++iz) {
+                const double u = iz / 8.0, o = 1.0 - u;
+                const double bz[4] = {o * o * o / 6.0, (3 * u * u * u - 6 * u * u + 4) / 6.0,
+                                      (-3 * u * u * u + 3 * u * u + 3 * u + 1) / 6.0, u * u * u / 6.0};
+                const double dz[4] = {-o * o / 2.0, (9 * u * u - 12 * u) / 6.0, (-9 * u * u + 6 * u + 3) / 6.0, u * u / 2.0};
+                for (int ir = 0; ir <= 8; ++ir) {
+                    const double t = ir / 8.0;
+                    double sv = 0.0, sr = 0.0, sz = 0.0;
+                    for (int b = 0; b < 4; ++b) {
+                        const double *q = rows64 + ((size_t)(kz + b) * n_r + kr) * 4;
+                        const double f = q[0] + t * (q[1] + t * (q[2] + t * q[3]));
+                        const double d = q[1] + t * (2.0 * q[2] + 3.0 * t * q[3]);
+                        sv += bz[b] * f;
+                        sr += bz[b] * d;
+                        sz += dz[b] * f;
+                    }
+                    if (sv > 0.0) {
+                        dlog_r = std::fmax(dlog_r, std::fabs(sr) * sc_r / sv);
+                        dlog_z = std::fmax(dlog_z, std::fabs(sz) * sc_z / sv);
+                    } else {
+                        positive = false;
+                    }
+                }
+            }
+        }
+}
+
 static bool finite_f(float v) { return std::isfinite(v); }
 
 extern "C" int ants_lrf_create(const float *sensor_xy, const float *gains, const float *knots,
@@ -149,15 +229,12 @@ extern "C" int ants_lrf_create(const float *sensor_xy, const float *gains, const
     for (size_t s = 0; s < n_spl; ++s)
         build_rows(coeffs + s * (n_r + 3), n_r, sc_r, rows32.data() + s * (n_r + 1),
                    rows64.data() + s * n_r * 4, positive, max_dlog);
-    if (dim == 2) {
-        // positivity / slope of the tensor product: sufficient test on the coefficients
-        // (all > 0 => s > 0 by the convex-hull property); the differential 3-D score needs it
-        positive = true;
-        for (size_t j = 0; j < n_coef; ++j)
-            if (!(coeffs[j] > 0.f)) positive = false;
-    }
+    double max_dlog_z = 0.0;
+    if (dim == 2) tensor_analysis(coeffs, rows64.data(), n_r, n_z, sc_r, (double)n_z / ((double)z_hi - (double)z_lo),
+                                  positive, max_dlog, max_dlog_z);
     h->positive = positive;
     h->max_dlog = max_dlog;
+    h->max_dlog_z = max_dlog_z;
     h->knot_r = 1.0 / sc_r;
     h->knot_z = dim == 2 ? ((double)z_hi - (double)z_lo) / n_z : 0.0;
 
@@ -234,6 +311,7 @@ struct Plan {
     int ctas_per_sm = 0;
     size_t smem = 0;         // dynamic shared memory per CTA
     int k_diff = 0;          // first differential iteration (K = never)
+    int k_series = 0;        // axial+z Poisson: first iteration with the log1p series
     const void *kernel = nullptr;
 };
 
@@ -275,27 +353,74 @@ static int validate_grid(const ants_lrf *h, const ants_grid_params_t *g, int32_t
 static int first_diff_iter(const ants_lrf *h, const ants_grid_params_t *g, int32_t method) {
     if (!h->positive) return g->n_iter;
     const double half = 0.5 * (g->nodes_per_axis - 1);
-    double hxy = g->step0_xy, hz = g->step0_z;
-    for (int k = 0; k < g->n_iter; ++k, hxy *= (double)g->factor, hz *= (double)g->factor) {
-        double reach = std::sqrt(2.0) * half * hxy * 1.001;
+    double hxy = g->step0_xy;
+    for (int k = 0; k < g->n_iter; ++k, hxy *= (double)g->factor) {
+        const double reach = std::sqrt(2.0) * half * hxy * 1.001;
         bool ok = reach <= 0.9 * h->knot_r;
-        if (g->dim == 3) ok = ok && (half * hz * 1.001 <= 0.9 * h->knot_z);
-        if (method == ANTS_POISSON_ML) {
-            double bound = std::expm1(h->max_dlog * reach);
-            if (g->dim == 3) bound = 1e9;   // 3-D decides by its own rule in make_plan3d
-            ok = ok && (bound <= kQSeries || g->dim == 3);
-        }
+        if (method == ANTS_POISSON_ML) ok = ok && std::expm1(h->max_dlog * reach) <= kQSeries;
         if (ok) return k;
     }
     return g->n_iter;
+}
+
+template <int METHOD>
+static const void *pick3d(int cpl, int gzm) {
+#define ANTS_K3(C, Z) if (cpl == C && gzm == Z) return (const void *)recon3d_kernel<C, Z, METHOD>
+    ANTS_K3(1, 1); ANTS_K3(2, 1); ANTS_K3(3, 1); ANTS_K3(4, 1); ANTS_K3(8, 1);
+    ANTS_K3(1, 4); ANTS_K3(2, 4); ANTS_K3(1, 8); ANTS_K3(2, 8);
+#undef ANTS_K3
+    return nullptr;
+}
+
+// axial+z LRF: search over (x, y, z) or over (x, y) at fixed z
+static int make_plan3d(const ants_lrf *h, const ants_grid_params_t *g, int32_t method, Plan &pl) {
+    const ModelDev &m = h->dev;
+    const int G = g->nodes_per_axis, Gz = g->dim == 3 ? G : 1;
+    int cpl = 0, gzm = 1;
+    if (g->dim == 3) {
+        if (G > 8) return ANTS_ERR_UNSUPPORTED;           // 512 nodes
+        cpl = G * G <= 32 ? 1 : 2;
+        gzm = G <= 4 ? 4 : 8;
+    } else {
+        if (G * G > 256) return ANTS_ERR_UNSUPPORTED;
+        const int need = (G * G + 31) / 32;
+        for (int c : kNpt2D)
+            if (c >= need) { cpl = c; break; }
+    }
+    pl.npt = cpl * Gz;
+    pl.kernel = method == ANTS_POISSON_ML ? pick3d<0>(cpl, gzm) : pick3d<1>(cpl, gzm);
+    if (!pl.kernel) return ANTS_ERR_UNSUPPORTED;
+    // differential from the first grid that stays within one knot interval of the centre (r and z);
+    // Poisson log1p by series once |dL/L0| <= kQSeries on the whole grid
+    pl.k_diff = pl.k_series = g->n_iter;
+    if (h->positive) {
+        const double half = 0.5 * (G - 1);
+        double hxy = g->step0_xy, hz = g->dim == 3 ? g->step0_z : 0.0;
+        for (int k = 0; k < g->n_iter; ++k, hxy *= (double)g->factor, hz *= (double)g->factor) {
+            const double reach = std::sqrt(2.0) * half * hxy * 1.001, reach_z = half * hz * 1.001;
+            const bool ok = reach <= 0.9 * h->knot_r && reach_z <= 0.9 * h->knot_z;
+            if (ok && pl.k_diff == g->n_iter) pl.k_diff = k;
+            if (ok && std::expm1(h->max_dlog * reach + h->max_dlog_z * reach_z) <= kQSeries) { pl.k_series = k; break; }
+        }
+        if (pl.k_series < pl.k_diff) pl.k_series = pl.k_diff;
+    }
+    const size_t tables = (size_t)(m.N + (m.n_z + 3) * (m.n_r + 1)) * 16;
+    const size_t per_warp = warp_smem_bytes_3d(m.N, Gz, m.n_r + 1);
+    const size_t budget = 227 * 1024;
+    pl.warps = 8;
+    while (pl.warps > 1 && tables + pl.warps * per_warp > budget / 2) pl.warps >>= 1;
+    pl.smem = tables + pl.warps * per_warp;
+    if (pl.smem > budget) return ANTS_ERR_UNSUPPORTED;
+    pl.ctas_per_sm = (int)std::min<size_t>(budget / (pl.smem + 1024), (size_t)(2048 / (pl.warps * 32)));
+    if (pl.ctas_per_sm < 1) pl.ctas_per_sm = 1;
+    return ANTS_OK;
 }
 
 static int make_plan(const ants_lrf *h, const ants_grid_params_t *g, int32_t method, Plan &pl) {
     int rc = validate_grid(h, g, method);
     if (rc != ANTS_OK) return rc;
     const ModelDev &m = h->dev;
-    if (g->dim == 3 || m.n_z > 0) return make_plan3d(h->positive, h->knot_r, h->knot_z, h->max_dlog, m, g, method,
-                                                    pl.npt, pl.warps, pl.ctas_per_sm, pl.smem, pl.k_diff, pl.kernel);
+    if (m.n_z > 0) return make_plan3d(h, g, method, pl);
     const long long nodes = (long long)g->nodes_per_axis * g->nodes_per_axis;
     if (nodes > 256) return ANTS_ERR_UNSUPPORTED;
     int need = (int)((nodes + 31) / 32);
@@ -308,6 +433,7 @@ static int make_plan(const ants_lrf *h, const ants_grid_params_t *g, int32_t met
     else
         pl.kernel = h->positive ? pick2d<1, true>(pl.npt) : pick2d<1, false>(pl.npt);
     pl.k_diff = first_diff_iter(h, g, method);
+    pl.k_series = pl.k_diff;
     const size_t tables = (size_t)(m.N + m.n_lrf * (m.n_r + 1)) * 16;
     const size_t per_warp = warp_smem_bytes_2d(m.N);
     const size_t budget = 227 * 1024;
@@ -358,6 +484,8 @@ static int launch(const ants_lrf *h, const float *signals, int64_t n_events, con
     p.K = g->n_iter;
     p.nodes = g->dim == 3 ? p.G * p.G * p.G : p.G * p.G;
     p.k_diff = pl.k_diff;
+    p.k_series = pl.k_series;
+    p.positive = h->positive ? 1 : 0;
     p.h0_xy = g->step0_xy;
     p.h0_z = g->dim == 3 ? g->step0_z : 0.f;
     p.factor = g->factor;

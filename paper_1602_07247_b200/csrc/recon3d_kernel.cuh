@@ -1,0 +1,152 @@
+// recon3d_kernel.cuh -- the axial+z kernel (included by recon3d.cuh, which documents the mapping).
+#pragma once
+
+namespace ants {
+
+// CPL columns per lane, GZM compiled maximum of z-levels, METHOD 0 Poisson ML / 1 weighted chi-square.
+template <int CPL, int GZM, int METHOD>
+__global__ void __launch_bounds__(256) recon3d_kernel(const Params p) {
+    extern __shared__ __align__(16) unsigned char smem[];
+    const ModelDev &m = p.m;
+    const int N = m.N, nr1 = m.n_r + 1;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int Gz = p.dim == 3 ? p.G : 1;
+    const int ncol = p.G * p.G;
+    const int rows = (m.n_z + 3) * nr1;
+    const double sczd = (double)m.n_z / ((double)m.z_hi - (double)m.z_lo);
+
+    // CTA-shared tables: sensor records and the per-z-coefficient spline rows
+    float4 *sens_s = reinterpret_cast<float4 *>(smem);
+    float4 *poly_s = sens_s + N;
+    for (int i = threadIdx.x; i < N; i += blockDim.x) sens_s[i] = m.sens[i];
+    for (int i = threadIdx.x; i < rows; i += blockDim.x) poly_s[i] = m.poly[i];
+    __syncthreads();
+    WarpSmem3D w = carve_3d(smem + (size_t)(N + rows) * 16 + (size_t)warp * warp_smem_bytes_3d(N, Gz, nr1), N, Gz, nr1);
+
+    // this lane's columns: offsets from the grid centre in units of the step
+    const float half = 0.5f * (float)(p.G - 1);
+    const float halfz = p.dim == 3 ? half : 0.f;
+    float fx[CPL], fy[CPL];
+    bool cv[CPL];
+#pragma unroll
+    for (int j = 0; j < CPL; ++j) {
+        int c = lane + 32 * j;
+        cv[j] = c < ncol;
+        int iy = c / p.G, ix = c - iy * p.G;
+        fx[j] = cv[j] ? (float)ix - half : 0.f;
+        fy[j] = cv[j] ? (float)iy - half : 0.f;
+    }
+    const float half_diag_units = 1.41421356f * half;
+    const float z_start = (p.z_seed == p.z_seed) ? p.z_seed : 0.5f * (m.z_lo + m.z_hi);   // R10
+
+    const long long stride = (long long)gridDim.x * p.warps_per_cta;
+    for (long long e = (long long)blockIdx.x * p.warps_per_cta + warp; e < p.n_events; e += stride) {
+        // ---- a1: load signals, prepare, centroid ----
+        const float *sig = p.signals + e * N;
+        float sumS = 0.f, sw = 0.f, sxw = 0.f, syw = 0.f;
+        bool finite = true;
+        for (int i = lane; i < N; i += 32) {
+            float S = __ldg(sig + i);
+            finite = finite && (fabsf(S) <= 3.402823466e38f);
+            if (METHOD == 0) S = fmaxf(S, 0.f);          // R18
+            float4 sn = sens_s[i];
+            float wgt = S * sn.w;
+            sumS += S;
+            sw += wgt;
+            sxw = fmaf(sn.x, wgt, sxw);
+            syw = fmaf(sn.y, wgt, syw);
+            float cs = 0.f;
+            if (METHOD == 0 && S > 0.f) cs = log2f(S * sn.w);
+            w.SC[i] = make_float2(S, cs);
+        }
+        finite = __all_sync(kFull, finite);
+        sumS = warp_sum(sumS);
+        sw = warp_sum(sw);
+        sxw = warp_sum(sxw);
+        syw = warp_sum(syw);
+        __syncwarp();
+        if (!finite || !(sumS > 0.f) || !(sw > 0.f)) {
+            if (lane == 0) {
+                const float qnan = __int_as_float(0x7fc00000);
+                reinterpret_cast<float4 *>(p.out_xyzA)[e] = make_float4(qnan, qnan, qnan, qnan);
+                p.out_score[e] = kInf;
+            }
+            if (p.out_path)
+                for (int k = lane; k < p.K; k += 32) p.out_path[e * p.K + k] = 0xFFFF;
+            continue;
+        }
+        float cx = sxw / sw, cy = syw / sw, cz = z_start;
+        float A_ref = 1.f;
+
+        float h = p.h0_xy, hz = p.h0_z;
+        for (int k = 0; k < p.K; ++k) {
+            build_level_tables(m, poly_s, w, lane, sczd, Gz, cz, hz, halfz);
+            if (k == 0) {
+                // reference energy for the plain score: A at the seed
+                float sl = 0.f;
+                for (int i = lane; i < N; i += 32) {
+                    float4 sn = sens_s[i];
+                    float dx = cx - sn.x, dy = cy - sn.y;
+                    float t = fminf(fmaxf(fmaf(sqrtf(fmaf(dx, dx, dy * dy)), m.sc, m.of), -0.5f), m.tmax);
+                    int kk;
+                    float v;
+                    split_t(t, kk, v);
+                    sl = fmaf(sn.z, horner(w.Tc[kk], v), sl);
+                }
+                sl = warp_sum(sl);
+                A_ref = sl > 0.f ? sumS / sl : 1.f;
+            }
+            const bool centre_ok = cz >= m.z_lo && cz <= m.z_hi;
+            float sc_node[CPL][GZM];       // node scores (lower is better), +inf = invalid
+            float aux_node[CPL][GZM];      // plain mode: sum L (Poisson) / A (chi2) at the node
+            const bool plain = k < p.k_diff || !centre_ok;
+            if (plain) {
+#include "recon3d_plain.inc"
+            } else {
+#include "recon3d_diff.inc"
+            }
+
+            // ---- a5: argmin over the G^2 * Gz nodes, recentre, contract ----
+            float bs = kInf;
+            int bi = 0x7fffffff;
+#pragma unroll
+            for (int l = 0; l < GZM; ++l)
+#pragma unroll
+                for (int j = 0; j < CPL; ++j)
+                    if (sc_node[j][l] < bs) { bs = sc_node[j][l]; bi = l * ncol + lane + 32 * j; }
+            warp_argmin(bs, bi);
+            const bool found = bs < kInf;
+            if (found) {
+                const int l = bi / ncol, c = bi - l * ncol;
+                if (plain) {
+                    float mine = 0.f;
+#pragma unroll
+                    for (int ll = 0; ll < GZM; ++ll)
+#pragma unroll
+                        for (int j = 0; j < CPL; ++j)
+                            if (ll == l && (c >> 5) == j) mine = aux_node[j][ll];
+                    float v = __shfl_sync(kFull, mine, c & 31);
+                    A_ref = METHOD == 0 ? sumS / v : v;
+                }
+                int iy = c / p.G, ix = c - iy * p.G;
+                cx = fmaf((float)ix - half, h, cx);
+                cy = fmaf((float)iy - half, h, cy);
+                cz = fmaf((float)l - halfz, hz, cz);
+            }
+            if (p.out_path && lane == 0) p.out_path[e * p.K + k] = found ? (uint16_t)bi : (uint16_t)0xFFFF;
+            h *= p.factor;
+            hz *= p.factor;
+            __syncwarp();
+        }
+
+        // ---- a6: FP64 energy and score at the final node, store ----
+        float A_fin, score_fin;
+        final_score_3d<METHOD>(m, sens_s, w, lane, sczd, cx, cy, cz, A_fin, score_fin);
+        if (lane == 0) {
+            reinterpret_cast<float4 *>(p.out_xyzA)[e] = make_float4(cx, cy, cz, A_fin);
+            p.out_score[e] = score_fin;
+        }
+    }
+}
+
+}  // namespace ants

@@ -35,6 +35,8 @@ struct Params {
     uint16_t *out_path;     // [E][K] or nullptr
     int G, K, nodes, dim;   // nodes = G^dim
     int k_diff;             // first iteration scored differentially (K = never)
+    int k_series;           // 3-D Poisson: first iteration whose log1p is the series (before: lg2(1 + q))
+    int positive;           // every LRF strictly positive on its domain (validity tests can be skipped)
     float h0_xy, h0_z, factor, z_seed;
     int warps_per_cta;
     int tile_events;        // events staged per CTA tile (= warps_per_cta)

@@ -243,3 +243,47 @@ def test_status_codes():
     with pytest.raises(recon.AntsError):
         recon.ants_lrf_create(cfg.sensor_xy, cfg.gains, np.array([5.0, 1.0], np.float32), cfg.coeffs,
                               recon.LrfDims(cfg.n_sensors, 1, 1, 16, 0))
+
+
+# ---------------------------------------------------------------------------
+# axial+z LRF variants beyond config 4
+# ---------------------------------------------------------------------------
+@pytest.mark.parametrize("G,method", [(7, 1), (4, 0), (8, 0), (3, 1), (5, 0)])
+def test_axial_z_grid_sizes_and_methods(G, method):
+    cfg = synth.make_config(4)
+    cfg.nodes_per_axis, cfg.method = G, method
+    cfg.step0_xy, cfg.step0_z = 48.0 / (G - 1), 18.0 / (G - 1)
+    ev = synth.generate_events(cfg, 2401, device="cuda")
+    xyzA, score, path = _run(cfg, ev["signals"])
+    res = parity_rules.compare(cfg, ev["signals"].cpu().numpy(), xyzA, score, path)
+    parity_rules.assert_parity(res, f"axial+z G={G} method={method}")
+
+
+@pytest.mark.parametrize("G,z_seed", [(9, 7.5), (12, float("nan")), (6, 0.0), (16, 20.0)])
+def test_axial_z_lrf_with_2d_search_at_fixed_z(G, z_seed):
+    """dim = 2 over an (r, z) LRF: the search runs in (x, y) at z = z_seed (NaN = mid-range)."""
+    cfg = synth.make_config(4)
+    cfg.dim, cfg.nodes_per_axis, cfg.z_seed = 2, G, z_seed
+    cfg.step0_xy = 48.0 / (G - 1)
+    z = 10.0 if z_seed != z_seed else z_seed
+    cfg.z_range = (z, z)
+    ev = synth.generate_events(cfg, 1203, device="cuda")
+    xyzA, score, path = _run(cfg, ev["signals"])
+    assert np.all(xyzA[:, 2] == np.float32(z))
+    res = parity_rules.compare(cfg, ev["signals"].cpu().numpy(), xyzA, score, path)
+    parity_rules.assert_parity(res, f"axial+z fixed z G={G}")
+
+
+def test_axial_z_seed_outside_range_gives_invalid_nodes():
+    """z_seed outside [z_lo, z_hi] with a 2-D search: every node is invalid (R6), the centre stays at
+    the centroid, A = NaN and score = +inf, exactly as the oracle."""
+    cfg = synth.make_config(4)
+    cfg.dim, cfg.z_seed = 2, 25.0
+    ev = synth.generate_events(cfg, 64, device="cuda")
+    xyzA, score, path = _run(cfg, ev["signals"])
+    assert np.isposinf(score).all() and np.isnan(xyzA[:, 3]).all() and np.isfinite(xyzA[:, :3]).all()
+    res = parity_rules.compare(cfg, ev["signals"].cpu().numpy(), xyzA, score, path)
+    assert res["idx_diverged"] == 0 and res["pos_frac_within"] == 1.0 or res["fail_mismatch"] >= 0
+    model = oracle.Model.from_config(cfg)
+    ref = oracle.reconstruct(model, ev["signals"].cpu().numpy(), oracle.grid_from_config(cfg), cfg.method)
+    assert np.allclose(ref["xyzA"][:, :2], xyzA[:, :2], atol=1e-4) and np.isposinf(ref["score"]).all()

@@ -13,6 +13,7 @@
 
 #include "../../include/ants_recon.h"
 #include "recon2d.cuh"
+#include "recon2d_pk.cuh"
 #include "recon3d.cuh"
 
 using namespace ants;
@@ -318,6 +319,18 @@ struct Plan {
 static const int kNpt2D[] = {1, 2, 3, 4, 8};
 static const double kQSeries = 0.1;   // |dL/L0| bound under which the degree-6 log1p series is used
 
+template <int METHOD>
+static const void *pick2d_pk(int npt) {
+    switch (npt) {
+        case 1: return (const void *)recon2d_pk_kernel<1, METHOD>;
+        case 2: return (const void *)recon2d_pk_kernel<2, METHOD>;
+        case 3: return (const void *)recon2d_pk_kernel<3, METHOD>;
+        case 4: return (const void *)recon2d_pk_kernel<4, METHOD>;
+        case 8: return (const void *)recon2d_pk_kernel<8, METHOD>;
+    }
+    return nullptr;
+}
+
 template <int METHOD, bool POS>
 static const void *pick2d(int npt) {
     switch (npt) {
@@ -428,14 +441,17 @@ static int make_plan(const ants_lrf *h, const ants_grid_params_t *g, int32_t met
     for (int c : kNpt2D)
         if (c >= need) { pl.npt = c; break; }
     if (!pl.npt) return ANTS_ERR_UNSUPPORTED;
-    if (method == ANTS_POISSON_ML)
-        pl.kernel = h->positive ? pick2d<0, true>(pl.npt) : pick2d<0, false>(pl.npt);
+    // strictly positive LRFs (the normal case) run the sensor-pair-packed kernel; others the generic one
+    const bool packed = h->positive;
+    if (packed)
+        pl.kernel = method == ANTS_POISSON_ML ? pick2d_pk<0>(pl.npt) : pick2d_pk<1>(pl.npt);
     else
-        pl.kernel = h->positive ? pick2d<1, true>(pl.npt) : pick2d<1, false>(pl.npt);
+        pl.kernel = method == ANTS_POISSON_ML ? pick2d<0, false>(pl.npt) : pick2d<1, false>(pl.npt);
     pl.k_diff = first_diff_iter(h, g, method);
     pl.k_series = pl.k_diff;
-    const size_t tables = (size_t)(m.N + m.n_lrf * (m.n_r + 1)) * 16;
-    const size_t per_warp = warp_smem_bytes_2d(m.N);
+    const size_t tables = packed ? (cta_smem_bytes_pk(m.N, m.n_lrf * (m.n_r + 1)) + 15) / 16 * 16
+                                 : (size_t)(m.N + m.n_lrf * (m.n_r + 1)) * 16;
+    const size_t per_warp = packed ? warp_smem_bytes_pk(m.N, method) : warp_smem_bytes_2d(m.N);
     const size_t budget = 227 * 1024;
     pl.warps = 8;
     while (pl.warps > 1 && tables + pl.warps * per_warp > budget / 2) pl.warps >>= 1;

@@ -1,0 +1,151 @@
+// recon2d_pk_kernel.cuh -- kernel body of recon2d_pk.cuh (which documents layout and packing).
+#pragma once
+
+namespace ants {
+
+// METHOD 0 Poisson ML, 1 weighted chi-square.  Requires every LRF strictly positive (host-checked).
+template <int NPT, int METHOD>
+__global__ void __launch_bounds__(256) recon2d_pk_kernel(const Params p) {
+    extern __shared__ __align__(16) unsigned char smem[];
+    const ModelDev &m = p.m;
+    const int N = m.N, nr1 = m.n_r + 1, Np = (N + 1) / 2;
+    const bool indiv = m.n_lrf > 1;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int rows = m.n_lrf * nr1;
+
+    // ---- CTA-shared tables ----
+    float4 *sens_s = reinterpret_cast<float4 *>(smem);
+    float4 *poly_s = sens_s + N;
+    float4 *XY2 = poly_s + rows;
+    float2 *G2 = reinterpret_cast<float2 *>(XY2 + Np);
+    for (int i = threadIdx.x; i < N; i += blockDim.x) sens_s[i] = m.sens[i];
+    for (int i = threadIdx.x; i < rows; i += blockDim.x) poly_s[i] = m.poly[i];
+    for (int q = threadIdx.x; q < Np; q += blockDim.x) {
+        const float4 e = m.sens[2 * q];
+        const bool has_o = 2 * q + 1 < N;
+        const float4 o = has_o ? m.sens[2 * q + 1] : make_float4(0.f, 0.f, 0.f, 0.f);
+        XY2[q] = make_float4(e.x, o.x, e.y, o.y);
+        G2[q] = make_float2(indiv ? 1.f : e.z, has_o ? (indiv ? 1.f : o.z) : 0.f);   // pad: g = 0
+    }
+    __syncthreads();
+    WarpSmemPk w = carve_pk(smem + (cta_smem_bytes_pk(N, rows) + 15) / 16 * 16 +
+                            (size_t)warp * warp_smem_bytes_pk(N, METHOD), N, METHOD);
+    const int np1 = pk_pairs(N);
+
+    // this lane's nodes: offsets from the grid centre in units of the step
+    const float half = 0.5f * (float)(p.G - 1);
+    float fx[NPT], fy[NPT];
+    bool nv[NPT];
+#pragma unroll
+    for (int j = 0; j < NPT; ++j) {
+        int n = lane + 32 * j;
+        nv[j] = n < p.nodes;
+        int iy = n / p.G, ix = n - iy * p.G;
+        fx[j] = nv[j] ? (float)ix - half : 0.f;
+        fy[j] = nv[j] ? (float)iy - half : 0.f;
+    }
+    const float half_diag_units = 1.41421356f * half;
+    const f32x2 sc2 = pk1(m.sc), of2 = pk1(m.of), magic2 = pk1(kMagic), nmagic2 = pk1(-kMagic);
+
+    const long long stride = (long long)gridDim.x * p.warps_per_cta;
+    for (long long e = (long long)blockIdx.x * p.warps_per_cta + warp; e < p.n_events; e += stride) {
+        // ---- a1: load signals (coalesced), prepare, centroid ----
+        const float *sig = p.signals + e * N;
+        float sumS = 0.f, sw = 0.f, sxw = 0.f, syw = 0.f;
+        bool finite = true;
+        for (int i = lane; i < N; i += 32) {
+            float S = __ldg(sig + i);
+            finite = finite && (fabsf(S) <= 3.402823466e38f);
+            if (METHOD == 0) S = fmaxf(S, 0.f);          // R18
+            float4 sn = sens_s[i];
+            float wgt = S * sn.w;
+            sumS += S;
+            sw += wgt;
+            sxw = fmaf(sn.x, wgt, sxw);
+            syw = fmaf(sn.y, wgt, syw);
+            float cs = 0.f;
+            if (METHOD == 0 && S > 0.f) cs = log2f(S * sn.w);
+            w.SC[i] = make_float2(S, cs);
+        }
+        finite = __all_sync(kFull, finite);
+        sumS = warp_sum(sumS);
+        sw = warp_sum(sw);
+        sxw = warp_sum(sxw);
+        syw = warp_sum(syw);
+        __syncwarp();
+        if (!finite || !(sumS > 0.f) || !(sw > 0.f)) {
+            if (lane == 0) {
+                const float qnan = __int_as_float(0x7fc00000);
+                reinterpret_cast<float4 *>(p.out_xyzA)[e] = make_float4(qnan, qnan, qnan, qnan);
+                p.out_score[e] = kInf;
+            }
+            if (p.out_path)
+                for (int k = lane; k < p.K; k += 32) p.out_path[e * p.K + k] = 0xFFFF;
+            continue;
+        }
+        float cx = sxw / sw, cy = syw / sw;
+
+        // reference energy for the plain score: A at the seed
+        float A_ref;
+        {
+            float sl = 0.f;
+            for (int i = lane; i < N; i += 32) {
+                float4 sn = sens_s[i];
+                float dx = cx - sn.x, dy = cy - sn.y;
+                float s = eval_axial(m, poly_s, i, sqrtf(fmaf(dx, dx, dy * dy)));
+                sl += (indiv ? 1.f : sn.z) * s;
+            }
+            sl = warp_sum(sl);
+            A_ref = sl > 0.f ? sumS / sl : 1.f;
+        }
+
+        float h = p.h0_xy;
+        for (int k = 0; k < p.K; ++k) {
+            float sc_node[NPT];          // node scores (lower is better), +inf = invalid
+            float aux_node[NPT];         // plain mode: sum L (Poisson) / A (chi2) at the node
+            if (k < p.k_diff) {
+#include "recon2d_pk_plain.inc"
+            } else {
+#include "recon2d_pk_diff.inc"
+            }
+
+            // ---- a5: argmin over the G^2 nodes, recentre, contract ----
+            float bs = kInf;
+            int bi = 0x7fffffff;
+#pragma unroll
+            for (int j = 0; j < NPT; ++j)
+                if (sc_node[j] < bs) { bs = sc_node[j]; bi = lane + 32 * j; }
+            warp_argmin_redux(bs, bi);
+            const bool found = bs < kInf;
+            if (found) {
+                if (k < p.k_diff) {
+                    float mine = 0.f;
+#pragma unroll
+                    for (int j = 0; j < NPT; ++j)
+                        if ((bi >> 5) == j) mine = aux_node[j];
+                    float v = __shfl_sync(kFull, mine, bi & 31);
+                    A_ref = METHOD == 0 ? sumS / v : v;
+                }
+                int iy = bi / p.G, ix = bi - iy * p.G;
+                cx = fmaf((float)ix - half, h, cx);
+                cy = fmaf((float)iy - half, h, cy);
+            }
+            if (p.out_path && lane == 0) p.out_path[e * p.K + k] = found ? (uint16_t)bi : (uint16_t)0xFFFF;
+            h *= p.factor;
+            __syncwarp();
+        }
+
+        // ---- a6: FP64 energy and score at the final node, store ----
+        float A_fin, score_fin;
+        WarpSmem2D w2;               // final_score_2d needs N doubles of scratch (D[0..1]) and SC
+        w2.A = w.D[0];
+        w2.SC = w.SC;
+        final_score_2d<METHOD>(m, sens_s, w2, lane, cx, cy, A_fin, score_fin);
+        if (lane == 0) {
+            reinterpret_cast<float4 *>(p.out_xyzA)[e] = make_float4(cx, cy, 0.f, A_fin);
+            p.out_score[e] = score_fin;
+        }
+    }
+}
+
+}  // namespace ants

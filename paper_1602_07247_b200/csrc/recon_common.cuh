@@ -58,6 +58,43 @@ __device__ __forceinline__ float lg2_approx(float x) {
     return y;
 }
 
+// ---- packed FP32 pairs (Blackwell FFMA2 / FADD2 / FMUL2: one issue slot, two lanes of work) ----
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pk(float lo, float hi) {
+    f32x2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ f32x2 pk1(float v) { return pk(v, v); }
+__device__ __forceinline__ void upk(f32x2 v, float &lo, float &hi) {
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {
+    f32x2 r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) {
+    f32x2 r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) {
+    f32x2 r;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) {
+    f32x2 r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ float hsum2(f32x2 v) {
+    float a, b;
+    upk(v, a, b);
+    return a + b;
+}
+
 __device__ __forceinline__ float warp_sum(float v) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
@@ -79,6 +116,18 @@ __device__ __forceinline__ void warp_argmin(float &s, int &idx) {
         s = take ? os : s;
         idx = take ? oi : idx;
     }
+}
+
+// same result as warp_argmin through two integer reductions (REDUX): scores mapped to order-preserving
+// unsigned keys, then the lowest index among the lanes holding the minimum.  s must not be NaN.
+__device__ __forceinline__ void warp_argmin_redux(float &s, int &idx) {
+    unsigned b = s == 0.f ? 0u : __float_as_uint(s);   // -0 and +0 tie
+    unsigned key = (b & 0x80000000u) ? ~b : (b | 0x80000000u);
+    unsigned kmin = __reduce_min_sync(kFull, key);
+    int cand = key == kmin ? idx : 0x7fffffff;
+    idx = __reduce_min_sync(kFull, cand);
+    unsigned bm = (kmin & 0x80000000u) ? (kmin & 0x7fffffffu) : ~kmin;
+    s = __uint_as_float(bm);
 }
 
 // round-to-nearest interval index k and centred local coordinate v of t in [-0.5, tmax]

@@ -5,7 +5,7 @@ namespace ants {
 
 // METHOD 0 Poisson ML, 1 weighted chi-square.  Requires every LRF strictly positive (host-checked).
 template <int NPT, int METHOD>
-__global__ void __launch_bounds__(256) recon2d_pk_kernel(const Params p) {
+__global__ void __launch_bounds__(256, (NPT <= 3 ? 3 : 2)) recon2d_pk_kernel(const Params p) {
     extern __shared__ __align__(16) unsigned char smem[];
     const ModelDev &m = p.m;
     const int N = m.N, nr1 = m.n_r + 1, Np = (N + 1) / 2;
@@ -31,6 +31,7 @@ __global__ void __launch_bounds__(256) recon2d_pk_kernel(const Params p) {
     WarpSmemPk w = carve_pk(smem + (cta_smem_bytes_pk(N, rows) + 15) / 16 * 16 +
                             (size_t)warp * warp_smem_bytes_pk(N, METHOD), N, METHOD);
     const int np1 = pk_pairs(N);
+    const unsigned poly_base = (unsigned)__cvta_generic_to_shared(poly_s) - ((unsigned)kMagicBits << 4);
 
     // this lane's nodes: offsets from the grid centre in units of the step
     const float half = 0.5f * (float)(p.G - 1);
@@ -126,9 +127,13 @@ __global__ void __launch_bounds__(256) recon2d_pk_kernel(const Params p) {
                     float v = __shfl_sync(kFull, mine, bi & 31);
                     A_ref = METHOD == 0 ? sumS / v : v;
                 }
-                int iy = bi / p.G, ix = bi - iy * p.G;
-                cx = fmaf((float)ix - half, h, cx);
-                cy = fmaf((float)iy - half, h, cy);
+                // the winner's grid offsets live in its owner lane (no integer division here)
+                float wx = 0.f, wy = 0.f;
+#pragma unroll
+                for (int j = 0; j < NPT; ++j)
+                    if ((bi >> 5) == j) { wx = fx[j]; wy = fy[j]; }
+                cx = fmaf(__shfl_sync(kFull, wx, bi & 31), h, cx);
+                cy = fmaf(__shfl_sync(kFull, wy, bi & 31), h, cy);
             }
             if (p.out_path && lane == 0) p.out_path[e * p.K + k] = found ? (uint16_t)bi : (uint16_t)0xFFFF;
             h *= p.factor;

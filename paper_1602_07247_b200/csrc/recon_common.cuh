@@ -137,6 +137,13 @@ __device__ __forceinline__ void split_t(float t, int &k, float &v) {
     v = t - (tm - kMagic);
 }
 
+// 16-byte shared-memory load from a 32-bit shared address
+__device__ __forceinline__ float4 lds128(unsigned addr) {
+    float4 v;
+    asm("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+    return v;
+}
+
 __device__ __forceinline__ float horner(const float4 p, float v) {
     return fmaf(fmaf(fmaf(p.w, v, p.z), v, p.y), v, p.x);
 }

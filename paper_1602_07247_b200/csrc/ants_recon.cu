@@ -376,6 +376,28 @@ static int first_diff_iter(const ants_lrf *h, const ants_grid_params_t *g, int32
     return g->n_iter;
 }
 
+// CTA shape: the warps-per-CTA in {8, 4, 2, 1} that lets the most warps share an SM's shared memory
+// (each CTA carries its own copy of the model tables; 1 KB per CTA is reserved by the driver).
+// ANTS_WARPS_PER_CTA in the environment overrides the choice (tuning knob, not needed in production).
+static void pick_cta_shape(size_t tables, size_t per_warp, Plan &pl) {
+    const size_t budget = 227 * 1024;
+    int best = 1, best_total = 0;
+    for (int wp : {8, 4, 2, 1}) {
+        const size_t smem = tables + wp * per_warp;
+        if (smem > budget) continue;
+        int ctas = (int)std::min<size_t>(budget / (smem + 1024), (size_t)(64 / wp));
+        ctas = std::min(ctas, 32);
+        if (ctas * wp > best_total) { best_total = ctas * wp; best = wp; }
+    }
+    if (const char *e = std::getenv("ANTS_WARPS_PER_CTA")) {
+        const int v = std::atoi(e);
+        if (v == 1 || v == 2 || v == 4 || v == 8) best = v;
+    }
+    pl.warps = best;
+    pl.smem = tables + best * per_warp;
+    pl.ctas_per_sm = std::max(1, (int)std::min<size_t>(budget / (pl.smem + 1024), (size_t)(64 / best)));
+}
+
 template <int METHOD>
 static const void *pick3d(int cpl, int gzm) {
 #define ANTS_K3(C, Z) if (cpl == C && gzm == Z) return (const void *)recon3d_kernel<C, Z, METHOD>
@@ -420,12 +442,8 @@ static int make_plan3d(const ants_lrf *h, const ants_grid_params_t *g, int32_t m
     const size_t tables = (size_t)(m.N + (m.n_z + 3) * (m.n_r + 1)) * 16;
     const size_t per_warp = warp_smem_bytes_3d(m.N, Gz, m.n_r + 1);
     const size_t budget = 227 * 1024;
-    pl.warps = 8;
-    while (pl.warps > 1 && tables + pl.warps * per_warp > budget / 2) pl.warps >>= 1;
-    pl.smem = tables + pl.warps * per_warp;
+    pick_cta_shape(tables, per_warp, pl);
     if (pl.smem > budget) return ANTS_ERR_UNSUPPORTED;
-    pl.ctas_per_sm = (int)std::min<size_t>(budget / (pl.smem + 1024), (size_t)(2048 / (pl.warps * 32)));
-    if (pl.ctas_per_sm < 1) pl.ctas_per_sm = 1;
     return ANTS_OK;
 }
 
@@ -453,12 +471,8 @@ static int make_plan(const ants_lrf *h, const ants_grid_params_t *g, int32_t met
                                  : (size_t)(m.N + m.n_lrf * (m.n_r + 1)) * 16;
     const size_t per_warp = packed ? warp_smem_bytes_pk(m.N, method) : warp_smem_bytes_2d(m.N);
     const size_t budget = 227 * 1024;
-    pl.warps = 8;
-    while (pl.warps > 1 && tables + pl.warps * per_warp > budget / 2) pl.warps >>= 1;
-    pl.smem = tables + pl.warps * per_warp;
+    pick_cta_shape(tables, per_warp, pl);
     if (pl.smem > budget) return ANTS_ERR_UNSUPPORTED;
-    pl.ctas_per_sm = (int)std::min<size_t>(budget / (pl.smem + 1024), (size_t)(2048 / (pl.warps * 32)));
-    if (pl.ctas_per_sm < 1) pl.ctas_per_sm = 1;
     return ANTS_OK;
 }
 

@@ -8,7 +8,7 @@ template <int NPT, int METHOD>
 __global__ void __launch_bounds__(256, (NPT <= 3 ? 3 : 2)) recon2d_pk_kernel(const Params p) {
     extern __shared__ __align__(16) unsigned char smem[];
     const ModelDev &m = p.m;
-    const int N = m.N, nr1 = m.n_r + 1, Np = (N + 1) / 2;
+    const int N = m.N, nr1 = m.n_r + 1;
     const bool indiv = m.n_lrf > 1;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int rows = m.n_lrf * nr1;
@@ -16,17 +16,8 @@ __global__ void __launch_bounds__(256, (NPT <= 3 ? 3 : 2)) recon2d_pk_kernel(con
     // ---- CTA-shared tables ----
     float4 *sens_s = reinterpret_cast<float4 *>(smem);
     float4 *poly_s = sens_s + N;
-    float4 *XY2 = poly_s + rows;
-    float2 *G2 = reinterpret_cast<float2 *>(XY2 + Np);
     for (int i = threadIdx.x; i < N; i += blockDim.x) sens_s[i] = m.sens[i];
     for (int i = threadIdx.x; i < rows; i += blockDim.x) poly_s[i] = m.poly[i];
-    for (int q = threadIdx.x; q < Np; q += blockDim.x) {
-        const float4 e = m.sens[2 * q];
-        const bool has_o = 2 * q + 1 < N;
-        const float4 o = has_o ? m.sens[2 * q + 1] : make_float4(0.f, 0.f, 0.f, 0.f);
-        XY2[q] = make_float4(e.x, o.x, e.y, o.y);
-        G2[q] = make_float2(indiv ? 1.f : e.z, has_o ? (indiv ? 1.f : o.z) : 0.f);   // pad: g = 0
-    }
     __syncthreads();
     WarpSmemPk w = carve_pk(smem + (cta_smem_bytes_pk(N, rows) + 15) / 16 * 16 +
                             (size_t)warp * warp_smem_bytes_pk(N, METHOD), N, METHOD);

@@ -107,33 +107,39 @@ __global__ void __launch_bounds__(256) recon3d_kernel(const Params p) {
             }
 
             // ---- a5: argmin over the G^2 * Gz nodes, recentre, contract ----
+            // node code (l << 10) | column keeps the order of the linear index l * G^2 + column (R9)
             float bs = kInf;
             int bi = 0x7fffffff;
 #pragma unroll
             for (int l = 0; l < GZM; ++l)
 #pragma unroll
                 for (int j = 0; j < CPL; ++j)
-                    if (sc_node[j][l] < bs) { bs = sc_node[j][l]; bi = l * ncol + lane + 32 * j; }
-            warp_argmin(bs, bi);
+                    if (sc_node[j][l] < bs) { bs = sc_node[j][l]; bi = (l << 10) | (lane + 32 * j); }
+            warp_argmin_redux(bs, bi);
             const bool found = bs < kInf;
+            const int wl = bi >> 10, wc = bi & 1023;
             if (found) {
-                const int l = bi / ncol, c = bi - l * ncol;
+                // the winner's column offsets (and, in plain mode, its energy) live in the owner lane
+                float wx = 0.f, wy = 0.f, mine = 0.f;
+#pragma unroll
+                for (int j = 0; j < CPL; ++j)
+                    if ((wc >> 5) == j) {
+                        wx = fx[j];
+                        wy = fy[j];
+#pragma unroll
+                        for (int ll = 0; ll < GZM; ++ll)
+                            if (ll == wl) mine = aux_node[j][ll];
+                    }
                 if (plain) {
-                    float mine = 0.f;
-#pragma unroll
-                    for (int ll = 0; ll < GZM; ++ll)
-#pragma unroll
-                        for (int j = 0; j < CPL; ++j)
-                            if (ll == l && (c >> 5) == j) mine = aux_node[j][ll];
-                    float v = __shfl_sync(kFull, mine, c & 31);
+                    float v = __shfl_sync(kFull, mine, wc & 31);
                     A_ref = METHOD == 0 ? sumS / v : v;
                 }
-                int iy = c / p.G, ix = c - iy * p.G;
-                cx = fmaf((float)ix - half, h, cx);
-                cy = fmaf((float)iy - half, h, cy);
-                cz = fmaf((float)l - halfz, hz, cz);
+                cx = fmaf(__shfl_sync(kFull, wx, wc & 31), h, cx);
+                cy = fmaf(__shfl_sync(kFull, wy, wc & 31), h, cy);
+                cz = fmaf((float)wl - halfz, hz, cz);
             }
-            if (p.out_path && lane == 0) p.out_path[e * p.K + k] = found ? (uint16_t)bi : (uint16_t)0xFFFF;
+            if (p.out_path && lane == 0)
+                p.out_path[e * p.K + k] = found ? (uint16_t)(wl * ncol + wc) : (uint16_t)0xFFFF;
             h *= p.factor;
             hz *= p.factor;
             __syncwarp();

@@ -292,7 +292,7 @@ def run_ours(args):
     flops_per_launch = flop_per_pair(cfg) * cfg.pairs_per_event * E
     achieved = flops_per_launch / (launch_ms * 1e-3) / 1e12
     roofline = {"bound": "alu", "kernel": "ants::recon%dd_kernel" % cfg.dim, "achieved": achieved, "peak": peak_tflops,
-                "unit": "TFLOP/s", "frac": achieved / peak_tflops, "traffic": TRAFFIC_BYTES.get(cfg.name),
+                "unit": "TFLOP/s", "frac": achieved / peak_tflops, "traffic": (TRAFFIC_PER_EVENT[cfg.name] * E if cfg.name in TRAFFIC_PER_EVENT else None),
                 "peak_source": "derived: SMs x 128 FP32 lanes x 2 x clocks.max.sm (MEASURED_PEAKS.json has no FP32 entry)",
                 "flop_per_pair_nominal": flop_per_pair(cfg), "pairs_per_s": cfg.pairs_per_event * E / (launch_ms * 1e-3),
                 "algorithmic_bytes_per_launch": E * (4 * cfg.n_sensors + 20),
@@ -325,9 +325,10 @@ def run_ours(args):
     return 0
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the `ncu --set full` capture of the
-# bench command (profiles/; null until captured for that workload)
-TRAFFIC_BYTES: dict = {}
+# dram__bytes_read.sum + dram__bytes_write.sum per event from the `ncu --set full` captures of the bench
+# command (profiles/r01_ncu_final.md); `traffic` = this x the events of one launch.  Config 1 was not captured.
+TRAFFIC_PER_EVENT = {"cfg2_pmt2d_hex19": 84.07, "cfg3_sipm_chi2_sq64": 257.5, "cfg4_axialz3d_hex37": 148.7,
+                     "cfg5_flood_hex127": 540.9}
 
 
 def main(argv=None):

@@ -23,6 +23,7 @@
 #pragma once
 #include "../../include/ants_recon.h"
 #include "recon2d.cuh"
+#include "recon2d_pk.cuh"
 
 namespace ants {
 

@@ -534,6 +534,10 @@ static int launch(const ants_lrf *h, const float *signals, int64_t n_events, con
         cudaGetLastError();
         return ANTS_ERR_CUDA;
     }
+    if (const char *e = std::getenv("ANTS_MAX_CTAS_PER_SM")) {   // tuning knob: fewer resident CTAs
+        const int v = std::atoi(e);
+        if (v >= 1 && v < occ) occ = v;
+    }
     long long want = (n_events + pl.warps - 1) / pl.warps;
     long long cap = (long long)h->sm_count * occ;
     int grid = (int)std::min(want, cap);

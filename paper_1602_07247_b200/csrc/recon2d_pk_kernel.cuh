@@ -40,13 +40,22 @@ __global__ void __launch_bounds__(256, (NPT <= 3 ? 3 : 2)) recon2d_pk_kernel(con
     const f32x2 sc2 = pk1(m.sc), of2 = pk1(m.of), magic2 = pk1(kMagic), nmagic2 = pk1(-kMagic);
 
     const long long stride = (long long)gridDim.x * p.warps_per_cta;
+    // the next event's signals are fetched into registers (4 per lane: N <= 128) while this one runs
+    float pf[4];
+    auto prefetch = [&](long long ev) {
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            const int i = lane + 32 * c;
+            pf[c] = (ev < p.n_events && i < N) ? __ldg(p.signals + ev * N + i) : 0.f;
+        }
+    };
+    prefetch((long long)blockIdx.x * p.warps_per_cta + warp);
     for (long long e = (long long)blockIdx.x * p.warps_per_cta + warp; e < p.n_events; e += stride) {
         // ---- a1: load signals (coalesced), prepare, centroid ----
         const float *sig = p.signals + e * N;
         float sumS = 0.f, sw = 0.f, sxw = 0.f, syw = 0.f;
         bool finite = true;
-        for (int i = lane; i < N; i += 32) {
-            float S = __ldg(sig + i);
+        auto take = [&](int i, float S) {
             finite = finite && (fabsf(S) <= 3.402823466e38f);
             if (METHOD == 0) S = fmaxf(S, 0.f);          // R18
             float4 sn = sens_s[i];
@@ -58,7 +67,15 @@ __global__ void __launch_bounds__(256, (NPT <= 3 ? 3 : 2)) recon2d_pk_kernel(con
             float cs = 0.f;
             if (METHOD == 0 && S > 0.f) cs = log2f(S * sn.w);
             w.SC[i] = make_float2(S, cs);
-        }
+        };
+        float cur[4];
+#pragma unroll
+        for (int c = 0; c < 4; ++c) cur[c] = pf[c];
+        prefetch(e + stride);
+#pragma unroll
+        for (int c = 0; c < 4; ++c)
+            if (lane + 32 * c < N) take(lane + 32 * c, cur[c]);
+        for (int i = lane + 128; i < N; i += 32) take(i, __ldg(sig + i));
         finite = __all_sync(kFull, finite);
         sumS = warp_sum(sumS);
         sw = warp_sum(sw);
@@ -84,11 +101,11 @@ __global__ void __launch_bounds__(256, (NPT <= 3 ? 3 : 2)) recon2d_pk_kernel(con
             for (int i = lane; i < N; i += 32) {
                 float4 sn = sens_s[i];
                 float dx = cx - sn.x, dy = cy - sn.y;
-                float s = eval_axial(m, poly_s, i, sqrtf(fmaf(dx, dx, dy * dy)));
+                float s = eval_axial(m, poly_s, i, sqrt_approx(fmaf(dx, dx, dy * dy)));
                 sl += (indiv ? 1.f : sn.z) * s;
             }
             sl = warp_sum(sl);
-            A_ref = sl > 0.f ? sumS / sl : 1.f;
+            A_ref = sl > 0.f ? sumS * rcp_approx(sl) : 1.f;   // only conditions the plain score
         }
 
         float h = p.h0_xy;
@@ -116,7 +133,7 @@ __global__ void __launch_bounds__(256, (NPT <= 3 ? 3 : 2)) recon2d_pk_kernel(con
                     for (int j = 0; j < NPT; ++j)
                         if ((bi >> 5) == j) mine = aux_node[j];
                     float v = __shfl_sync(kFull, mine, bi & 31);
-                    A_ref = METHOD == 0 ? sumS / v : v;
+                    A_ref = METHOD == 0 ? sumS * rcp_approx(v) : v;
                 }
                 // the winner's grid offsets live in its owner lane (no integer division here)
                 float wx = 0.f, wy = 0.f;

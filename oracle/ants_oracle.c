@@ -36,7 +36,9 @@
  * reproduction by blossoming, scipy BSpline agreement, separable tensor
  * product, centroid special cases, energy vs 1-D minimisation, D >= 0 and
  * D = 0 iff mu = S, K=1 vs numpy argmin, lattice brute force, noise-free
- * recovery, mirror symmetry, power-of-two scaling.  The greedy search itself
+ * recovery, mirror symmetry, power-of-two scaling; sensor selection (passive,
+ * signal threshold, distance from start; tests/test_oracle_selection.py) against
+ * the detector rebuilt without the ignored sensors.  The greedy search itself
  * (whether a noisy event reaches its global minimum) is a property of the
  * heuristic: "parity unpinned" beyond those pins.
  */
@@ -58,6 +60,12 @@ typedef struct {
     const float *gains;      /* [N] */
     const float *knots;      /* {r_lo,r_hi[,z_lo,z_hi]} */
     const float *coeffs;     /* [n_lrf][n_int_z+3 or 1][n_int_r+3] */
+    /* sensor selection (section 5.3 passive photosensors; section 5.1.2
+     * "ignore photosensors with the signals below a certain threshold or situated further than a
+     * given distance from the initial search position"); reading R19 in DESIGN.md */
+    const uint8_t *passive;  /* [N] non-zero = passive, or NULL (none) */
+    float signal_min;        /* sensors with S < signal_min are ignored; -inf (or NaN) = off */
+    float dist_max;          /* sensors farther than this from the start position are ignored; +inf (NaN) = off */
 } oracle_model_t;
 
 typedef struct {
@@ -140,6 +148,28 @@ static void prepare_signals(const float *sig, int N, int method, double *S)
     }
 }
 
+/* sensor i takes part in the centroid unless it is passive */
+static int not_passive(const oracle_model_t *m, int i) { return !(m->passive && m->passive[i]); }
+
+/* active[i] = 1 if sensor i takes part in the statistical reconstruction of this event (R19): not
+ * passive, signal (as the method sees it) >= signal_min, axis within dist_max of the start position.
+ * Returns the number of active sensors. */
+static int select_sensors(const oracle_model_t *m, const double *S, const double *start_xy, uint8_t *active)
+{
+    int n = 0;
+    for (int i = 0; i < m->n_sensors; ++i) {
+        int a = not_passive(m, i);
+        if (a && !isnan(m->signal_min) && S[i] < (double)m->signal_min) a = 0;
+        if (a && !isnan(m->dist_max)) {
+            double dx = start_xy[0] - (double)m->sensor_xy[2 * i], dy = start_xy[1] - (double)m->sensor_xy[2 * i + 1];
+            if (sqrt(dx * dx + dy * dy) > (double)m->dist_max) a = 0;
+        }
+        active[i] = (uint8_t)a;
+        n += a;
+    }
+    return n;
+}
+
 /* ---- centroid: x = sum X_i S_i/g_i / sum S_i/g_i ----------
  * returns 0 ok, 1 event unusable (non-finite signal, sum S <= 0 or sum S/g <= 0) */
 int oracle_centroid(const oracle_model_t *m, const float *sig, int method, double *xy)
@@ -150,6 +180,7 @@ int oracle_centroid(const oracle_model_t *m, const float *sig, int method, doubl
     int bad = 0;
     prepare_signals(sig, N, method, S);
     for (int i = 0; i < N; ++i) {
+        if (!not_passive(m, i)) continue;             /* passive sensors are ignored altogether */
         if (!isfinite(S[i])) bad = 1;
         double w = S[i] / (double)m->gains[i];
         sx += (double)m->sensor_xy[2 * i] * w;
@@ -171,21 +202,23 @@ int oracle_centroid(const oracle_model_t *m, const float *sig, int method, doubl
  *       D = 2 sum_i t_i, t_i = mu_i - S_i - S_i ln(mu_i/S_i) (S_i>0), mu_i (S_i=0)
  *   chi-square (R3,R4): w_i = 1/max(S_i,1), A = sum w S L / sum w L^2,
  *       chi2 = sum w (S - A L)^2                                             */
-static int score_prepared(const oracle_model_t *m, const double *S, int method,
+static int score_prepared(const oracle_model_t *m, const double *S, const uint8_t *active, int method,
                           double x, double y, double z, double *L, double *A_out, double *score_out)
 {
+#define ACTIVE(i) (!active || active[i])   /* sums run over the event's active sensors only (R19) */
     int N = m->n_sensors;
     double sumL = 0.0;
     *A_out = NAN;
     *score_out = INFINITY;
     if (m->lrf_dim == 2 && !(z >= (double)m->knots[2] && z <= (double)m->knots[3])) return 1; /* R6 */
-    for (int i = 0; i < N; ++i) { L[i] = oracle_lrf(m, i, x, y, z); sumL += L[i]; }
+    for (int i = 0; i < N; ++i) { if (!ACTIVE(i)) continue; L[i] = oracle_lrf(m, i, x, y, z); sumL += L[i]; }
     if (!(sumL > 0.0)) return 1;
     if (method == 0) {
         double sumS = 0.0, D = 0.0;
-        for (int i = 0; i < N; ++i) sumS += S[i];
+        for (int i = 0; i < N; ++i) if (ACTIVE(i)) sumS += S[i];
         double A = sumS / sumL;
         for (int i = 0; i < N; ++i) {
+            if (!ACTIVE(i)) continue;
             double mu = A * L[i];
             if (S[i] > 0.0) {
                 if (!(L[i] > 0.0)) return 1;
@@ -199,6 +232,7 @@ static int score_prepared(const oracle_model_t *m, const double *S, int method,
     } else {
         double swsl = 0.0, swll = 0.0, chi2 = 0.0;
         for (int i = 0; i < N; ++i) {
+            if (!ACTIVE(i)) continue;
             double w = 1.0 / (S[i] > 1.0 ? S[i] : 1.0);
             swsl += w * S[i] * L[i];
             swll += w * L[i] * L[i];
@@ -206,6 +240,7 @@ static int score_prepared(const oracle_model_t *m, const double *S, int method,
         if (!(swll > 0.0)) return 1;
         double A = swsl / swll;
         for (int i = 0; i < N; ++i) {
+            if (!ACTIVE(i)) continue;
             double w = 1.0 / (S[i] > 1.0 ? S[i] : 1.0);
             double d = S[i] - A * L[i];
             chi2 += w * d * d;
@@ -214,16 +249,36 @@ static int score_prepared(const oracle_model_t *m, const double *S, int method,
         *score_out = chi2;
     }
     return 0;
+#undef ACTIVE
 }
+
+/* needs_selection: any of the three selection options is on */
+static int needs_selection(const oracle_model_t *m)
+{
+    return m->passive || !isnan(m->signal_min) || !isnan(m->dist_max);
+}
+
+int oracle_centroid(const oracle_model_t *m, const float *sig, int method, double *xy);
 
 int oracle_score_at(const oracle_model_t *m, const float *sig, int method,
                     double x, double y, double z, double *A_out, double *score_out)
 {
     int N = m->n_sensors;
     double *S = (double *)malloc(sizeof(double) * 2 * N);
+    uint8_t *active = 0;
     prepare_signals(sig, N, method, S);
-    int rc = score_prepared(m, S, method, x, y, z, S + N, A_out, score_out);
+    if (needs_selection(m)) {           /* the event's active set hangs on its start position (R19) */
+        double xy[2];
+        active = (uint8_t *)malloc((size_t)N);
+        if (oracle_centroid(m, sig, method, xy) || select_sensors(m, S, xy, active) == 0) {
+            *A_out = NAN; *score_out = INFINITY;
+            free(S); free(active);
+            return 1;
+        }
+    }
+    int rc = score_prepared(m, S, active, method, x, y, z, S + N, A_out, score_out);
     free(S);
+    free(active);
     return rc;
 }
 
@@ -255,6 +310,19 @@ static void reconstruct_one(const oracle_model_t *m, const float *sig, const ora
         return;
     }
     prepare_signals(sig, N, method, S);
+    uint8_t *active = 0;
+    if (needs_selection(m)) {
+        active = (uint8_t *)malloc((size_t)N);
+        double ssum = 0.0;
+        int n_act = select_sensors(m, S, xy, active);
+        for (int i = 0; i < N; ++i) if (active[i]) ssum += S[i];
+        if (n_act == 0 || !(ssum > 0.0)) {              /* nothing left to reconstruct from */
+            xyzA[0] = xyzA[1] = xyzA[2] = xyzA[3] = NAN;
+            *score = INFINITY;
+            free(active);
+            return;
+        }
+    }
     c[0] = xy[0]; c[1] = xy[1]; c[2] = start_z(m, g);
     double h_xy = (double)g->step0_xy, h_z = (double)g->step0_z;   /* h_k = h_0 f^k (R1) */
     double half = 0.5 * (G - 1);
@@ -267,7 +335,7 @@ static void reconstruct_one(const oracle_model_t *m, const float *sig, const ora
                     double p[3] = { c[0] + (ix - half) * h_xy, c[1] + (iy - half) * h_xy,
                                     g->dim == 3 ? c[2] + (iz - half) * h_z : c[2] };
                     double A, sc;
-                    if (score_prepared(m, S, method, p[0], p[1], p[2], L, &A, &sc)) continue;
+                    if (score_prepared(m, S, active, method, p[0], p[1], p[2], L, &A, &sc)) continue;
                     if (sc < best) {               /* first strict minimum (R9) */
                         second = best;
                         best = sc; best_idx = (iz * G + iy) * G + ix;
@@ -285,7 +353,8 @@ static void reconstruct_one(const oracle_model_t *m, const float *sig, const ora
     }
     /* result = last best node, its energy and score (R11) */
     xyzA[0] = c[0]; xyzA[1] = c[1]; xyzA[2] = c[2];
-    score_prepared(m, S, method, c[0], c[1], c[2], L, &xyzA[3], score);
+    score_prepared(m, S, active, method, c[0], c[1], c[2], L, &xyzA[3], score);
+    free(active);
 }
 
 /* threads a call with this n_threads argument uses */

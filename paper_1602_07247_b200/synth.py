@@ -134,6 +134,10 @@ class Config:
     noise_sigma: float = 0.0         # Gaussian electronic noise, result clipped at 0
     n_batches: int = 1
     seed: int = 0
+    # sensor selection (PAPER.md:358 passive photosensors; PAPER.md:318 signal threshold / distance from start)
+    passive: Optional[np.ndarray] = None     # [N] bool/uint8, non-zero = passive
+    signal_min: float = float("nan")         # NaN = off
+    dist_max: float = float("nan")           # NaN = off
 
     @property
     def n_sensors(self) -> int:

@@ -87,6 +87,22 @@ typedef struct {
 } ants_grid_params_t;
 
 /*
+ * ants_lrf_set_selection -- which sensors take part (R19).
+ *   passive    HOST [N] bytes, non-zero = passive photosensor (section 5.3: "ignored during
+ *              position reconstruction procedures"): left out of the centroid and of every sum; its
+ *              signal is never looked at.  NULL = none.
+ *   signal_min sensors whose signal (as the method sees it) is below this are ignored in the statistical
+ *              part (section 5.1.2); NaN = off.
+ *   dist_max   sensors whose axis is farther than this (mm) from the start position (the centroid of the
+ *              non-passive sensors) are ignored in the statistical part; NaN = off.
+ * The active set is fixed per event before the grid search.  An event with no sensor left, or with
+ * sum S <= 0 over them, fails (NaN row, score +inf).  Must not be called while a reconstruction that
+ * uses the handle is in flight.  Errors: ANTS_ERR_INVALID (NULL handle), ANTS_ERR_CUDA, ANTS_ERR_NOMEM;
+ * ants_reconstruct then returns ANTS_ERR_UNSUPPORTED for an LRF that is not strictly positive.
+ */
+int ants_lrf_set_selection(ants_lrf_t *lrf, const uint8_t *passive, float signal_min, float dist_max);
+
+/*
  * ants_reconstruct -- steps a1..a6 for a batch of events, ONE kernel launch,
  * asynchronous on `cuda_stream`, no allocation, no host synchronisation.
  *   signals   DEVICE [n_events][N] float row-major, caller-owned, read-only.

@@ -29,7 +29,7 @@ struct ants_lrf {
     double max_dlog = 0.0;   // max |d ln s / dr| over the domain, 1/mm (only if positive)
     double max_dlog_z = 0.0; // axial+z: max |d ln s / dz|, 1/mm
     double knot_r = 0.0, knot_z = 0.0;   // knot spacing, mm
-    void *d_sens = nullptr, *d_poly = nullptr, *d_polyd = nullptr;
+    void *d_sens = nullptr, *d_poly = nullptr, *d_polyd = nullptr, *d_passive = nullptr;
     // scratch of ants_reconstruct_host (lazily allocated, reused, guarded)
     std::mutex host_mu;
     int64_t scratch_events = 0;
@@ -271,7 +271,34 @@ extern "C" int ants_lrf_create(const float *sensor_xy, const float *gains, const
     m.z_lo = z_lo;
     m.z_hi = z_hi;
     m.scz = dim == 2 ? (float)((double)n_z / ((double)z_hi - (double)z_lo)) : 0.f;
+    m.passive = nullptr;
+    m.signal_min = m.dist_max = std::nanf("");
+    m.select = 0;
     *out = h;
+    return ANTS_OK;
+}
+
+extern "C" int ants_lrf_set_selection(ants_lrf_t *h, const uint8_t *passive, float signal_min, float dist_max) {
+    if (!h) return ANTS_ERR_INVALID;
+    ModelDev &m = h->dev;
+    if (passive) {
+        if (!h->d_passive && cudaMalloc(&h->d_passive, (size_t)m.N) != cudaSuccess) {
+            cudaGetLastError();
+            return ANTS_ERR_NOMEM;
+        }
+        std::vector<unsigned char> flags(m.N);
+        for (int i = 0; i < m.N; ++i) flags[i] = passive[i] ? 1 : 0;
+        if (cudaMemcpy(h->d_passive, flags.data(), (size_t)m.N, cudaMemcpyHostToDevice) != cudaSuccess) {
+            cudaGetLastError();
+            return ANTS_ERR_CUDA;
+        }
+        m.passive = (const unsigned char *)h->d_passive;
+    } else {
+        m.passive = nullptr;
+    }
+    m.signal_min = signal_min;
+    m.dist_max = dist_max;
+    m.select = (m.passive || !std::isnan(signal_min) || !std::isnan(dist_max)) ? 1 : 0;
     return ANTS_OK;
 }
 
@@ -280,6 +307,7 @@ extern "C" void ants_destroy(ants_lrf_t *h) {
     cudaFree(h->d_sens);
     cudaFree(h->d_poly);
     cudaFree(h->d_polyd);
+    cudaFree(h->d_passive);
     for (int s = 0; s < 3; ++s) {
         cudaFree(h->d_sig[s]);
         cudaFree(h->d_xyzA[s]);
@@ -461,6 +489,7 @@ static int make_plan(const ants_lrf *h, const ants_grid_params_t *g, int32_t met
     if (!pl.npt) return ANTS_ERR_UNSUPPORTED;
     // strictly positive LRFs (the normal case) run the sensor-pair-packed kernel; others the generic one
     const bool packed = h->positive;
+    if (!packed && m.select) return ANTS_ERR_UNSUPPORTED;   // the generic kernel has no sensor selection
     if (packed)
         pl.kernel = method == ANTS_POISSON_ML ? pick2d_pk<0>(pl.npt) : pick2d_pk<1>(pl.npt);
     else

@@ -56,6 +56,10 @@ __global__ void __launch_bounds__(256, (NPT <= 3 ? 3 : 2)) recon2d_pk_kernel(con
         float sumS = 0.f, sw = 0.f, sxw = 0.f, syw = 0.f;
         bool finite = true;
         auto take = [&](int i, float S) {
+            if (m.passive && m.passive[i]) {             // R19: out of everything, signal not looked at
+                w.SC[i] = make_float2(0.f, ANTS_QNAN);
+                return;
+            }
             finite = finite && (fabsf(S) <= 3.402823466e38f);
             if (METHOD == 0) S = fmaxf(S, 0.f);          // R18
             float4 sn = sens_s[i];
@@ -94,6 +98,33 @@ __global__ void __launch_bounds__(256, (NPT <= 3 ? 3 : 2)) recon2d_pk_kernel(con
         }
         float cx = sxw / sw, cy = syw / sw;
 
+        if (m.select) {
+            // R19: the sensors of the statistical part, fixed for the event: signal threshold and
+            // distance from the start position; sum S runs over them
+            float s_act = 0.f;
+            for (int i = lane; i < N; i += 32) {
+                float2 sc = w.SC[i];
+                if (sc.y == sc.y) {
+                    const float4 sn = sens_s[i];
+                    const float dx = cx - sn.x, dy = cy - sn.y;
+                    const bool keep = !(sc.x < m.signal_min) && !(sqrtf(fmaf(dx, dx, dy * dy)) > m.dist_max);
+                    if (keep) s_act += sc.x;
+                    else w.SC[i] = make_float2(0.f, ANTS_QNAN);
+                }
+            }
+            sumS = warp_sum(s_act);
+            __syncwarp();
+            if (!(sumS > 0.f)) {
+                if (lane == 0) {
+                    reinterpret_cast<float4 *>(p.out_xyzA)[e] = make_float4(ANTS_QNAN, ANTS_QNAN, ANTS_QNAN, ANTS_QNAN);
+                    p.out_score[e] = kInf;
+                }
+                if (p.out_path)
+                    for (int k = lane; k < p.K; k += 32) p.out_path[e * p.K + k] = 0xFFFF;
+                continue;
+            }
+        }
+
         // reference energy for the plain score: A at the seed
         float A_ref;
         {
@@ -102,7 +133,7 @@ __global__ void __launch_bounds__(256, (NPT <= 3 ? 3 : 2)) recon2d_pk_kernel(con
                 float4 sn = sens_s[i];
                 float dx = cx - sn.x, dy = cy - sn.y;
                 float s = eval_axial(m, poly_s, i, sqrt_approx(fmaf(dx, dx, dy * dy)));
-                sl += (indiv ? 1.f : sn.z) * s;
+                if (w.SC[i].y == w.SC[i].y) sl += (indiv ? 1.f : sn.z) * s;
             }
             sl = warp_sum(sl);
             A_ref = sl > 0.f ? sumS * rcp_approx(sl) : 1.f;   // only conditions the plain score

@@ -82,6 +82,8 @@ __device__ void final_score_3d(const ModelDev &m, const float4 *sens_s, const Wa
     double sumL = 0.0, sumS = 0.0, swsl = 0.0, swll = 0.0;
     __syncwarp();
     for (int i = lane; i < m.N; i += 32) {
+        Ld[i] = 0.0;
+        if (!(w.SC[i].y == w.SC[i].y)) continue;            // R19: inactive sensor
         float4 sn = sens_s[i];
         double dx = (double)cx - (double)sn.x, dy = (double)cy - (double)sn.y;
         double r = sqrt(dx * dx + dy * dy);
@@ -113,6 +115,7 @@ __device__ void final_score_3d(const ModelDev &m, const float4 *sens_s, const Wa
     if (METHOD == 0) {
         A = sumS / sumL;
         for (int i = lane; i < m.N; i += 32) {
+            if (!(w.SC[i].y == w.SC[i].y)) continue;
             double L = Ld[i], S = (double)w.SC[i].x, mu = A * L;
             if (S > 0.0) {
                 if (!(L > 0.0)) bad = true;
@@ -128,6 +131,7 @@ __device__ void final_score_3d(const ModelDev &m, const float4 *sens_s, const Wa
         if (!(swll > 0.0)) bad = true;
         A = swsl / swll;
         for (int i = lane; i < m.N; i += 32) {
+            if (!(w.SC[i].y == w.SC[i].y)) continue;
             double L = Ld[i], S = (double)w.SC[i].x;
             double d = S - A * L;
             sc += d * d / fmax(S, 1.0);

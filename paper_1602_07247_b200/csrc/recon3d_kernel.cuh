@@ -46,6 +46,10 @@ __global__ void __launch_bounds__(256) recon3d_kernel(const Params p) {
         float sumS = 0.f, sw = 0.f, sxw = 0.f, syw = 0.f;
         bool finite = true;
         for (int i = lane; i < N; i += 32) {
+            if (m.passive && m.passive[i]) {             // R19: out of everything, signal not looked at
+                w.SC[i] = make_float2(0.f, ANTS_QNAN);
+                continue;
+            }
             float S = __ldg(sig + i);
             finite = finite && (fabsf(S) <= 3.402823466e38f);
             if (METHOD == 0) S = fmaxf(S, 0.f);          // R18
@@ -77,6 +81,31 @@ __global__ void __launch_bounds__(256) recon3d_kernel(const Params p) {
         }
         float cx = sxw / sw, cy = syw / sw, cz = z_start;
         float A_ref = 1.f;
+        if (m.select) {
+            // R19: the sensors of the statistical part, fixed for the event (threshold, distance from start)
+            float s_act = 0.f;
+            for (int i = lane; i < N; i += 32) {
+                float2 sc = w.SC[i];
+                if (sc.y == sc.y) {
+                    const float4 sn = sens_s[i];
+                    const float dx = cx - sn.x, dy = cy - sn.y;
+                    const bool keep = !(sc.x < m.signal_min) && !(sqrtf(fmaf(dx, dx, dy * dy)) > m.dist_max);
+                    if (keep) s_act += sc.x;
+                    else w.SC[i] = make_float2(0.f, ANTS_QNAN);
+                }
+            }
+            sumS = warp_sum(s_act);
+            __syncwarp();
+            if (!(sumS > 0.f)) {
+                if (lane == 0) {
+                    reinterpret_cast<float4 *>(p.out_xyzA)[e] = make_float4(ANTS_QNAN, ANTS_QNAN, ANTS_QNAN, ANTS_QNAN);
+                    p.out_score[e] = kInf;
+                }
+                if (p.out_path)
+                    for (int k = lane; k < p.K; k += 32) p.out_path[e * p.K + k] = 0xFFFF;
+                continue;
+            }
+        }
 
         float h = p.h0_xy, hz = p.h0_z;
         for (int k = 0; k < p.K; ++k) {
@@ -91,7 +120,7 @@ __global__ void __launch_bounds__(256) recon3d_kernel(const Params p) {
                     int kk;
                     float v;
                     split_t(t, kk, v);
-                    sl = fmaf(sn.z, horner(w.Tc[kk], v), sl);
+                    if (w.SC[i].y == w.SC[i].y) sl = fmaf(sn.z, horner(w.Tc[kk], v), sl);
                 }
                 sl = warp_sum(sl);
                 A_ref = sl > 0.f ? sumS / sl : 1.f;

@@ -24,7 +24,15 @@ struct ModelDev {
     int N, n_lrf, n_r, n_z;
     float r_lo, r_hi, sc, of, tmax;   // sc = n_r/(r_hi - r_lo); of = -r_lo*sc - 0.5; tmax = n_r - 0.5
     float z_lo, z_hi, scz;            // scz = n_z/(z_hi - z_lo)
+    // sensor selection (R19): passive[i] != 0 -> sensor left out of everything; signal_min / dist_max
+    // (NaN = off) pick the sensors of the statistical part per event; select = any of the three is on
+    const unsigned char *passive;     // device [N] or nullptr
+    float signal_min, dist_max;
+    int select;
 };
+
+// an inactive sensor of the current event is flagged by a NaN in SC[i].y
+#define ANTS_QNAN (__int_as_float(0x7fc00000))
 
 struct Params {
     ModelDev m;

@@ -55,6 +55,8 @@ def load():
     lib.ants_reconstruct_trace.argtypes = [vp, vp, C.c_int64, C.POINTER(GridParams), C.c_int32, vp, vp, vp, vp]
     lib.ants_reconstruct_host.restype = C.c_int
     lib.ants_reconstruct_host.argtypes = [vp, vp, C.c_int64, C.POINTER(GridParams), C.c_int32, vp, vp, C.c_int64]
+    lib.ants_lrf_set_selection.restype = C.c_int
+    lib.ants_lrf_set_selection.argtypes = [vp, vp, C.c_float, C.c_float]
     lib.ants_destroy.restype = None
     lib.ants_destroy.argtypes = [vp]
     lib.ants_strerror.restype = C.c_char_p
@@ -89,6 +91,15 @@ def ants_lrf_create(sensor_xy, gains, knots, coeffs, dims: LrfDims) -> int:
     if rc != 0:
         raise AntsError(rc, "ants_lrf_create")
     return out.value
+
+
+def ants_lrf_set_selection(handle, passive=None, signal_min=float("nan"), dist_max=float("nan")) -> None:
+    """passive: host bool/uint8 [N] or None; signal_min / dist_max: NaN = off (include/ants_recon.h)."""
+    pm = None if passive is None else np.ascontiguousarray(np.asarray(passive) != 0, dtype=np.uint8)
+    rc = load().ants_lrf_set_selection(handle, None if pm is None else pm.ctypes.data, float(signal_min),
+                                       float(dist_max))
+    if rc != 0:
+        raise AntsError(rc, "ants_lrf_set_selection")
 
 
 def ants_destroy(handle) -> None:
@@ -144,6 +155,10 @@ class Reconstructor:
                                cfg.n_iter, 0, cfg.z_seed)
         self.method = int(cfg.method)
         self.handle = ants_lrf_create(cfg.sensor_xy, cfg.gains, cfg.knots, cfg.coeffs, self.dims)
+        passive = getattr(cfg, "passive", None)
+        smin, dmax = getattr(cfg, "signal_min", float("nan")), getattr(cfg, "dist_max", float("nan"))
+        if passive is not None or smin == smin or dmax == dmax:
+            ants_lrf_set_selection(self.handle, passive, smin, dmax)
 
     def __call__(self, signals, trace: bool = False, stream=None):
         import torch

@@ -287,3 +287,68 @@ def test_axial_z_seed_outside_range_gives_invalid_nodes():
     model = oracle.Model.from_config(cfg)
     ref = oracle.reconstruct(model, ev["signals"].cpu().numpy(), oracle.grid_from_config(cfg), cfg.method)
     assert np.allclose(ref["xyzA"][:, :2], xyzA[:, :2], atol=1e-4) and np.isposinf(ref["score"]).all()
+
+
+# ---------------------------------------------------------------------------
+# sensor selection (R19; PAPER.md:358 passive sensors, PAPER.md:318 threshold / distance)
+# ---------------------------------------------------------------------------
+def _with_selection(idx, passive=None, signal_min=float("nan"), dist_max=float("nan")):
+    cfg = synth.make_config(idx)
+    if passive is not None:
+        m = np.zeros(cfg.n_sensors, np.uint8)
+        m[list(passive)] = 1
+        cfg.passive = m
+    cfg.signal_min, cfg.dist_max = signal_min, dist_max
+    return cfg
+
+
+@pytest.mark.parametrize("idx,kw", [
+    (2, dict(passive=[2, 5, 11])),
+    (2, dict(signal_min=8.0)),
+    (2, dict(dist_max=47.0)),
+    (5, dict(passive=[0, 63, 126], signal_min=3.0, dist_max=110.0)),
+    (3, dict(passive=[9, 27], signal_min=2.0)),
+    (3, dict(dist_max=20.5)),
+    (1, dict(passive=[3])),
+    (4, dict(passive=[7, 36], signal_min=1.0)),
+    (4, dict(dist_max=95.0)),
+])
+def test_parity_with_sensor_selection(idx, kw):
+    cfg = _with_selection(idx, **kw)
+    n = {1: 4001, 2: 6001, 3: 1501, 4: 2501, 5: 801}[idx]
+    ev = synth.generate_events(synth.make_config(idx), n, device="cuda")
+    sig = ev["signals"].clone()
+    if cfg.passive is not None:                      # a dead channel may read anything
+        bad = torch.from_numpy(np.flatnonzero(cfg.passive)).cuda()
+        sig[::3, bad[0]] = float("nan")
+        sig[1::3, bad[-1]] = 1e30
+    xyzA, score, path = _run(cfg, sig)
+    res = parity_rules.compare(cfg, sig.cpu().numpy(), xyzA, score, path)
+    parity_rules.assert_parity(res, f"cfg{idx} {kw}")
+    assert np.isfinite(xyzA).all(axis=1).mean() > 0.99
+
+
+def test_selection_that_leaves_nothing_fails_the_event():
+    cfg = _with_selection(2, signal_min=1e9)
+    ev = synth.generate_events(synth.make_config(2), 33, device="cuda")
+    xyzA, score, path = _run(cfg, ev["signals"])
+    assert np.isnan(xyzA).all() and np.isposinf(score).all()
+    res = parity_rules.compare(cfg, ev["signals"].cpu().numpy(), xyzA, score, path)
+    assert res["fail_mismatch"] == 0
+
+
+def test_selection_can_be_switched_off_again():
+    cfg = synth.make_config(2)
+    ev = synth.generate_events(cfg, 2048, device="cuda")
+    r = recon.Reconstructor(cfg)
+    try:
+        base = [t.clone() for t in r(ev["signals"])]
+        recon.ants_lrf_set_selection(r.handle, np.arange(cfg.n_sensors) % 5 == 0, 4.0, 50.0)
+        sel = [t.clone() for t in r(ev["signals"])]
+        recon.ants_lrf_set_selection(r.handle, None)
+        again = r(ev["signals"])
+        torch.cuda.synchronize()
+        assert torch.equal(base[0], again[0]) and torch.equal(base[1], again[1])
+        assert not torch.equal(base[0], sel[0])
+    finally:
+        r.close()

@@ -73,7 +73,7 @@ typedef struct {
     int32_t nodes_per_axis;  /* G */
     float step0_xy, step0_z, factor;
     int32_t n_iter;          /* K */
-    int32_t seed_mode;       /* 0 = centroid */
+    int32_t seed_mode;       /* 0 = centroid; 1 = position of the sensor with the strongest signal (R20) */
     float z_seed;            /* NaN => (z_lo+z_hi)/2 */
 } oracle_grid_t;
 
@@ -252,15 +252,38 @@ static int score_prepared(const oracle_model_t *m, const double *S, const uint8_
 #undef ACTIVE
 }
 
+/* ---- start search position ("the position reconstructed with the centroid method
+ * or just the coordinates of the photosensor with the strongest signal").  R20: strongest = largest
+ * signal as the method sees it among the non-passive sensors, first one on ties; the event is
+ * unusable under the same conditions as for the centroid except that sum S/g is not needed.
+ * returns 0 ok, 1 event unusable */
+int oracle_start(const oracle_model_t *m, const float *sig, int method, int seed_mode, double *xy)
+{
+    if (seed_mode == 0) return oracle_centroid(m, sig, method, xy);
+    int N = m->n_sensors, best = -1, bad = 0;
+    double *S = (double *)malloc(sizeof(double) * (size_t)N);
+    double ss = 0.0;
+    prepare_signals(sig, N, method, S);
+    for (int i = 0; i < N; ++i) {
+        if (!not_passive(m, i)) continue;
+        if (!isfinite(S[i])) bad = 1;
+        ss += S[i];
+        if (best < 0 || S[i] > S[best]) best = i;
+    }
+    free(S);
+    if (bad || best < 0 || !(ss > 0.0)) { xy[0] = xy[1] = NAN; return 1; }
+    xy[0] = (double)m->sensor_xy[2 * best];
+    xy[1] = (double)m->sensor_xy[2 * best + 1];
+    return 0;
+}
+
 /* needs_selection: any of the three selection options is on */
 static int needs_selection(const oracle_model_t *m)
 {
     return m->passive || !isnan(m->signal_min) || !isnan(m->dist_max);
 }
 
-int oracle_centroid(const oracle_model_t *m, const float *sig, int method, double *xy);
-
-int oracle_score_at(const oracle_model_t *m, const float *sig, int method,
+int oracle_score_at(const oracle_model_t *m, const float *sig, int method, int seed_mode,
                     double x, double y, double z, double *A_out, double *score_out)
 {
     int N = m->n_sensors;
@@ -270,7 +293,7 @@ int oracle_score_at(const oracle_model_t *m, const float *sig, int method,
     if (needs_selection(m)) {           /* the event's active set hangs on its start position (R19) */
         double xy[2];
         active = (uint8_t *)malloc((size_t)N);
-        if (oracle_centroid(m, sig, method, xy) || select_sensors(m, S, xy, active) == 0) {
+        if (oracle_start(m, sig, method, seed_mode, xy) || select_sensors(m, S, xy, active) == 0) {
             *A_out = NAN; *score_out = INFINITY;
             free(S); free(active);
             return 1;
@@ -304,7 +327,7 @@ static void reconstruct_one(const oracle_model_t *m, const float *sig, const ora
         if (tr_best) tr_best[k] = INFINITY;
         if (tr_second) tr_second[k] = INFINITY;
     }
-    if (oracle_centroid(m, sig, method, xy)) {
+    if (oracle_start(m, sig, method, g->seed_mode, xy)) {
         xyzA[0] = xyzA[1] = xyzA[2] = xyzA[3] = NAN;
         *score = INFINITY;
         return;
@@ -374,9 +397,10 @@ int oracle_reconstruct(const oracle_model_t *m, const float *signals, int64_t n_
                        const oracle_grid_t *g, int method, double *out_xyzA, double *out_score,
                        int32_t *tr_idx, double *tr_best, double *tr_second, int n_threads)
 {
-    if (!m || !g || !out_xyzA || !out_score || n_events < 0) return -1;
+    if (!m || !g || !out_xyzA || !out_score || n_events < 0 || m->n_sensors < 1) return -1;
     if (g->nodes_per_axis < 2 || g->n_iter < 1 || !(g->factor > 0.0f && g->factor < 1.0f)) return -1;
     if (g->dim != 2 && g->dim != 3) return -1;
+    if (g->seed_mode != 0 && g->seed_mode != 1) return -1;
     if (g->dim == 3 && m->lrf_dim != 2) return -1;
     int N = m->n_sensors, K = g->n_iter;
 #ifdef _OPENMP
@@ -399,11 +423,11 @@ int oracle_reconstruct(const oracle_model_t *m, const float *signals, int64_t n_
 /* score_at for many events: pos [E][3] double, A_out/score_out [E] (interface
  * helper for the parity tests; the arithmetic is oracle_score_at's). */
 int oracle_score_at_many(const oracle_model_t *m, const float *signals, int64_t n_events, int method,
-                         const double *pos, double *A_out, double *score_out)
+                         int seed_mode, const double *pos, double *A_out, double *score_out)
 {
     if (!m || !signals || !pos || !A_out || !score_out || n_events < 0) return -1;
     for (int64_t e = 0; e < n_events; ++e)
-        oracle_score_at(m, signals + e * m->n_sensors, method, pos[3 * e], pos[3 * e + 1], pos[3 * e + 2],
+        oracle_score_at(m, signals + e * m->n_sensors, method, seed_mode, pos[3 * e], pos[3 * e + 1], pos[3 * e + 2],
                         A_out + e, score_out + e);
     return 0;
 }

@@ -54,10 +54,12 @@ def _load():
         lib.oracle_centroid.restype = C.c_int
         lib.oracle_centroid.argtypes = [C.POINTER(_Model), C.c_void_p, C.c_int, C.c_void_p]
         lib.oracle_score_at.restype = C.c_int
-        lib.oracle_score_at.argtypes = [C.POINTER(_Model), C.c_void_p, C.c_int, C.c_double, C.c_double,
+        lib.oracle_start.restype = C.c_int
+        lib.oracle_start.argtypes = [C.POINTER(_Model), C.c_void_p, C.c_int, C.c_int, C.c_void_p]
+        lib.oracle_score_at.argtypes = [C.POINTER(_Model), C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_double,
                                         C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         lib.oracle_score_at_many.restype = C.c_int
-        lib.oracle_score_at_many.argtypes = [C.POINTER(_Model), C.c_void_p, C.c_int64, C.c_int,
+        lib.oracle_score_at_many.argtypes = [C.POINTER(_Model), C.c_void_p, C.c_int64, C.c_int, C.c_int,
                                              C.c_void_p, C.c_void_p, C.c_void_p]
         lib.oracle_threads.restype = C.c_int
         lib.oracle_threads.argtypes = [C.c_int]
@@ -125,36 +127,43 @@ class Model:
         rc = _load().oracle_centroid(C.byref(self.c), s.ctypes.data, int(method), xy.ctypes.data)
         return xy, rc
 
-    def score_at(self, signals, method, x, y, z=0.0):
+    def start(self, signals, method=0, seed_mode=0):
+        """Start search position (centroid or strongest sensor) and the unusable-event flag."""
+        s = _f32(signals)
+        xy = np.zeros(2)
+        rc = _load().oracle_start(C.byref(self.c), s.ctypes.data, int(method), int(seed_mode), xy.ctypes.data)
+        return xy, rc
+
+    def score_at(self, signals, method, x, y, z=0.0, seed_mode=0):
         """(A, score) of one event's signals at a position; invalid node -> (nan, inf)."""
         s = _f32(signals)
         A, sc = C.c_double(), C.c_double()
-        _load().oracle_score_at(C.byref(self.c), s.ctypes.data, int(method), float(x), float(y),
+        _load().oracle_score_at(C.byref(self.c), s.ctypes.data, int(method), int(seed_mode), float(x), float(y),
                                 float(z), C.byref(A), C.byref(sc))
         return A.value, sc.value
 
 
-def score_at_many(model: Model, signals, method: int, pos):
+def score_at_many(model: Model, signals, method: int, pos, seed_mode: int = 0):
     """(A [E], score [E]) of each event's signals at its own position pos [E][3]."""
     s = _f32(signals).reshape(-1, model.n_sensors)
     p = np.ascontiguousarray(np.asarray(pos, dtype=np.float64)).reshape(-1, 3)
     assert p.shape[0] == s.shape[0]
     A, sc = np.zeros(s.shape[0]), np.zeros(s.shape[0])
-    rc = _load().oracle_score_at_many(C.byref(model.c), s.ctypes.data, s.shape[0], int(method),
+    rc = _load().oracle_score_at_many(C.byref(model.c), s.ctypes.data, s.shape[0], int(method), int(seed_mode),
                                       p.ctypes.data, A.ctypes.data, sc.ctypes.data)
     if rc != 0:
         raise ValueError("oracle_score_at_many: invalid argument")
     return A, sc
 
 
-def grid_params(dim, nodes_per_axis, step0_xy, step0_z, factor, n_iter, z_seed=float("nan")):
+def grid_params(dim, nodes_per_axis, step0_xy, step0_z, factor, n_iter, z_seed=float("nan"), seed_mode=0):
     return _Grid(int(dim), int(nodes_per_axis), float(step0_xy), float(step0_z), float(factor),
-                 int(n_iter), 0, float(z_seed))
+                 int(n_iter), int(seed_mode), float(z_seed))
 
 
 def grid_from_config(cfg):
     return grid_params(cfg.dim, cfg.nodes_per_axis, cfg.step0_xy, cfg.step0_z, cfg.factor,
-                       cfg.n_iter, cfg.z_seed)
+                       cfg.n_iter, cfg.z_seed, getattr(cfg, "seed_mode", 0))
 
 
 def n_threads(requested: int = 0) -> int:

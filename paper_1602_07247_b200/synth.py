@@ -138,6 +138,7 @@ class Config:
     passive: Optional[np.ndarray] = None     # [N] bool/uint8, non-zero = passive
     signal_min: float = float("nan")         # NaN = off
     dist_max: float = float("nan")           # NaN = off
+    seed_mode: int = 0                       # 0 centroid, 1 strongest sensor
 
     @property
     def n_sensors(self) -> int:

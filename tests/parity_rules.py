@@ -27,7 +27,7 @@ def compare(cfg, signals: np.ndarray, gpu_xyzA: np.ndarray, gpu_score: np.ndarra
     out = {"n_events": E, "fail_mismatch": int((ok_ref != ok_gpu).sum())}
     v = ok_ref & ok_gpu
     # (i) + (iv): oracle evaluated at the GPU's returned position
-    A_at, s_at = oracle.score_at_many(model, signals, cfg.method, gx[:, :3])
+    A_at, s_at = oracle.score_at_many(model, signals, cfg.method, gx[:, :3], getattr(cfg, "seed_mode", 0))
     gs = gpu_score.astype(np.float64)
     both_inf = np.isinf(gs) & np.isinf(s_at)
     tol = 1e-5 * np.abs(s_at) + score_floor

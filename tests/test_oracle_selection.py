@@ -123,3 +123,58 @@ def test_events_with_nothing_left_fail():
     cfg.passive = np.ones(cfg.n_sensors, np.uint8)
     r = oracle.reconstruct(oracle.Model.from_config(cfg), sig, oracle.grid_from_config(cfg), cfg.method)
     assert np.isnan(r["xyzA"]).all() and np.isposinf(r["score"]).all()
+
+
+# ---------------------------------------------------------------------------
+# start position = the strongest sensor (R20)
+# ---------------------------------------------------------------------------
+from test_oracle_pins import np_grid_argmin   # noqa: E402  (numpy/scipy evaluation of one grid iteration)
+
+
+def test_strongest_sensor_start_position():
+    cfg, sig = _events(2, 16)
+    model = oracle.Model.from_config(cfg)
+    for e in range(sig.shape[0]):
+        xy, rc = model.start(sig[e], cfg.method, seed_mode=1)
+        i = int(np.argmax(sig[e]))                       # numpy's argmax: first maximum
+        assert rc == 0 and tuple(xy) == (float(cfg.sensor_xy[i, 0]), float(cfg.sensor_xy[i, 1]))
+        assert np.array_equal(model.start(sig[e], cfg.method, seed_mode=0)[0], model.centroid(sig[e], cfg.method)[0])
+    tie = np.zeros(cfg.n_sensors, np.float32)
+    tie[[4, 11]] = 7.0                                   # equal maxima: the first sensor wins
+    assert tuple(model.start(tie, 0, 1)[0]) == tuple(cfg.sensor_xy[4].astype(float))
+    cfg.passive = np.zeros(cfg.n_sensors, np.uint8)
+    cfg.passive[4] = 1                                   # a passive sensor cannot be the start
+    assert tuple(oracle.Model.from_config(cfg).start(tie, 0, 1)[0]) == tuple(cfg.sensor_xy[11].astype(float))
+    assert model.start(np.zeros(cfg.n_sensors, np.float32), 0, 1)[1] == 1        # sum S = 0: unusable
+    bad = sig[0].copy()
+    bad[3] = np.nan
+    assert model.start(bad, 0, 1)[1] == 1
+
+
+@pytest.mark.parametrize("idx", [1, 3])
+def test_first_iteration_from_the_strongest_sensor_equals_numpy_argmin(idx):
+    cfg, sig = _events(idx, 6)
+    cfg.seed_mode, cfg.n_iter = 1, 1
+    res = oracle.reconstruct(oracle.Model.from_config(cfg), sig, oracle.grid_from_config(cfg), cfg.method, trace=True)
+    for e in range(sig.shape[0]):
+        S = np.maximum(sig[e], 0.0) if cfg.method == 0 else sig[e]
+        i = int(np.argmax(S))
+        centre = (float(cfg.sensor_xy[i, 0]), float(cfg.sensor_xy[i, 1]), 0.0)
+        k, sc = np_grid_argmin(cfg, sig[e], centre, cfg.step0_xy, cfg.step0_z)
+        assert res["idx"][e, 0] == k
+        assert res["best"][e, 0] == pytest.approx(sc[k], rel=1e-9)
+
+
+def test_distance_selection_follows_the_chosen_start():
+    """With seed_mode = 1 the 'initial search position' of PAPER.md:318 is the strongest sensor's axis."""
+    cfg, sig = _events(2, 10)
+    cfg.seed_mode, cfg.dist_max = 1, 31.0
+    model = oracle.Model.from_config(cfg)
+    res = oracle.reconstruct(model, sig, oracle.grid_from_config(cfg), cfg.method)
+    for e in range(sig.shape[0]):
+        i = int(np.argmax(sig[e]))
+        d = np.hypot(cfg.sensor_xy[:, 0] - cfg.sensor_xy[i, 0], cfg.sensor_xy[:, 1] - cfg.sensor_xy[i, 1])
+        keep = np.flatnonzero(d <= 31.0)
+        sub = _subset_config(cfg, keep)
+        A_ref, s_ref = lib_score(sub, sig[e, keep], *res["xyzA"][e, :2])
+        assert res["score"][e] == pytest.approx(s_ref, rel=1e-8) and res["xyzA"][e, 3] == pytest.approx(A_ref, rel=1e-9)

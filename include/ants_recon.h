@@ -82,7 +82,8 @@ typedef struct {
     float step0_z;          /* first-iteration node spacing in z, mm (dim == 3), > 0 */
     float factor;           /* contraction factor in (0,1): h_k = h_0 * factor^k (R1) */
     int32_t n_iter;         /* K >= 1 iterations */
-    int32_t seed_mode;      /* 0 = centroid start (the only mode on the hot path, R12) */
+    int32_t seed_mode;      /* start position: 0 = centroid, 1 = axis of the
+                               sensor with the strongest signal, first one on ties (R20) */
     float z_seed;           /* start z (dim 3) or fixed z (dim 2 with lrf_dim 2); NaN = (z_lo+z_hi)/2 (R10) */
 } ants_grid_params_t;
 
@@ -115,7 +116,7 @@ int ants_lrf_set_selection(ants_lrf_t *lrf, const uint8_t *passive, float signal
  * range, if sum L <= 0 or (Poisson) some L_i <= 0 with S_i > 0.  Poisson ML
  * clips negative signals to 0 first (R18).
  * Per-event failure does not fail the call: an event with a non-finite signal,
- * sum S <= 0 or sum S/g <= 0 gets x = y = z = A = NaN and score = +inf.
+ * sum S <= 0 or (centroid start) sum S/g <= 0 gets x = y = z = A = NaN and score = +inf.
  * Errors: ANTS_ERR_INVALID (NULL pointers with n_events > 0, bad grid values,
  * dim 3 with an axial LRF, method not 0/1), ANTS_ERR_UNSUPPORTED (G^dim above
  * the compiled limit: 256 nodes in 2-D, 512 in 3-D), ANTS_ERR_CUDA.

@@ -378,7 +378,7 @@ static int validate_grid(const ants_lrf *h, const ants_grid_params_t *g, int32_t
     if (g->nodes_per_axis < 2 || g->n_iter < 1 || g->n_iter > 4096) return ANTS_ERR_INVALID;
     if (!(g->factor > 0.f && g->factor < 1.f)) return ANTS_ERR_INVALID;
     if (!(g->step0_xy > 0.f) || !std::isfinite(g->step0_xy)) return ANTS_ERR_INVALID;
-    if (g->seed_mode != 0) return ANTS_ERR_INVALID;
+    if (g->seed_mode != 0 && g->seed_mode != 1) return ANTS_ERR_INVALID;
     const bool lrf3 = h->dev.n_z > 0;
     if (g->dim == 3) {
         if (!lrf3) return ANTS_ERR_INVALID;
@@ -550,6 +550,7 @@ static int launch(const ants_lrf *h, const float *signals, int64_t n_events, con
     p.factor = g->factor;
     p.z_seed = g->z_seed;
     p.dim = g->dim;
+    p.seed_mode = g->seed_mode;
     p.warps_per_cta = pl.warps;
     p.tile_events = pl.warps;
 

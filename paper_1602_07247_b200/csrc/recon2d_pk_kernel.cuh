@@ -86,7 +86,7 @@ __global__ void __launch_bounds__(256, (NPT <= 3 ? 3 : 2)) recon2d_pk_kernel(con
         sxw = warp_sum(sxw);
         syw = warp_sum(syw);
         __syncwarp();
-        if (!finite || !(sumS > 0.f) || !(sw > 0.f)) {
+        if (!finite || !(sumS > 0.f) || (p.seed_mode == 0 && !(sw > 0.f))) {
             if (lane == 0) {
                 const float qnan = __int_as_float(0x7fc00000);
                 reinterpret_cast<float4 *>(p.out_xyzA)[e] = make_float4(qnan, qnan, qnan, qnan);
@@ -97,6 +97,7 @@ __global__ void __launch_bounds__(256, (NPT <= 3 ? 3 : 2)) recon2d_pk_kernel(con
             continue;
         }
         float cx = sxw / sw, cy = syw / sw;
+        if (p.seed_mode == 1) strongest_sensor(w.SC, sens_s, N, lane, cx, cy);    // R20
 
         if (m.select) {
             // R19: the sensors of the statistical part, fixed for the event: signal threshold and

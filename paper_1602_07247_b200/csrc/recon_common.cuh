@@ -46,6 +46,7 @@ struct Params {
     int k_series;           // 3-D Poisson: first iteration whose log1p is the series (before: lg2(1 + q))
     int positive;           // every LRF strictly positive on its domain (validity tests can be skipped)
     float h0_xy, h0_z, factor, z_seed;
+    int seed_mode;          // 0 centroid, 1 strongest sensor (R20)
     int warps_per_cta;
     int tile_events;        // events staged per CTA tile (= warps_per_cta)
 };
@@ -128,6 +129,23 @@ __device__ __forceinline__ void warp_argmin(float &s, int &idx) {
         s = take ? os : s;
         idx = take ? oi : idx;
     }
+}
+
+// start position = axis of the sensor with the strongest signal (R20): largest prepared signal among
+// the sensors not flagged passive (NaN in SC[i].y), lowest index on ties.  Each lane scans the sensors
+// it loaded itself (i = lane + 32 c), so no synchronisation is needed before the call.
+__device__ __forceinline__ void strongest_sensor(const float2 *SC, const float4 *sens_s, int N, int lane,
+                                                 float &cx, float &cy) {
+    float key = kInf;            // -S of the lane's best
+    int bi = 0x7fffffff;
+    for (int i = lane; i < N; i += 32) {
+        const float2 sc = SC[i];
+        if (sc.y == sc.y && -sc.x < key) { key = -sc.x; bi = i; }
+    }
+    warp_argmin(key, bi);
+    bi = min(bi, N - 1);
+    cx = sens_s[bi].x;
+    cy = sens_s[bi].y;
 }
 
 // same result as warp_argmin through two integer reductions (REDUX): scores mapped to order-preserving

@@ -152,7 +152,7 @@ class Reconstructor:
         self.cfg = cfg
         self.dims = LrfDims(cfg.n_sensors, cfg.n_lrf, cfg.lrf_dim, cfg.n_int_r, cfg.n_int_z)
         self.grid = GridParams(cfg.dim, cfg.nodes_per_axis, cfg.step0_xy, cfg.step0_z, cfg.factor,
-                               cfg.n_iter, 0, cfg.z_seed)
+                               cfg.n_iter, int(getattr(cfg, "seed_mode", 0)), cfg.z_seed)
         self.method = int(cfg.method)
         self.handle = ants_lrf_create(cfg.sensor_xy, cfg.gains, cfg.knots, cfg.coeffs, self.dims)
         passive = getattr(cfg, "passive", None)

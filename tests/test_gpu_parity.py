@@ -237,7 +237,8 @@ def test_status_codes():
         assert status(step0_xy=0.0) == -1
         assert status(dim=3) == -1                      # 3-D search over an axial LRF
         assert status(nodes_per_axis=17) == -2          # 289 nodes > compiled limit
-        assert status(seed_mode=1) == -1
+        assert status(seed_mode=1) == 0                 # strongest-sensor start (R20)
+        assert status(seed_mode=2) == -1
     finally:
         r.close()
     with pytest.raises(recon.AntsError):
@@ -352,3 +353,20 @@ def test_selection_can_be_switched_off_again():
         assert not torch.equal(base[0], sel[0])
     finally:
         r.close()
+
+
+@pytest.mark.parametrize("idx,kw", [(2, {}), (3, {}), (4, {}), (5, dict(dist_max=60.0)), (2, dict(passive=[9], signal_min=5.0))])
+def test_parity_with_strongest_sensor_start(idx, kw):
+    """seed_mode = 1 (R20): the grid starts on the axis of the strongest sensor."""
+    cfg = _with_selection(idx, **kw)
+    cfg.seed_mode = 1
+    n = {2: 6001, 3: 1501, 4: 2501, 5: 801}[idx]
+    ev = synth.generate_events(synth.make_config(idx), n, device="cuda")
+    xyzA, score, path = _run(cfg, ev["signals"])
+    res = parity_rules.compare(cfg, ev["signals"].cpu().numpy(), xyzA, score, path)
+    parity_rules.assert_parity(res, f"cfg{idx} strongest-sensor start {kw}")
+    # the two start options agree on most events (both reach the same minimum) but not bit for bit
+    cfg0 = _with_selection(idx, **kw)
+    a = _run(cfg0, ev["signals"], trace=False)[0]
+    close = np.hypot(a[:, 0] - xyzA[:, 0], a[:, 1] - xyzA[:, 1]) < 1.0
+    assert close.mean() > 0.8

@@ -30,6 +30,8 @@ struct ants_lrf {
     double max_dlog_z = 0.0; // axial+z: max |d ln s / dz|, 1/mm
     double knot_r = 0.0, knot_z = 0.0;   // knot spacing, mm
     void *d_sens = nullptr, *d_poly = nullptr, *d_polyd = nullptr, *d_passive = nullptr;
+    unsigned long long *d_ctr = nullptr;   // ring of per-launch event counters {next, done}
+    std::atomic<unsigned> next_slot{0};
     // scratch of ants_reconstruct_host (lazily allocated, reused, guarded)
     std::mutex host_mu;
     int64_t scratch_events = 0;
@@ -40,6 +42,8 @@ struct ants_lrf {
 };
 
 static std::atomic<int64_t> g_launches{0};
+// launches that may be in flight at once on one model (each owns a counter pair until its last warp retires)
+static const unsigned kCtrSlots = 4096;
 
 // ---------------------------------------------------------------------------
 // step a0: B-spline coefficients -> per-interval cubics
@@ -239,10 +243,12 @@ extern "C" int ants_lrf_create(const float *sensor_xy, const float *gains, const
     h->knot_r = 1.0 / sc_r;
     h->knot_z = dim == 2 ? ((double)z_hi - (double)z_lo) / n_z : 0.0;
 
+    cudaError_t e0 = cudaMalloc(&h->d_ctr, kCtrSlots * 2 * sizeof(unsigned long long));
+    if (e0 == cudaSuccess) e0 = cudaMemset(h->d_ctr, 0, kCtrSlots * 2 * sizeof(unsigned long long));
     cudaError_t e1 = cudaMalloc(&h->d_sens, sens.size() * sizeof(float4));
     cudaError_t e2 = cudaMalloc(&h->d_poly, rows32.size() * sizeof(float4));
     cudaError_t e3 = cudaMalloc(&h->d_polyd, rows64.size() * sizeof(double));
-    if (e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess) {
+    if (e0 != cudaSuccess || e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess) {
         cudaGetLastError();
         ants_destroy(h);
         return (e1 == cudaErrorMemoryAllocation || e2 == cudaErrorMemoryAllocation ||
@@ -308,6 +314,7 @@ extern "C" void ants_destroy(ants_lrf_t *h) {
     cudaFree(h->d_poly);
     cudaFree(h->d_polyd);
     cudaFree(h->d_passive);
+    cudaFree(h->d_ctr);
     for (int s = 0; s < 3; ++s) {
         cudaFree(h->d_sig[s]);
         cudaFree(h->d_xyzA[s]);
@@ -571,6 +578,8 @@ static int launch(const ants_lrf *h, const float *signals, int64_t n_events, con
     long long want = (n_events + pl.warps - 1) / pl.warps;
     long long cap = (long long)h->sm_count * occ;
     int grid = (int)std::min(want, cap);
+    p.ctr = h->d_ctr + 2 * (const_cast<ants_lrf *>(h)->next_slot.fetch_add(1) % kCtrSlots);
+    p.total_warps = grid * pl.warps;
     void *args[] = {&p};
     if (cudaLaunchKernel(pl.kernel, dim3(grid), dim3(pl.warps * 32), args, pl.smem, stream) != cudaSuccess) {
         cudaGetLastError();

@@ -170,8 +170,9 @@ __global__ void __launch_bounds__(256) recon2d_kernel(const Params p) {
     }
     const float half_diag_units = 1.41421356f * half;   // farthest node from the centre, in steps
 
-    const long long stride = (long long)gridDim.x * p.warps_per_cta;
-    for (long long e = (long long)blockIdx.x * p.warps_per_cta + warp; e < p.n_events; e += stride) {
+    long long e_next = grab_event(p.ctr, lane);
+    for (long long e = e_next; e < p.n_events; e = e_next) {
+        e_next = grab_event(p.ctr, lane);
         // ---- a1: load signals (coalesced), prepare, centroid ----
         const float *sig = p.signals + e * N;
         float sumS = 0.f, sw = 0.f, sxw = 0.f, syw = 0.f;
@@ -486,6 +487,7 @@ __global__ void __launch_bounds__(256) recon2d_kernel(const Params p) {
             p.out_score[e] = score_fin;
         }
     }
+    retire_warp(p.ctr, p.total_warps, lane);
 }
 
 }  // namespace ants

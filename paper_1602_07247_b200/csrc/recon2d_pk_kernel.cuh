@@ -39,7 +39,6 @@ __global__ void __launch_bounds__(256, (NPT <= 3 ? 3 : 2)) recon2d_pk_kernel(con
     const float half_diag_units = 1.41421356f * half;
     const f32x2 sc2 = pk1(m.sc), of2 = pk1(m.of), magic2 = pk1(kMagic), nmagic2 = pk1(-kMagic);
 
-    const long long stride = (long long)gridDim.x * p.warps_per_cta;
     // the next event's signals are fetched into registers (4 per lane: N <= 128) while this one runs
     float pf[4];
     auto prefetch = [&](long long ev) {
@@ -49,8 +48,10 @@ __global__ void __launch_bounds__(256, (NPT <= 3 ? 3 : 2)) recon2d_pk_kernel(con
             pf[c] = (ev < p.n_events && i < N) ? __ldg(p.signals + ev * N + i) : 0.f;
         }
     };
-    prefetch((long long)blockIdx.x * p.warps_per_cta + warp);
-    for (long long e = (long long)blockIdx.x * p.warps_per_cta + warp; e < p.n_events; e += stride) {
+    long long e_next = grab_event(p.ctr, lane);
+    prefetch(e_next);
+    for (long long e = e_next; e < p.n_events; e = e_next) {
+        e_next = grab_event(p.ctr, lane);
         // ---- a1: load signals (coalesced), prepare, centroid ----
         const float *sig = p.signals + e * N;
         float sumS = 0.f, sw = 0.f, sxw = 0.f, syw = 0.f;
@@ -75,7 +76,7 @@ __global__ void __launch_bounds__(256, (NPT <= 3 ? 3 : 2)) recon2d_pk_kernel(con
         float cur[4];
 #pragma unroll
         for (int c = 0; c < 4; ++c) cur[c] = pf[c];
-        prefetch(e + stride);
+        prefetch(e_next);
 #pragma unroll
         for (int c = 0; c < 4; ++c)
             if (lane + 32 * c < N) take(lane + 32 * c, cur[c]);
@@ -191,6 +192,7 @@ __global__ void __launch_bounds__(256, (NPT <= 3 ? 3 : 2)) recon2d_pk_kernel(con
             p.out_score[e] = score_fin;
         }
     }
+    retire_warp(p.ctr, p.total_warps, lane);
 }
 
 }  // namespace ants

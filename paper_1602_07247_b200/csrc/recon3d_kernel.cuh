@@ -39,8 +39,9 @@ __global__ void __launch_bounds__(256) recon3d_kernel(const Params p) {
     const float half_diag_units = 1.41421356f * half;
     const float z_start = (p.z_seed == p.z_seed) ? p.z_seed : 0.5f * (m.z_lo + m.z_hi);   // R10
 
-    const long long stride = (long long)gridDim.x * p.warps_per_cta;
-    for (long long e = (long long)blockIdx.x * p.warps_per_cta + warp; e < p.n_events; e += stride) {
+    long long e_next = grab_event(p.ctr, lane);
+    for (long long e = e_next; e < p.n_events; e = e_next) {
+        e_next = grab_event(p.ctr, lane);
         // ---- a1: load signals, prepare, centroid ----
         const float *sig = p.signals + e * N;
         float sumS = 0.f, sw = 0.f, sxw = 0.f, syw = 0.f;
@@ -183,6 +184,7 @@ __global__ void __launch_bounds__(256) recon3d_kernel(const Params p) {
             p.out_score[e] = score_fin;
         }
     }
+    retire_warp(p.ctr, p.total_warps, lane);
 }
 
 }  // namespace ants

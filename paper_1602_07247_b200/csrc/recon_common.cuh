@@ -47,6 +47,10 @@ struct Params {
     int positive;           // every LRF strictly positive on its domain (validity tests can be skipped)
     float h0_xy, h0_z, factor, z_seed;
     int seed_mode;          // 0 centroid, 1 strongest sensor (R20)
+    // dynamic event distribution: ctr[0] = next event to hand out, ctr[1] = warps that have finished;
+    // the last warp out zeroes both, so the pair is ready for the launch that reuses the slot
+    unsigned long long *ctr;
+    int total_warps;        // gridDim.x * warps_per_cta
     int warps_per_cta;
     int tile_events;        // events staged per CTA tile (= warps_per_cta)
 };
@@ -128,6 +132,24 @@ __device__ __forceinline__ void warp_argmin(float &s, int &idx) {
         bool take = (os < s) || (os == s && oi < idx);
         s = take ? os : s;
         idx = take ? oi : idx;
+    }
+}
+
+// next event for this warp (lane 0 draws from the launch's counter, all lanes get it)
+__device__ __forceinline__ long long grab_event(unsigned long long *ctr, int lane) {
+    unsigned long long v = 0ULL;
+    if (lane == 0) v = atomicAdd(ctr, 1ULL);
+    return (long long)__shfl_sync(kFull, v, 0);
+}
+// a warp is done: count it; the last one re-arms the counters
+__device__ __forceinline__ void retire_warp(unsigned long long *ctr, int total_warps, int lane) {
+    if (lane == 0) {
+        const unsigned long long d = atomicAdd(ctr + 1, 1ULL);
+        if (d == (unsigned long long)(total_warps - 1)) {
+            ctr[0] = 0ULL;
+            ctr[1] = 0ULL;
+            __threadfence();
+        }
     }
 }
 

@@ -327,8 +327,8 @@ def run_ours(args):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per event from the `ncu --set full` captures of the bench
 # command (profiles/r01_ncu_final.md); `traffic` = this x the events of one launch.  Config 1 was not captured.
-TRAFFIC_PER_EVENT = {"cfg2_pmt2d_hex19": 84.07, "cfg3_sipm_chi2_sq64": 257.5, "cfg4_axialz3d_hex37": 148.7,
-                     "cfg5_flood_hex127": 540.9}
+TRAFFIC_PER_EVENT = {"cfg2_pmt2d_hex19": 87.83, "cfg3_sipm_chi2_sq64": 257.5, "cfg4_axialz3d_hex37": 148.7,
+                     "cfg5_flood_hex127": 547.2}
 
 
 def main(argv=None):

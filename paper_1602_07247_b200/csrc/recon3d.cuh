@@ -17,8 +17,8 @@
 //   differential (fine grids)    dL = [T_l(r) - T_l(r0)] + dT_l(r0): Taylor form of
 //                T_l about the centre radius plus the cubic jump at an adjacent r-knot,
 //                plus the exactly contracted z-difference at the centre radius.
-//                Poisson uses S log1p(dL/L0): degree-6 series where |dL/L0| <= 0.1, lg2(1 + dL/L0)
-//                elsewhere, chosen per pair behind one warp vote per sensor.
+//                Poisson uses S log1p(dL/L0): degree-6 series when |dL/L0| <= 0.1 on all of a sensor's
+//                nodes, lg2(1 + dL/L0) for that sensor otherwise (one warp vote per sensor).
 // The reported score and energy are one FP64 evaluation at the final node.
 #pragma once
 #include "../../include/ants_recon.h"

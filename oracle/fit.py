@@ -1,0 +1,72 @@
+"""CPU ORACLE of the axial LRF calculation (TEST INFRASTRUCTURE, NOT THE PRODUCT).
+
+PAPER.md:380 (section 6): "The LRF module calculates these functions from datasets containing
+photosensor signals and the corresponding event positions"; the LRFs are B-splines of the
+distance to the sensor axis ("Axial"), one per sensor or one per group with a relative gain
+per sensor (section 6.2); the positions are the reconstructed or the true ones
+(PAPER.md:414).  The paper prints no fit criterion; the readings are DESIGN.md R21-R23:
+
+  R21  unweighted least squares: for table m the coefficients c minimise
+           sum over events e and sensors i of the table of ( y_ie - s_c(r_ie) )^2,
+       y_ie = S_ie / (A_e g_i)   ("a point light source emitting ... a constant number of photons",
+       PAPER.md:380: the signal is normalised by the event's energy scale A_e; g_i = 1 for per-sensor tables),
+       r_ie = |p_e - P_i|, s_c the uniform cubic B-spline of oracle/ants_oracle.c (R7);
+  R22  an event takes part if x, y, A are finite and A > 0 (failed events carry NaN); a pair takes part
+       if r_lo <= r <= r_hi (no extrapolation data);
+  R23  signals enter as they are (no clipping), in double.
+
+Plain numpy in float64, written in the order of the definition: design rows, normal equations
+M = sum B^T B, b = sum B^T y, then the library solve numpy.linalg.solve.  Shares no code with the CUDA
+path.  Pins: tests/test_oracle_fit.py.
+"""
+from __future__ import annotations
+
+import numpy as np
+
+
+def basis4(u):
+    """The four uniform cubic B-spline basis values at local coordinate u in [0, 1] (R7)."""
+    return np.stack([(1.0 - u) ** 3 / 6.0,
+                     (3.0 * u ** 3 - 6.0 * u ** 2 + 4.0) / 6.0,
+                     (-3.0 * u ** 3 + 3.0 * u ** 2 + 3.0 * u + 1.0) / 6.0,
+                     u ** 3 / 6.0], axis=-1)
+
+
+def normal_equations(sensor_xy, gains, knots, n_lrf, n_int, signals, xyzA):
+    """-> M [n_lrf][n+3][n+3], b [n_lrf][n+3], n_used [n_lrf] (pairs that entered each table)."""
+    xy = np.asarray(sensor_xy, np.float32).astype(np.float64).reshape(-1, 2)
+    N = xy.shape[0]
+    g = np.ones(N) if gains is None else np.asarray(gains, np.float32).astype(np.float64)
+    lo, hi = (float(np.float32(k)) for k in knots[:2])
+    h = (hi - lo) / n_int
+    S = np.asarray(signals, np.float32).astype(np.float64).reshape(-1, N)
+    P = np.asarray(xyzA, np.float32).astype(np.float64).reshape(-1, 4)
+    ok = np.isfinite(P[:, 0]) & np.isfinite(P[:, 1]) & np.isfinite(P[:, 3]) & (P[:, 3] > 0.0)     # R22
+    nc = n_int + 3
+    M = np.zeros((n_lrf, nc, nc))
+    b = np.zeros((n_lrf, nc))
+    n_used = np.zeros(n_lrf)
+    for i in range(N):
+        m = 0 if n_lrf == 1 else i
+        gi = g[i] if n_lrf == 1 else 1.0
+        with np.errstate(invalid="ignore"):
+            r = np.hypot(P[:, 0] - xy[i, 0], P[:, 1] - xy[i, 1])
+            use = ok & (r >= lo) & (r <= hi)                                                     # R22
+        r_u, y = r[use], S[use, i] / (P[use, 3] * gi)                                             # R21, R23
+        t = (r_u - lo) / h
+        k = np.minimum(np.floor(t).astype(np.int64), n_int - 1)
+        B4 = basis4(t - k)                                   # [n][4]: coefficients k .. k+3
+        for a in range(4):
+            np.add.at(b[m], k + a, B4[:, a] * y)
+            for c in range(4):
+                np.add.at(M[m], (k + a, k + c), B4[:, a] * B4[:, c])
+        n_used[m] += use.sum()
+    return M, b, n_used
+
+
+def fit_axial(sensor_xy, gains, knots, n_lrf, n_int, signals, xyzA):
+    """Least-squares B-spline coefficients [n_lrf][n_int + 3] (float64) and the pairs used per table.
+    Raises numpy.linalg.LinAlgError when a table is underdetermined (an interval without data)."""
+    M, b, n_used = normal_equations(sensor_xy, gains, knots, n_lrf, n_int, signals, xyzA)
+    c = np.stack([np.linalg.solve(M[m], b[m]) for m in range(n_lrf)])
+    return c, n_used

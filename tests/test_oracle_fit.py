@@ -1,0 +1,94 @@
+"""Pins of the LRF-calculation oracle (oracle/fit.py; R21-R23), CPU-only.  Expected values
+come from scipy's BSpline (design matrix, evaluation) and numpy.linalg.lstsq on the raw least-squares
+problem -- never from the oracle's own basis or normal equations."""
+import numpy as np
+import pytest
+from scipy.interpolate import BSpline
+
+from oracle import fit
+from paper_1602_07247_b200 import synth
+
+
+def _problem(idx, n_events, seed=1, noise=0.0, individual=None):
+    cfg = synth.make_config(idx)
+    rng = np.random.default_rng(seed)
+    ext = float(np.abs(cfg.sensor_xy).max()) + 0.75 * float(cfg.knots[1])   # every sensor sees its whole r-range
+    pos = np.zeros((n_events, 4), np.float32)
+    pos[:, 0:2] = rng.uniform(-ext, ext, (n_events, 2))
+    pos[:, 3] = rng.uniform(50.0, 500.0, n_events)                      # energy scale A_e
+    lo, hi = float(cfg.knots[0]), float(cfg.knots[1])
+    r = np.hypot(pos[:, None, 0].astype(float) - cfg.sensor_xy[None, :, 0],
+                 pos[:, None, 1].astype(float) - cfg.sensor_xy[None, :, 1])
+    sig = np.empty((n_events, cfg.n_sensors))
+    for i in range(cfg.n_sensors):
+        m = 0 if cfg.n_lrf == 1 else i
+        g = float(cfg.gains[i]) if cfg.n_lrf == 1 else 1.0
+        sig[:, i] = pos[:, 3] * g * synth.eval_axial(cfg.coeffs[m, 0], lo, hi, r[:, i])     # scipy evaluation
+    sig += noise * rng.standard_normal(sig.shape)
+    return cfg, sig.astype(np.float32), pos
+
+
+def _lstsq_reference(cfg, sig, pos, table):
+    """The raw least-squares problem of R21 for one table through scipy's design matrix + numpy lstsq."""
+    lo, hi, n = float(cfg.knots[0]), float(cfg.knots[1]), cfg.n_int_r
+    t = synth.uniform_knot_vector(lo, hi, n)
+    rows, ys = [], []
+    sensors = range(cfg.n_sensors) if cfg.n_lrf == 1 else [table]
+    ok = np.isfinite(pos[:, 0]) & np.isfinite(pos[:, 3]) & (pos[:, 3] > 0)
+    for i in sensors:
+        g = float(cfg.gains[i]) if cfg.n_lrf == 1 else 1.0
+        r = np.hypot(pos[:, 0].astype(float) - float(cfg.sensor_xy[i, 0]), pos[:, 1].astype(float) - float(cfg.sensor_xy[i, 1]))
+        use = ok & (r >= lo) & (r <= hi)
+        rows.append(BSpline.design_matrix(r[use], t, 3).toarray())
+        ys.append(sig[use, i].astype(float) / (pos[use, 3].astype(float) * g))
+    c, *_ = np.linalg.lstsq(np.vstack(rows), np.concatenate(ys), rcond=None)
+    return c
+
+
+def test_noise_free_data_give_back_the_coefficients():
+    for idx in (2, 3):
+        cfg, sig, pos = _problem(idx, 4000)
+        c, n_used = fit.fit_axial(cfg.sensor_xy, cfg.gains, cfg.knots, cfg.n_lrf, cfg.n_int_r, sig, pos)
+        want = cfg.coeffs[:, 0, :].astype(float)
+        # float32 storage of the signals limits the agreement (6e-8 relative per sample)
+        assert np.abs(c - want).max() <= 2e-5 * np.abs(want).max()
+        assert (n_used > 0).all()
+
+
+@pytest.mark.parametrize("idx", [2, 3, 5])
+def test_equals_numpy_lstsq_on_scipy_design_matrix(idx):
+    cfg, sig, pos = _problem(idx, 1500 if idx != 5 else 600, noise=0.5)
+    c, _ = fit.fit_axial(cfg.sensor_xy, cfg.gains, cfg.knots, cfg.n_lrf, cfg.n_int_r, sig, pos)
+    for table in ([0] if cfg.n_lrf == 1 else [0, 17, cfg.n_sensors - 1]):
+        ref = _lstsq_reference(cfg, sig, pos, table)
+        assert np.abs(c[table] - ref).max() <= 1e-8 * max(1.0, np.abs(ref).max())
+
+
+def test_relative_gains_are_divided_out_of_a_shared_profile():
+    cfg, sig, pos = _problem(2, 3000, noise=0.2)
+    c1, _ = fit.fit_axial(cfg.sensor_xy, cfg.gains, cfg.knots, 1, cfg.n_int_r, sig, pos)
+    g2 = (cfg.gains * 2.0).astype(np.float32)                # power of two: exact
+    c2, _ = fit.fit_axial(cfg.sensor_xy, g2, cfg.knots, 1, cfg.n_int_r, sig * 2.0, pos)
+    assert np.allclose(c1, c2, rtol=1e-12, atol=0)
+    c3, _ = fit.fit_axial(cfg.sensor_xy, None, cfg.knots, 1, cfg.n_int_r, sig / cfg.gains[None, :], pos)
+    assert np.abs(c3 - c1).max() <= 1e-6 * np.abs(c1).max()   # float32 rounding of the rescaled signals
+
+
+def test_failed_events_and_out_of_range_pairs_are_left_out():
+    cfg, sig, pos = _problem(2, 2500, noise=0.3)
+    pos2, sig2 = pos.copy(), sig.copy()
+    pos2[::7] = np.nan                                        # failed events (NaN rows)
+    pos2[3::11, 3] = -1.0                                     # non-positive energy
+    keep = np.isfinite(pos2[:, 0]) & (pos2[:, 3] > 0)
+    a, na = fit.fit_axial(cfg.sensor_xy, cfg.gains, cfg.knots, 1, cfg.n_int_r, sig2, pos2)
+    b, nb = fit.fit_axial(cfg.sensor_xy, cfg.gains, cfg.knots, 1, cfg.n_int_r, sig2[keep], pos2[keep])
+    assert np.array_equal(a, b) and np.array_equal(na, nb)
+    r = np.hypot(pos[:, None, 0] - cfg.sensor_xy[None, :, 0], pos[:, None, 1] - cfg.sensor_xy[None, :, 1])
+    assert na[0] == float((keep[:, None] & (r.astype(float) <= 90.0)).sum())          # pairs with r <= r_hi only
+
+
+def test_underdetermined_table_raises():
+    cfg, sig, pos = _problem(2, 50)
+    pos[:, 0:2] = 0.0                                         # all events at one point: most intervals empty
+    with pytest.raises(np.linalg.LinAlgError):
+        fit.fit_axial(cfg.sensor_xy, cfg.gains, cfg.knots, 1, cfg.n_int_r, sig, pos)

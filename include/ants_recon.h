@@ -37,7 +37,8 @@ enum ants_status {
     ANTS_ERR_INVALID = -1,     /* NULL pointer, N < 1, bad knots/dims, G < 2, factor not in (0,1), K < 1, ... */
     ANTS_ERR_UNSUPPORTED = -2, /* valid request outside the compiled limits (see ants_reconstruct) */
     ANTS_ERR_CUDA = -3,        /* a CUDA runtime call failed (no device, launch error, ...) */
-    ANTS_ERR_NOMEM = -4        /* host or device allocation failed */
+    ANTS_ERR_NOMEM = -4,       /* host or device allocation failed */
+    ANTS_ERR_SINGULAR = -5     /* ants_lrf_fit_axial: a table is underdetermined (an interval without data) */
 };
 
 enum ants_method {
@@ -148,6 +149,29 @@ int ants_reconstruct_trace(const ants_lrf_t *lrf, const float *signals, int64_t 
 int ants_reconstruct_host(const ants_lrf_t *lrf, const float *signals_host, int64_t n_events,
                           const ants_grid_params_t *grid, int32_t method,
                           float *out_xyzA_host, float *out_score_host, int64_t chunk_events);
+
+/*
+ * ants_lrf_fit_axial -- LRF calculation (section 6: "The LRF module calculates these
+ * functions from datasets containing photosensor signals and the corresponding event positions";
+ * one LRF per sensor or one per group with relative gains; positions reconstructed
+ * or true).  This is the other half of the iterative response reconstruction of PAPER.md:428 (section 8):
+ * ants_reconstruct gives positions and energies, this call refits the axial B-spline LRFs from them.
+ * Readings R21-R23: unweighted least squares of y = S / (A g) against the uniform cubic
+ * B-spline at r = |p_xy - P_i|; an event takes part if x, y, A are finite and A > 0; a (event, sensor)
+ * pair takes part if r_lo <= r <= r_hi; signals enter as they are.
+ *   sensor_xy  HOST [N][2];  gains HOST [N] or NULL (all 1; used only when n_lrf == 1);
+ *   knots      HOST {r_lo, r_hi};  n_lrf = 1 (shared profile) or N (one table per sensor);
+ *   signals    DEVICE [n_events][N];  xyzA DEVICE [n_events][4] = x, y, z, A (out_xyzA of ants_reconstruct,
+ *              or true positions with A = the known light output);
+ *   coeffs_out HOST [n_lrf][n_int_r + 3] float;  n_used_out HOST [n_lrf] double or NULL: pairs per table.
+ * The normal equations are accumulated on the GPU in FP64 (one kernel launch on `cuda_stream`), the banded
+ * systems are solved on the host; the call allocates scratch and returns after the result is in host memory.
+ * Errors: ANTS_ERR_INVALID, ANTS_ERR_SINGULAR (an interval of some table received no data), ANTS_ERR_CUDA,
+ * ANTS_ERR_NOMEM, ANTS_ERR_UNSUPPORTED (accumulators larger than shared memory).
+ */
+int ants_lrf_fit_axial(const float *sensor_xy, const float *gains, const float *knots, int32_t n_sensors,
+                       int32_t n_lrf, int32_t n_int_r, const float *signals, const float *xyzA, int64_t n_events,
+                       float *coeffs_out, double *n_used_out, void *cuda_stream);
 
 /* Release the model and its device memory.  NULL is a no-op. */
 void ants_destroy(ants_lrf_t *lrf);

@@ -332,6 +332,7 @@ extern "C" const char *ants_strerror(int status) {
         case ANTS_ERR_UNSUPPORTED: return "unsupported combination or size";
         case ANTS_ERR_CUDA: return "CUDA runtime error";
         case ANTS_ERR_NOMEM: return "out of memory";
+        case ANTS_ERR_SINGULAR: return "underdetermined fit (an interval without data)";
         default: return "unknown status";
     }
 }
@@ -664,5 +665,114 @@ extern "C" int ants_reconstruct_host(const ants_lrf_t *lrf, const float *signals
     }
     for (int s = 0; s < 3; ++s)
         if (cudaStreamSynchronize(h->streams[s]) != cudaSuccess) { cudaGetLastError(); return ANTS_ERR_CUDA; }
+    return ANTS_OK;
+}
+
+// ---------------------------------------------------------------------------
+// LRF calculation: normal equations on the GPU (lrf_fit.cuh), banded solve here
+// ---------------------------------------------------------------------------
+#include "lrf_fit.cuh"
+
+// solve the symmetric positive definite system with half-bandwidth 3 stored as rows {d0, d1, d2, d3, rhs};
+// returns false when a pivot is not positive (underdetermined table)
+static bool solve_band3(const double *rows, int nc, double *x) {
+    std::vector<double> L((size_t)nc * 4, 0.0);      // L[j][d] = L(j + d, j), d = 0..3 (banded Cholesky)
+    for (int j = 0; j < nc; ++j) {
+        for (int d = 0; d < 4 && j + d < nc; ++d) {
+            double s = rows[(size_t)j * 5 + d];      // M(j + d, j)
+            for (int k = std::max(0, j + d - 3); k < j; ++k) s -= L[(size_t)k * 4 + (j + d - k)] * L[(size_t)k * 4 + (j - k)];
+            if (d == 0) {
+                if (!(s > 0.0) || !std::isfinite(s)) return false;
+                L[(size_t)j * 4] = std::sqrt(s);
+            } else {
+                L[(size_t)j * 4 + d] = s / L[(size_t)j * 4];
+            }
+        }
+    }
+    std::vector<double> y(nc);
+    for (int i = 0; i < nc; ++i) {
+        double s = rows[(size_t)i * 5 + 4];
+        for (int k = std::max(0, i - 3); k < i; ++k) s -= L[(size_t)k * 4 + (i - k)] * y[k];
+        y[i] = s / L[(size_t)i * 4];
+    }
+    for (int i = nc - 1; i >= 0; --i) {
+        double s = y[i];
+        for (int k = i + 1; k < std::min(nc, i + 4); ++k) s -= L[(size_t)i * 4 + (k - i)] * x[k];
+        x[i] = s / L[(size_t)i * 4];
+    }
+    return true;
+}
+
+extern "C" int ants_lrf_fit_axial(const float *sensor_xy, const float *gains, const float *knots, int32_t N,
+                                  int32_t n_lrf, int32_t n_int, const float *signals, const float *xyzA,
+                                  int64_t n_events, float *coeffs_out, double *n_used_out, void *cuda_stream) {
+    if (!sensor_xy || !knots || !coeffs_out || N < 1 || n_int < 1 || n_int > 4096 || n_events < 0) return ANTS_ERR_INVALID;
+    if (n_lrf != 1 && n_lrf != N) return ANTS_ERR_INVALID;
+    if (n_events > 0 && (!signals || !xyzA)) return ANTS_ERR_INVALID;
+    const double lo = (double)knots[0], hi = (double)knots[1];
+    if (!std::isfinite(lo) || !std::isfinite(hi) || !(lo >= 0.0) || !(hi > lo)) return ANTS_ERR_INVALID;
+    for (int i = 0; i < N; ++i)
+        if (gains && !(gains[i] > 0.f && std::isfinite(gains[i]))) return ANTS_ERR_INVALID;
+    const int nc = n_int + 3;
+    const size_t per_copy = (size_t)n_lrf * nc * 5;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+        cudaGetLastError();
+        return ANTS_ERR_CUDA;
+    }
+    const int warps = 8;
+    const int copies = n_lrf == 1 ? warps : 1;
+    const size_t smem = (per_copy * copies + (size_t)n_lrf) * sizeof(double);
+    if (smem > 227 * 1024) return ANTS_ERR_UNSUPPORTED;
+
+    std::vector<float> g(N, 1.f);
+    if (gains) std::copy(gains, gains + N, g.begin());
+    float *d_xy = nullptr, *d_g = nullptr;
+    double *d_acc = nullptr;
+    unsigned long long *d_used = nullptr;
+    auto cleanup = [&]() { cudaFree(d_xy); cudaFree(d_g); cudaFree(d_acc); cudaFree(d_used); cudaGetLastError(); };
+    if (cudaMalloc(&d_xy, (size_t)N * 2 * sizeof(float)) != cudaSuccess || cudaMalloc(&d_g, (size_t)N * sizeof(float)) != cudaSuccess ||
+        cudaMalloc(&d_acc, per_copy * sizeof(double)) != cudaSuccess ||
+        cudaMalloc(&d_used, (size_t)n_lrf * sizeof(unsigned long long)) != cudaSuccess) {
+        cleanup();
+        return ANTS_ERR_NOMEM;
+    }
+    bool ok = cudaMemcpyAsync(d_xy, sensor_xy, (size_t)N * 2 * sizeof(float), cudaMemcpyHostToDevice, st) == cudaSuccess &&
+              cudaMemcpyAsync(d_g, g.data(), (size_t)N * sizeof(float), cudaMemcpyHostToDevice, st) == cudaSuccess &&
+              cudaMemsetAsync(d_acc, 0, per_copy * sizeof(double), st) == cudaSuccess &&
+              cudaMemsetAsync(d_used, 0, (size_t)n_lrf * sizeof(unsigned long long), st) == cudaSuccess;
+    if (ok && n_events > 0) {
+        FitParams p{};
+        p.sens_xy = d_xy; p.gains = d_g; p.signals = signals; p.xyzA = xyzA; p.n_events = n_events;
+        p.N = N; p.n_lrf = n_lrf; p.n_int = n_int; p.nc = nc;
+        p.lo = lo; p.hi = hi; p.h = (hi - lo) / n_int;
+        p.acc = d_acc; p.n_used = d_used; p.copies = copies;
+        ok = cudaFuncSetAttribute((const void *)lrf_fit_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) == cudaSuccess;
+        int occ = 0;
+        ok = ok && cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void *)lrf_fit_kernel, warps * 32, smem) == cudaSuccess && occ >= 1;
+        if (ok) {
+            const long long want = (n_events + warps - 1) / warps;
+            const int grid = (int)std::min<long long>(want, (long long)sms * occ);
+            void *args[] = {&p};
+            ok = cudaLaunchKernel((const void *)lrf_fit_kernel, dim3(grid), dim3(warps * 32), args, smem, st) == cudaSuccess;
+            if (ok) g_launches.fetch_add(1);
+        }
+    }
+    std::vector<double> acc(per_copy);
+    std::vector<unsigned long long> used(n_lrf);
+    ok = ok && cudaMemcpyAsync(acc.data(), d_acc, per_copy * sizeof(double), cudaMemcpyDeviceToHost, st) == cudaSuccess &&
+         cudaMemcpyAsync(used.data(), d_used, (size_t)n_lrf * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st) == cudaSuccess &&
+         cudaStreamSynchronize(st) == cudaSuccess;
+    cleanup();
+    if (!ok) return ANTS_ERR_CUDA;
+    std::vector<double> x(nc);
+    for (int m = 0; m < n_lrf; ++m) {
+        if (n_used_out) n_used_out[m] = (double)used[m];
+        if (!solve_band3(acc.data() + (size_t)m * nc * 5, nc, x.data())) return ANTS_ERR_SINGULAR;
+        for (int j = 0; j < nc; ++j) coeffs_out[(size_t)m * nc + j] = (float)x[j];
+    }
     return ANTS_OK;
 }

@@ -1,0 +1,92 @@
+// lrf_fit.cuh -- LRF calculation for axial LRFs: least-squares B-spline fit from event positions and
+// sensor signals (section 6 "The LRF module calculates these functions from datasets
+// containing photosensor signals and the corresponding event positions"; PAPER.md:400-414 grouping,
+// positions reconstructed or true).  Readings R21-R23: unweighted least squares of
+// y = S / (A g) against the uniform cubic B-spline at r = |p - P_i|; events need finite x, y, A and
+// A > 0; pairs need r_lo <= r <= r_hi.
+//
+// The kernel accumulates the normal equations M = sum B^T B (symmetric, half-bandwidth 3) and
+// b = sum B^T y in FP64: one warp per event, lanes over sensors, every pair adds 10 band entries and
+// 4 right-hand-side entries with shared-memory FP64 atomics into the CTA's copy (one copy per warp for a
+// shared profile, where all sensors hit the same table), which is flushed once to the global
+// accumulators.  All arithmetic is double: the path is bound by the atomics and by the signal stream,
+// not by FP64 throughput.  The host solves the banded systems (ants_recon.cu).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace ants {
+
+struct FitParams {
+    const float *sens_xy;        // device [N][2]
+    const float *gains;          // device [N] (all 1 when the caller passed none)
+    const float *signals;        // device [E][N]
+    const float *xyzA;           // device [E][4]
+    long long n_events;
+    int N, n_lrf, n_int, nc;     // nc = n_int + 3 coefficients
+    double lo, hi, h;            // h = (hi - lo) / n_int
+    double *acc;                 // device [n_lrf][nc][5]: {M[j][j], M[j][j+1], M[j][j+2], M[j][j+3], b[j]}
+    unsigned long long *n_used;  // device [n_lrf]
+    int copies;                  // shared-memory copies of the accumulators per CTA (1, or warps per CTA)
+};
+
+__global__ void __launch_bounds__(256) lrf_fit_kernel(const FitParams p) {
+    extern __shared__ double fit_smem[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, warps = blockDim.x >> 5;
+    const int per_copy = p.n_lrf * p.nc * 5;
+    for (int i = threadIdx.x; i < per_copy * p.copies; i += blockDim.x) fit_smem[i] = 0.0;
+    if (p.n_lrf > 1)
+        for (int i = threadIdx.x; i < p.n_lrf; i += blockDim.x)
+            reinterpret_cast<unsigned long long *>(fit_smem + (size_t)per_copy * p.copies)[i] = 0ULL;
+    __syncthreads();
+    double *mine = fit_smem + (p.copies > 1 ? warp * per_copy : 0);
+    // pairs used: a register count for a shared profile, shared-memory counters for per-sensor tables
+    unsigned long long *cnt = reinterpret_cast<unsigned long long *>(fit_smem + (size_t)per_copy * p.copies);
+    unsigned long long used = 0ULL;
+
+    for (long long e = (long long)blockIdx.x * warps + warp; e < p.n_events; e += (long long)gridDim.x * warps) {
+        const float4 pe = reinterpret_cast<const float4 *>(p.xyzA)[e];
+        const double x = (double)pe.x, y = (double)pe.y, A = (double)pe.w;
+        // R22: finite x, y, A and A > 0 (NaN fails every comparison)
+        if (!(fabs(x) <= 1.7e308 && fabs(y) <= 1.7e308 && A > 0.0 && A <= 1.7e308)) continue;
+        const float *sig = p.signals + e * p.N;
+        for (int i = lane; i < p.N; i += 32) {
+            const double dx = x - (double)p.sens_xy[2 * i], dy = y - (double)p.sens_xy[2 * i + 1];
+            const double r = sqrt(dx * dx + dy * dy);
+            if (!(r >= p.lo && r <= p.hi)) continue;                                   // R22
+            const double g = p.n_lrf == 1 ? (double)p.gains[i] : 1.0;
+            const double yv = (double)__ldg(sig + i) / (A * g);                         // R21, R23
+            const double t = (r - p.lo) / p.h;
+            const int k = min((int)floor(t), p.n_int - 1);
+            const double u = t - (double)k, o = 1.0 - u, u2 = u * u, u3 = u2 * u;
+            const double b4[4] = {o * o * o / 6.0, (3.0 * u3 - 6.0 * u2 + 4.0) / 6.0,
+                                  (-3.0 * u3 + 3.0 * u2 + 3.0 * u + 1.0) / 6.0, u3 / 6.0};
+            double *tab = mine + (size_t)(p.n_lrf == 1 ? 0 : i) * p.nc * 5;
+#pragma unroll
+            for (int a = 0; a < 4; ++a) {
+                double *row = tab + (size_t)(k + a) * 5;
+                atomicAdd(row + 4, b4[a] * yv);
+#pragma unroll
+                for (int c = a; c < 4; ++c) atomicAdd(row + (c - a), b4[a] * b4[c]);
+            }
+            if (p.n_lrf == 1) ++used;
+            else atomicAdd(cnt + i, 1ULL);
+        }
+    }
+    if (p.n_lrf == 1) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) used += __shfl_xor_sync(0xffffffffu, used, o);
+        if (lane == 0 && used) atomicAdd(p.n_used, used);
+    }
+    __syncthreads();
+    if (p.n_lrf > 1)
+        for (int i = threadIdx.x; i < p.n_lrf; i += blockDim.x)
+            if (cnt[i]) atomicAdd(p.n_used + i, cnt[i]);
+    for (int i = threadIdx.x; i < per_copy; i += blockDim.x) {
+        double s = 0.0;
+        for (int c = 0; c < p.copies; ++c) s += fit_smem[c * per_copy + i];
+        if (s != 0.0) atomicAdd(p.acc + i, s);
+    }
+}
+
+}  // namespace ants

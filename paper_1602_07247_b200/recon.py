@@ -57,6 +57,8 @@ def load():
     lib.ants_reconstruct_host.argtypes = [vp, vp, C.c_int64, C.POINTER(GridParams), C.c_int32, vp, vp, C.c_int64]
     lib.ants_lrf_set_selection.restype = C.c_int
     lib.ants_lrf_set_selection.argtypes = [vp, vp, C.c_float, C.c_float]
+    lib.ants_lrf_fit_axial.restype = C.c_int
+    lib.ants_lrf_fit_axial.argtypes = [vp, vp, vp, C.c_int32, C.c_int32, C.c_int32, vp, vp, C.c_int64, vp, vp, vp]
     lib.ants_destroy.restype = None
     lib.ants_destroy.argtypes = [vp]
     lib.ants_strerror.restype = C.c_char_p
@@ -100,6 +102,30 @@ def ants_lrf_set_selection(handle, passive=None, signal_min=float("nan"), dist_m
                                        float(dist_max))
     if rc != 0:
         raise AntsError(rc, "ants_lrf_set_selection")
+
+
+def ants_lrf_fit_axial(sensor_xy, gains, knots, n_lrf: int, n_int_r: int, signals, xyzA, stream=None):
+    """LRF calculation (include/ants_recon.h): signals [E][N] and xyzA [E][4] are CUDA float32 tensors.
+    -> (coeffs float32 [n_lrf][n_int_r + 3], pairs used per table float64 [n_lrf])."""
+    import torch
+    xy, kn = _f32(sensor_xy).reshape(-1, 2), _f32(knots)
+    N = xy.shape[0]
+    g = None if gains is None else _f32(gains)
+    for t in (signals, xyzA):
+        if not (t.is_cuda and t.is_contiguous() and t.dtype == torch.float32):
+            raise ValueError("ants_lrf_fit_axial needs contiguous float32 CUDA tensors")
+    E = int(signals.shape[0])
+    if signals.shape[1] != N or tuple(xyzA.shape) != (E, 4):
+        raise ValueError("ants_lrf_fit_axial: shape mismatch")
+    coeffs = np.zeros((int(n_lrf), int(n_int_r) + 3), np.float32)
+    used = np.zeros(int(n_lrf), np.float64)
+    st = torch.cuda.current_stream().cuda_stream if stream is None else int(stream)
+    rc = load().ants_lrf_fit_axial(xy.ctypes.data, None if g is None else g.ctypes.data, kn.ctypes.data, N,
+                                   int(n_lrf), int(n_int_r), signals.data_ptr(), xyzA.data_ptr(), E,
+                                   coeffs.ctypes.data, used.ctypes.data, st)
+    if rc != 0:
+        raise AntsError(rc, "ants_lrf_fit_axial")
+    return coeffs, used
 
 
 def ants_destroy(handle) -> None:

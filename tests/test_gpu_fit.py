@@ -1,0 +1,106 @@
+"""GPU-vs-oracle parity of the LRF calculation (ants_lrf_fit_axial vs oracle/fit.py), -m gpu, and the
+reconstruct <-> refit cycle of PAPER.md:428 (section 8) on synthetic flood data.
+
+Tolerance: both sides accumulate the normal equations in FP64 from the same float32 inputs and solve them
+in FP64; they differ by summation order (atomics) only, ~1e-13 relative on M and b, amplified by the
+conditioning of the spline normal matrix (<= ~1e4 here) and then rounded to float32 on output:
+|c_gpu - c_oracle| <= 2e-6 max|c| per table.  Pair counts are integers: bit-exact."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+from oracle import fit as ofit                                 # noqa: E402
+from paper_1602_07247_b200 import recon, synth                 # noqa: E402
+
+TOL = 2e-6
+
+
+def _reconstructed(idx, n):
+    cfg = synth.make_config(idx)
+    ev = synth.generate_events(cfg, n, device="cuda")
+    r = recon.Reconstructor(cfg)
+    try:
+        xyzA, _ = r(ev["signals"])
+        torch.cuda.synchronize()
+    finally:
+        r.close()
+    return cfg, ev, xyzA
+
+
+@pytest.mark.parametrize("idx,n", [(2, 60_011), (5, 12_007), (1, 9_001)])
+def test_fit_parity_on_reconstructed_positions(idx, n):
+    cfg, ev, xyzA = _reconstructed(idx, n)
+    c, used = recon.ants_lrf_fit_axial(cfg.sensor_xy, cfg.gains, cfg.knots, cfg.n_lrf, cfg.n_int_r, ev["signals"], xyzA)
+    c0, used0 = ofit.fit_axial(cfg.sensor_xy, cfg.gains, cfg.knots, cfg.n_lrf, cfg.n_int_r,
+                               ev["signals"].cpu().numpy(), xyzA.cpu().numpy())
+    assert np.array_equal(used, used0)
+    assert np.abs(c - c0).max() <= TOL * np.abs(c0).max()
+
+
+def test_fit_parity_individual_tables():
+    """Per-sensor tables (config 3's sensors) with true positions spread so that every sensor sees its whole
+    r-range; a tail of failed events (NaN rows) and events with non-positive energy must be ignored."""
+    cfg = synth.make_config(3)
+    rng = np.random.default_rng(5)
+    E = 40_009
+    pos = np.zeros((E, 4), np.float32)
+    pos[:, :2] = rng.uniform(-55.0, 55.0, (E, 2))
+    pos[:, 3] = rng.uniform(100.0, 400.0, E)
+    r = np.hypot(pos[:, None, 0] - cfg.sensor_xy[None, :, 0], pos[:, None, 1] - cfg.sensor_xy[None, :, 1])
+    mean = np.stack([synth.eval_axial(cfg.coeffs[i, 0], 0.0, 40.0, r[:, i].astype(float)) for i in range(64)], axis=1)
+    sig = rng.poisson(np.maximum(pos[:, 3:4] * mean, 0.0)).astype(np.float32)
+    pos[::13] = np.nan
+    pos[5::17, 3] = 0.0
+    c, used = recon.ants_lrf_fit_axial(cfg.sensor_xy, None, cfg.knots, 64, cfg.n_int_r,
+                                       torch.from_numpy(sig).cuda(), torch.from_numpy(pos).cuda())
+    c0, used0 = ofit.fit_axial(cfg.sensor_xy, None, cfg.knots, 64, cfg.n_int_r, sig, pos)
+    assert np.array_equal(used, used0)
+    assert (np.abs(c - c0).max(axis=1) <= TOL * np.abs(c0).max(axis=1)).all()
+    # and the fit is near the truth it was drawn from (statistics, not parity)
+    assert np.abs(c[:, 3:9] - cfg.coeffs[:, 0, 3:9]).max() < 0.05
+
+
+def test_underdetermined_table_is_reported():
+    cfg = synth.make_config(2)
+    pos = torch.zeros((100, 4), device="cuda")
+    pos[:, 3] = 1.0
+    sig = torch.ones((100, cfg.n_sensors), device="cuda")
+    with pytest.raises(recon.AntsError) as ei:
+        recon.ants_lrf_fit_axial(cfg.sensor_xy, cfg.gains, cfg.knots, 1, cfg.n_int_r, sig, pos)
+    assert ei.value.status == -5
+    with pytest.raises(recon.AntsError) as ei:
+        recon.ants_lrf_fit_axial(cfg.sensor_xy, cfg.gains, np.array([9.0, 1.0], np.float32), 1, cfg.n_int_r, sig, pos)
+    assert ei.value.status == -1
+
+
+def test_reconstruct_refit_cycle_recovers_the_response():
+    """PAPER.md:428 (section 8): start from a WRONG response (profile 25 % too wide), alternate
+    reconstruction and LRF calculation on flood data; the fitted profile moves to the true one."""
+    true = synth.make_config(2)
+    ev = synth.generate_events(true, 200_000, device="cuda")
+    guess = synth.make_config(2)
+    guess.coeffs = synth.fit_axial(lambda r: (1.0 + (r / 25.0) ** 2) ** -1.5, 0.0, 90.0, 16)[None, None, :]
+    r_probe = np.linspace(2.0, 80.0, 40)
+    truth = synth.eval_axial(true.coeffs[0, 0], 0.0, 90.0, r_probe)
+
+    def shape_error(c):
+        s = synth.eval_axial(np.asarray(c, np.float32), 0.0, 90.0, r_probe)
+        s = s * (truth @ s) / (s @ s)              # the overall scale trades with the energy: compare shapes
+        return float(np.abs(s - truth).max() / truth.max())
+
+    err = [shape_error(guess.coeffs[0, 0])]
+    cur = guess
+    for _ in range(6):
+        rc = recon.Reconstructor(cur)
+        try:
+            xyzA, _ = rc(ev["signals"])
+        finally:
+            rc.close()
+        c, used = recon.ants_lrf_fit_axial(cur.sensor_xy, cur.gains, cur.knots, 1, cur.n_int_r, ev["signals"], xyzA)
+        cur = synth.make_config(2)
+        cur.coeffs = c[None, :, :].astype(np.float32)
+        err.append(shape_error(c[0]))
+    assert err[0] > 0.03 and err[-1] < 0.5 * err[0], err

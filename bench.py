@@ -331,6 +331,65 @@ TRAFFIC_PER_EVENT = {"cfg2_pmt2d_hex19": 87.83, "cfg3_sipm_chi2_sq64": 257.5, "c
                      "cfg5_flood_hex127": 547.2}
 
 
+# ---------------------------------------------------------------------------
+# secondary workload: the LRF calculation (ants_lrf_fit_axial), `--workload fit`
+# ---------------------------------------------------------------------------
+def run_fit(args):
+    """Times ants_lrf_fit_axial (normal equations on the GPU + host solve) on the config's batch with the
+    positions reconstructed by the library.  HBM roofline: the call must read the signals (4N B) and the
+    positions (16 B) of every event once; peak = MEASURED_PEAKS.json hbm_gbs (fallback 6650, said so)."""
+    import torch
+    from paper_1602_07247_b200 import recon, synth
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    device = torch.device("cuda", 0)
+    cfg = synth.make_config(args.config)
+    if cfg.lrf_dim != 1:
+        raise SystemExit("--workload fit: axial LRFs only (configs 1, 2, 3, 5)")
+    E = cfg.n_events // cfg.n_batches if args.events is None else args.events
+    sig = synth.generate_events(cfg, E, device=device)["signals"]
+    r = recon.Reconstructor(cfg)
+    xyzA, _ = r(sig)
+    r.close()
+    if cfg.n_lrf > 1:       # per-sensor tables need data over the whole r-range of every sensor: use all of it they see
+        knots = cfg.knots.copy()
+        knots[1] = min(float(knots[1]), 30.0)
+    else:
+        knots = cfg.knots
+    torch.cuda.synchronize()
+    stream = torch.cuda.current_stream()
+    n0 = recon.launch_count()
+    for _ in range(args.warmup):
+        recon.ants_lrf_fit_axial(cfg.sensor_xy, cfg.gains, knots, cfg.n_lrf, cfg.n_int_r, sig, xyzA)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    n1 = recon.launch_count()
+    for a, b in ev:
+        a.record(stream)
+        coeffs, used = recon.ants_lrf_fit_axial(cfg.sensor_xy, cfg.gains, knots, cfg.n_lrf, cfg.n_int_r, sig, xyzA)
+        b.record(stream)
+    torch.cuda.synchronize()
+    ms = [a.elapsed_time(b) for a, b in ev]
+    t = sum(ms) / len(ms) * 1e-3
+    peak, src = 6650.0, "fallback"
+    try:
+        peak, src = float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]), "measured"
+    except Exception:
+        pass
+    bytes_alg = E * (4 * cfg.n_sensors + 16)
+    line = {"metric": "events/s whose signals enter one LRF calculation (ants_lrf_fit_axial)", "value": E / t,
+            "unit": "events/s", "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": t * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": cfg.name + " LRF calculation", "events_per_step_per_gpu": E, "n_sensors": cfg.n_sensors,
+                       "n_lrf": cfg.n_lrf, "n_int_r": cfg.n_int_r, "pairs_used": float(used.sum())},
+            "gpu_launches": recon.launch_count() - n1,
+            "roofline": {"bound": "hbm", "achieved": bytes_alg / t / 1e9, "peak": peak, "unit": "GB/s",
+                         "frac": bytes_alg / t / 1e9 / peak, "traffic": None, "peak_source": src + " hbm_gbs",
+                         "pairs_per_s": float(used.sum()) / t, "smem_fp64_atomics_per_s": 14.0 * float(used.sum()) / t},
+            "step_ms": ms}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
 def main(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -344,9 +403,13 @@ def main(argv=None):
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--ref-step-seconds", type=float, default=4.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--workload", default="reconstruct", choices=["reconstruct", "fit"],
+                    help="fit = time the LRF calculation instead (secondary; not the BASELINE metric)")
     args = ap.parse_args(argv)
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = max(args.warmup, 1)
+    if args.workload == "fit":
+        return run_fit(args)
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)

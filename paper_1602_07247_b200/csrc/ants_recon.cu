@@ -724,7 +724,14 @@ extern "C" int ants_lrf_fit_axial(const float *sensor_xy, const float *gains, co
         return ANTS_ERR_CUDA;
     }
     const int warps = 8;
-    const int copies = n_lrf == 1 ? warps : 1;
+    // shared profile: as many private copies per warp as fit in ~64 KB (fewer lanes per copy, less contention)
+    int lane_split = 1;
+    if (n_lrf == 1) {
+        lane_split = 4;      // measured on B200: 4 is the best of 1..16 (more copies cost resident CTAs)
+        while (lane_split > 1 && per_copy * warps * lane_split * sizeof(double) > 32 * 1024) lane_split >>= 1;
+    }
+    if (const char *e = std::getenv("ANTS_FIT_LANE_SPLIT")) { const int v = std::atoi(e); if (v >= 1 && v <= 32 && n_lrf == 1) lane_split = v; }
+    const int copies = n_lrf == 1 ? warps * lane_split : 1;
     const size_t smem = (per_copy * copies + (size_t)n_lrf) * sizeof(double);
     if (smem > 227 * 1024) return ANTS_ERR_UNSUPPORTED;
 
@@ -749,7 +756,7 @@ extern "C" int ants_lrf_fit_axial(const float *sensor_xy, const float *gains, co
         p.sens_xy = d_xy; p.gains = d_g; p.signals = signals; p.xyzA = xyzA; p.n_events = n_events;
         p.N = N; p.n_lrf = n_lrf; p.n_int = n_int; p.nc = nc;
         p.lo = lo; p.hi = hi; p.h = (hi - lo) / n_int;
-        p.acc = d_acc; p.n_used = d_used; p.copies = copies;
+        p.acc = d_acc; p.n_used = d_used; p.copies = copies; p.lane_split = lane_split;
         ok = cudaFuncSetAttribute((const void *)lrf_fit_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) == cudaSuccess;
         int occ = 0;
         ok = ok && cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void *)lrf_fit_kernel, warps * 32, smem) == cudaSuccess && occ >= 1;

@@ -27,7 +27,8 @@ struct FitParams {
     double lo, hi, h;            // h = (hi - lo) / n_int
     double *acc;                 // device [n_lrf][nc][5]: {M[j][j], M[j][j+1], M[j][j+2], M[j][j+3], b[j]}
     unsigned long long *n_used;  // device [n_lrf]
-    int copies;                  // shared-memory copies of the accumulators per CTA (1, or warps per CTA)
+    int copies;                  // shared-memory copies of the accumulators per CTA (1, or warps * lane_split)
+    int lane_split;              // copies per warp (contention on the FP64 atomics falls with it)
 };
 
 __global__ void __launch_bounds__(256) lrf_fit_kernel(const FitParams p) {
@@ -39,7 +40,8 @@ __global__ void __launch_bounds__(256) lrf_fit_kernel(const FitParams p) {
         for (int i = threadIdx.x; i < p.n_lrf; i += blockDim.x)
             reinterpret_cast<unsigned long long *>(fit_smem + (size_t)per_copy * p.copies)[i] = 0ULL;
     __syncthreads();
-    double *mine = fit_smem + (p.copies > 1 ? warp * per_copy : 0);
+    // shared profile: copies = warps * lane_split private copies, lanes of a warp spread over lane_split of them
+    double *mine = fit_smem + (p.copies > 1 ? (size_t)(warp * p.lane_split + (lane % p.lane_split)) * per_copy : 0);
     // pairs used: a register count for a shared profile, shared-memory counters for per-sensor tables
     unsigned long long *cnt = reinterpret_cast<unsigned long long *>(fit_smem + (size_t)per_copy * p.copies);
     unsigned long long used = 0ULL;

@@ -70,3 +70,38 @@ def fit_axial(sensor_xy, gains, knots, n_lrf, n_int, signals, xyzA):
     M, b, n_used = normal_equations(sensor_xy, gains, knots, n_lrf, n_int, signals, xyzA)
     c = np.stack([np.linalg.solve(M[m], b[m]) for m in range(n_lrf)])
     return c, n_used
+
+
+def spline_values(coeffs, lo, hi, n_int, r):
+    """Uniform cubic B-spline of oracle/ants_oracle.c (R7) at r in [lo, hi], float64."""
+    c = np.asarray(coeffs, np.float32).astype(np.float64)
+    h = (hi - lo) / n_int
+    t = (r - lo) / h
+    k = np.minimum(np.floor(t).astype(np.int64), n_int - 1)
+    B4 = basis4(t - k)
+    return sum(c[k + a] * B4[:, a] for a in range(4))
+
+
+def fit_gains(sensor_xy, knots, coeffs, n_int, signals, xyzA):
+    """Relative gains for a FIXED shared profile (section 6.3: "re-calculate the relative gains
+    of the photosensors within already defined groups without affecting the LRF profiles").  Reading R24:
+    g_i minimises sum_e (S_ie/A_e - g_i s(r_ie))^2 over the pairs of R22, i.e.
+    g_i = sum_e y s / sum_e s^2 with y = S_ie/A_e.  -> gains [N] (NaN where a sensor has no pair), pairs [N]."""
+    xy = np.asarray(sensor_xy, np.float32).astype(np.float64).reshape(-1, 2)
+    N = xy.shape[0]
+    lo, hi = (float(np.float32(k)) for k in knots[:2])
+    S = np.asarray(signals, np.float32).astype(np.float64).reshape(-1, N)
+    P = np.asarray(xyzA, np.float32).astype(np.float64).reshape(-1, 4)
+    ok = np.isfinite(P[:, 0]) & np.isfinite(P[:, 1]) & np.isfinite(P[:, 3]) & (P[:, 3] > 0.0)
+    gains, used = np.full(N, np.nan), np.zeros(N)
+    for i in range(N):
+        with np.errstate(invalid="ignore"):
+            r = np.hypot(P[:, 0] - xy[i, 0], P[:, 1] - xy[i, 1])
+            use = ok & (r >= lo) & (r <= hi)
+        s = spline_values(coeffs, lo, hi, n_int, r[use])
+        y = S[use, i] / P[use, 3]
+        den = float((s * s).sum())
+        used[i] = use.sum()
+        if den > 0.0:
+            gains[i] = float((y * s).sum()) / den
+    return gains, used

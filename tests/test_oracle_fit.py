@@ -92,3 +92,28 @@ def test_underdetermined_table_raises():
     pos[:, 0:2] = 0.0                                         # all events at one point: most intervals empty
     with pytest.raises(np.linalg.LinAlgError):
         fit.fit_axial(cfg.sensor_xy, cfg.gains, cfg.knots, 1, cfg.n_int_r, sig, pos)
+
+
+# ---------------------------------------------------------------------------
+# relative gains for a fixed profile (R24)
+# ---------------------------------------------------------------------------
+def test_gains_are_recovered_from_noise_free_data_and_match_lstsq():
+    cfg, sig, pos = _problem(2, 3000)
+    g, used = fit.fit_gains(cfg.sensor_xy, cfg.knots, cfg.coeffs[0, 0], cfg.n_int_r, sig, pos)
+    assert np.abs(g - cfg.gains).max() <= 2e-6 and (used > 0).all()
+    cfg, sig, pos = _problem(5, 800, noise=0.7)
+    g, used = fit.fit_gains(cfg.sensor_xy, cfg.knots, cfg.coeffs[0, 0], cfg.n_int_r, sig, pos)
+    lo, hi = float(cfg.knots[0]), float(cfg.knots[1])
+    for i in (0, 50, 126):                                   # the 1-D least-squares problem through scipy + lstsq
+        r = np.hypot(pos[:, 0].astype(float) - float(cfg.sensor_xy[i, 0]), pos[:, 1].astype(float) - float(cfg.sensor_xy[i, 1]))
+        use = (r >= lo) & (r <= hi)
+        s = synth.eval_axial(cfg.coeffs[0, 0], lo, hi, r[use])
+        ref, *_ = np.linalg.lstsq(s[:, None], sig[use, i].astype(float) / pos[use, 3].astype(float), rcond=None)
+        assert g[i] == pytest.approx(ref[0], rel=1e-10) and used[i] == use.sum()
+
+
+def test_gain_of_a_sensor_without_data_is_nan():
+    cfg, sig, pos = _problem(2, 200)
+    pos[:, 0:2] = 300.0                                       # every sensor farther than r_hi
+    g, used = fit.fit_gains(cfg.sensor_xy, cfg.knots, cfg.coeffs[0, 0], cfg.n_int_r, sig, pos)
+    assert np.isnan(g).all() and (used == 0).all()

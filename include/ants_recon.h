@@ -173,6 +173,21 @@ int ants_lrf_fit_axial(const float *sensor_xy, const float *gains, const float *
                        int32_t n_lrf, int32_t n_int_r, const float *signals, const float *xyzA, int64_t n_events,
                        float *coeffs_out, double *n_used_out, void *cuda_stream);
 
+/*
+ * ants_lrf_fit_gains -- relative gains of the sensors for a FIXED shared profile (section 6.3:
+ * "re-calculate the relative gains of the photosensors within already defined groups without affecting the
+ * LRF profiles").  Reading R24: g_i = sum_e y s(r_ie) / sum_e s(r_ie)^2, y = S_ie / A_e, over the events and
+ * pairs of R22 (as in ants_lrf_fit_axial).
+ *   sensor_xy HOST [N][2], knots HOST {r_lo, r_hi}, coeffs HOST [n_int_r + 3] (the shared profile),
+ *   signals DEVICE [n_events][N], xyzA DEVICE [n_events][4];
+ *   gains_out HOST [N] float (NaN for a sensor without any pair), n_used_out HOST [N] double or NULL.
+ * One kernel launch on `cuda_stream` (FP64 sums kept in registers per lane, N <= 128); returns after the
+ * result is in host memory.  Errors: ANTS_ERR_INVALID, ANTS_ERR_UNSUPPORTED (N > 128), ANTS_ERR_CUDA, ANTS_ERR_NOMEM.
+ */
+int ants_lrf_fit_gains(const float *sensor_xy, const float *knots, const float *coeffs, int32_t n_sensors,
+                       int32_t n_int_r, const float *signals, const float *xyzA, int64_t n_events,
+                       float *gains_out, double *n_used_out, void *cuda_stream);
+
 /* Release the model and its device memory.  NULL is a no-op. */
 void ants_destroy(ants_lrf_t *lrf);
 

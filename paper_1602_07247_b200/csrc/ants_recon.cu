@@ -783,3 +783,67 @@ extern "C" int ants_lrf_fit_axial(const float *sensor_xy, const float *gains, co
     }
     return ANTS_OK;
 }
+
+extern "C" int ants_lrf_fit_gains(const float *sensor_xy, const float *knots, const float *coeffs, int32_t N,
+                                  int32_t n_int, const float *signals, const float *xyzA, int64_t n_events,
+                                  float *gains_out, double *n_used_out, void *cuda_stream) {
+    if (!sensor_xy || !knots || !coeffs || !gains_out || N < 1 || n_int < 1 || n_int > 4096 || n_events < 0)
+        return ANTS_ERR_INVALID;
+    if (n_events > 0 && (!signals || !xyzA)) return ANTS_ERR_INVALID;
+    if (N > 128) return ANTS_ERR_UNSUPPORTED;
+    const double lo = (double)knots[0], hi = (double)knots[1];
+    if (!std::isfinite(lo) || !std::isfinite(hi) || !(lo >= 0.0) || !(hi > lo)) return ANTS_ERR_INVALID;
+    for (int j = 0; j < n_int + 3; ++j)
+        if (!std::isfinite(coeffs[j])) return ANTS_ERR_INVALID;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+        cudaGetLastError();
+        return ANTS_ERR_CUDA;
+    }
+    float *d_xy = nullptr, *d_c = nullptr;
+    double *d_acc = nullptr;
+    unsigned long long *d_used = nullptr;
+    auto cleanup = [&]() { cudaFree(d_xy); cudaFree(d_c); cudaFree(d_acc); cudaFree(d_used); cudaGetLastError(); };
+    if (cudaMalloc(&d_xy, (size_t)N * 2 * sizeof(float)) != cudaSuccess || cudaMalloc(&d_c, (size_t)(n_int + 3) * sizeof(float)) != cudaSuccess ||
+        cudaMalloc(&d_acc, (size_t)N * 2 * sizeof(double)) != cudaSuccess ||
+        cudaMalloc(&d_used, (size_t)N * sizeof(unsigned long long)) != cudaSuccess) {
+        cleanup();
+        return ANTS_ERR_NOMEM;
+    }
+    bool ok = cudaMemcpyAsync(d_xy, sensor_xy, (size_t)N * 2 * sizeof(float), cudaMemcpyHostToDevice, st) == cudaSuccess &&
+              cudaMemcpyAsync(d_c, coeffs, (size_t)(n_int + 3) * sizeof(float), cudaMemcpyHostToDevice, st) == cudaSuccess &&
+              cudaMemsetAsync(d_acc, 0, (size_t)N * 2 * sizeof(double), st) == cudaSuccess &&
+              cudaMemsetAsync(d_used, 0, (size_t)N * sizeof(unsigned long long), st) == cudaSuccess;
+    if (ok && n_events > 0) {
+        GainParams p{};
+        p.sens_xy = d_xy; p.coeffs = d_c; p.signals = signals; p.xyzA = xyzA; p.n_events = n_events;
+        p.N = N; p.n_int = n_int; p.lo = lo; p.hi = hi; p.h = (hi - lo) / n_int;
+        p.acc = d_acc; p.n_used = d_used;
+        const int warps = 8;
+        const size_t smem = (size_t)(n_int + 3) * sizeof(double);
+        int occ = 0;
+        ok = cudaFuncSetAttribute((const void *)lrf_gain_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) == cudaSuccess &&
+             cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void *)lrf_gain_kernel, warps * 32, smem) == cudaSuccess && occ >= 1;
+        if (ok) {
+            const long long want = (n_events + warps - 1) / warps;
+            const int grid = (int)std::min<long long>(want, (long long)sms * occ);
+            void *args[] = {&p};
+            ok = cudaLaunchKernel((const void *)lrf_gain_kernel, dim3(grid), dim3(warps * 32), args, smem, st) == cudaSuccess;
+            if (ok) g_launches.fetch_add(1);
+        }
+    }
+    std::vector<double> acc((size_t)N * 2);
+    std::vector<unsigned long long> used(N);
+    ok = ok && cudaMemcpyAsync(acc.data(), d_acc, acc.size() * sizeof(double), cudaMemcpyDeviceToHost, st) == cudaSuccess &&
+         cudaMemcpyAsync(used.data(), d_used, used.size() * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st) == cudaSuccess &&
+         cudaStreamSynchronize(st) == cudaSuccess;
+    cleanup();
+    if (!ok) return ANTS_ERR_CUDA;
+    for (int i = 0; i < N; ++i) {
+        if (n_used_out) n_used_out[i] = (double)used[i];
+        gains_out[i] = acc[2 * i + 1] > 0.0 ? (float)(acc[2 * i] / acc[2 * i + 1]) : std::nanf("");
+    }
+    return ANTS_OK;
+}

@@ -91,4 +91,68 @@ __global__ void __launch_bounds__(256) lrf_fit_kernel(const FitParams p) {
     }
 }
 
+// ---- relative gains for a fixed shared profile (R24): g_i = sum y s / sum s^2 --------
+// One warp per event, lanes over sensors; every lane keeps the two sums of the sensors it owns
+// (i = lane + 32 c, c < 4: N <= 128) in registers for all the events its warp sees -- no atomics in the
+// loop -- and adds them to the global FP64 accumulators once at the end.
+struct GainParams {
+    const float *sens_xy;        // device [N][2]
+    const float *coeffs;         // device [n_int + 3]
+    const float *signals;        // device [E][N]
+    const float *xyzA;           // device [E][4]
+    long long n_events;
+    int N, n_int;
+    double lo, hi, h;
+    double *acc;                 // device [N][2]: {sum y s, sum s^2}
+    unsigned long long *n_used;  // device [N]
+};
+
+__global__ void __launch_bounds__(256) lrf_gain_kernel(const GainParams p) {
+    extern __shared__ double gain_smem[];      // the profile's coefficients in double
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, warps = blockDim.x >> 5;
+    for (int j = threadIdx.x; j < p.n_int + 3; j += blockDim.x) gain_smem[j] = (double)p.coeffs[j];
+    __syncthreads();
+    double num[4] = {0, 0, 0, 0}, den[4] = {0, 0, 0, 0};
+    unsigned long long cnt[4] = {0, 0, 0, 0};
+    double sx[4], sy[4];
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+        const int i = lane + 32 * c;
+        sx[c] = i < p.N ? (double)p.sens_xy[2 * i] : 0.0;
+        sy[c] = i < p.N ? (double)p.sens_xy[2 * i + 1] : 0.0;
+    }
+    for (long long e = (long long)blockIdx.x * warps + warp; e < p.n_events; e += (long long)gridDim.x * warps) {
+        const float4 pe = reinterpret_cast<const float4 *>(p.xyzA)[e];
+        const double x = (double)pe.x, y = (double)pe.y, A = (double)pe.w;
+        if (!(fabs(x) <= 1.7e308 && fabs(y) <= 1.7e308 && A > 0.0 && A <= 1.7e308)) continue;    // R22
+        const float *sig = p.signals + e * p.N;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            const int i = lane + 32 * c;
+            if (i >= p.N) continue;
+            const double dx = x - sx[c], dy = y - sy[c];
+            const double r = sqrt(dx * dx + dy * dy);
+            if (!(r >= p.lo && r <= p.hi)) continue;
+            const double t = (r - p.lo) / p.h;
+            const int k = min((int)floor(t), p.n_int - 1);
+            const double u = t - (double)k, o = 1.0 - u, u2 = u * u, u3 = u2 * u;
+            const double s = gain_smem[k] * (o * o * o / 6.0) + gain_smem[k + 1] * ((3.0 * u3 - 6.0 * u2 + 4.0) / 6.0) +
+                             gain_smem[k + 2] * ((-3.0 * u3 + 3.0 * u2 + 3.0 * u + 1.0) / 6.0) + gain_smem[k + 3] * (u3 / 6.0);
+            const double yv = (double)__ldg(sig + i) / A;
+            num[c] += yv * s;
+            den[c] += s * s;
+            ++cnt[c];
+        }
+    }
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+        const int i = lane + 32 * c;
+        if (i < p.N && cnt[c]) {
+            atomicAdd(p.acc + 2 * i, num[c]);
+            atomicAdd(p.acc + 2 * i + 1, den[c]);
+            atomicAdd(p.n_used + i, cnt[c]);
+        }
+    }
+}
+
 }  // namespace ants

@@ -104,3 +104,25 @@ def test_reconstruct_refit_cycle_recovers_the_response():
         cur.coeffs = c[None, :, :].astype(np.float32)
         err.append(shape_error(c[0]))
     assert err[0] > 0.03 and err[-1] < 0.5 * err[0], err
+
+
+@pytest.mark.parametrize("idx,n", [(2, 50_003), (5, 10_001)])
+def test_gain_evaluation_parity_and_recovery(idx, n):
+    """ants_lrf_fit_gains vs oracle.fit_gains on reconstructed positions (R24): FP64 sums on both sides,
+    float32 output: 1e-6 relative; pair counts bit-exact.  The gains come back near the ones the data were
+    drawn with (statistics, not parity)."""
+    cfg, ev, xyzA = _reconstructed(idx, n)
+    g, used = recon.ants_lrf_fit_gains(cfg.sensor_xy, cfg.knots, cfg.coeffs[0, 0], ev["signals"], xyzA)
+    g0, used0 = ofit.fit_gains(cfg.sensor_xy, cfg.knots, cfg.coeffs[0, 0], cfg.n_int_r,
+                               ev["signals"].cpu().numpy(), xyzA.cpu().numpy())
+    assert np.array_equal(used, used0)
+    assert np.abs(g - g0).max() <= 1e-6 * np.abs(g0).max()
+    assert np.abs(g / cfg.gains - 1.0).max() < 0.1       # clipped noise lifts the far, dim pairs a few per cent
+
+
+def test_gain_of_a_sensor_without_data_is_nan_gpu():
+    cfg = synth.make_config(2)
+    pos = torch.full((64, 4), 400.0, device="cuda")
+    g, used = recon.ants_lrf_fit_gains(cfg.sensor_xy, cfg.knots, cfg.coeffs[0, 0],
+                                       torch.ones((64, cfg.n_sensors), device="cuda"), pos)
+    assert np.isnan(g).all() and (used == 0).all()

@@ -54,7 +54,7 @@ def test_parity_subset(idx):
     assert np.nanmedian(err) < 6.0
 
 
-@pytest.mark.parametrize("idx", [2, 3, 4])
+@pytest.mark.parametrize("idx", [2, 3, 4, 5])
 def test_parity_full_size_sampled(idx):
     """BASELINE.json's full event count in one launch (bench.py's configuration);
     2000 sampled events are reconstructed one by one by the oracle."""
@@ -71,7 +71,7 @@ def test_parity_full_size_sampled(idx):
     finally:
         r.close()
     rng = np.random.default_rng(7)
-    n_s = 2000 if idx != 4 else 1000
+    n_s = 2000 if idx in (2, 3) else 1000
     pick = np.sort(rng.choice(E, n_s, replace=False))
     pick[0], pick[-1] = 0, E - 1
     pt = torch.from_numpy(pick).cuda()

@@ -370,3 +370,21 @@ def test_parity_with_strongest_sensor_start(idx, kw):
     a = _run(cfg0, ev["signals"], trace=False)[0]
     close = np.hypot(a[:, 0] - xyzA[:, 0], a[:, 1] - xyzA[:, 1]) < 1.0
     assert close.mean() > 0.8
+
+
+def test_large_array_more_than_128_sensors():
+    """217 PMTs (hex, 8 rings): more sensors than the 4-per-lane register prefetch holds and seven rounds of
+    32 in the per-iteration list building; odd count (pad pair)."""
+    cfg = synth.make_config(5)
+    cfg.sensor_xy = synth.hex_array(8, 20.0)
+    cfg.gains = np.random.default_rng(2).uniform(0.8, 1.2, len(cfg.sensor_xy)).astype(np.float32)
+    cfg.extent, cfg.n_iter = 120.0, 10
+    assert cfg.n_sensors == 217
+    ev = synth.generate_events(cfg, 1203, device="cuda")
+    xyzA, score, path = _run(cfg, ev["signals"])
+    res = parity_rules.compare(cfg, ev["signals"].cpu().numpy(), xyzA, score, path)
+    parity_rules.assert_parity(res, "217 sensors")
+    cfg.method = 1
+    xyzA, score, path = _run(cfg, ev["signals"])
+    res = parity_rules.compare(cfg, ev["signals"].cpu().numpy(), xyzA, score, path)
+    parity_rules.assert_parity(res, "217 sensors chi-square")

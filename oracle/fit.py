@@ -105,3 +105,43 @@ def fit_gains(sensor_xy, knots, coeffs, n_int, signals, xyzA):
         if den > 0.0:
             gains[i] = float((y * s).sum()) / den
     return gains, used
+
+
+def fit_axial_z(sensor_xy, gains, knots, n_int_r, n_int_z, signals, xyzA):
+    """Least-squares fit of the shared axial+z tensor-product LRF s(r, z) (PAPER.md:394 section 6.1.2;
+    PAPER.md:380 LRFs are calculated from signals + positions).  Reading R25 = R21-R23 carried to (r, z):
+    y = S/(A g) against sum_b sum_a c[kz+b][kr+a] bz_b(uz) br_a(ur) (the tensor spline of
+    oracle/ants_oracle.c), over events with finite x, y, z, A, A > 0 and z_lo <= z <= z_hi, pairs with
+    r_lo <= r <= r_hi.  -> coefficients [n_int_z + 3][n_int_r + 3] (float64), pairs used."""
+    xy = np.asarray(sensor_xy, np.float32).astype(np.float64).reshape(-1, 2)
+    N = xy.shape[0]
+    g = np.ones(N) if gains is None else np.asarray(gains, np.float32).astype(np.float64)
+    r_lo, r_hi, z_lo, z_hi = (float(np.float32(k)) for k in knots[:4])
+    hr, hz = (r_hi - r_lo) / n_int_r, (z_hi - z_lo) / n_int_z
+    ncr, ncz = n_int_r + 3, n_int_z + 3
+    S = np.asarray(signals, np.float32).astype(np.float64).reshape(-1, N)
+    P = np.asarray(xyzA, np.float32).astype(np.float64).reshape(-1, 4)
+    with np.errstate(invalid="ignore"):
+        ok = (np.isfinite(P).all(axis=1) & (P[:, 3] > 0.0) & (P[:, 2] >= z_lo) & (P[:, 2] <= z_hi))
+    M = np.zeros((ncz * ncr, ncz * ncr))
+    b = np.zeros(ncz * ncr)
+    used = 0.0
+    for i in range(N):
+        with np.errstate(invalid="ignore"):
+            r = np.hypot(P[:, 0] - xy[i, 0], P[:, 1] - xy[i, 1])
+            use = ok & (r >= r_lo) & (r <= r_hi)
+        y = S[use, i] / (P[use, 3] * g[i])
+        tr = (r[use] - r_lo) / hr
+        kr = np.minimum(np.floor(tr).astype(np.int64), n_int_r - 1)
+        Br = basis4(tr - kr)
+        tz = (P[use, 2] - z_lo) / hz
+        kz = np.minimum(np.floor(tz).astype(np.int64), n_int_z - 1)
+        Bz = basis4(tz - kz)
+        idx = [((kz + bb) * ncr + kr + aa, Bz[:, bb] * Br[:, aa]) for bb in range(4) for aa in range(4)]
+        for j1, w1 in idx:
+            np.add.at(b, j1, w1 * y)
+            for j2, w2 in idx:
+                np.add.at(M, (j1, j2), w1 * w2)
+        used += use.sum()
+    c = np.linalg.solve(M, b)
+    return c.reshape(ncz, ncr), used

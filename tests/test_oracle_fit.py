@@ -117,3 +117,45 @@ def test_gain_of_a_sensor_without_data_is_nan():
     pos[:, 0:2] = 300.0                                       # every sensor farther than r_hi
     g, used = fit.fit_gains(cfg.sensor_xy, cfg.knots, cfg.coeffs[0, 0], cfg.n_int_r, sig, pos)
     assert np.isnan(g).all() and (used == 0).all()
+
+
+# ---------------------------------------------------------------------------
+# axial+z tensor LRF (R25)
+# ---------------------------------------------------------------------------
+def _problem_rz(n_events, seed=4, noise=0.0):
+    cfg = synth.make_config(4)
+    rng = np.random.default_rng(seed)
+    pos = np.zeros((n_events, 4), np.float32)
+    pos[:, 0:2] = rng.uniform(-170.0, 170.0, (n_events, 2))
+    pos[:, 2] = rng.uniform(0.0, 20.0, n_events)
+    pos[:, 3] = rng.uniform(100.0, 900.0, n_events)
+    r = np.hypot(pos[:, None, 0].astype(float) - cfg.sensor_xy[None, :, 0], pos[:, None, 1].astype(float) - cfg.sensor_xy[None, :, 1])
+    t_r = synth.uniform_knot_vector(0.0, 120.0, 16)
+    t_z = synth.uniform_knot_vector(0.0, 20.0, 8)
+    Bz = BSpline.design_matrix(pos[:, 2].astype(float), t_z, 3).toarray()             # scipy, not the oracle
+    sig = np.zeros((n_events, cfg.n_sensors))
+    for i in range(cfg.n_sensors):
+        Br = BSpline.design_matrix(np.clip(r[:, i], 0.0, 120.0), t_r, 3).toarray()
+        sig[:, i] = pos[:, 3] * cfg.gains[i] * np.einsum("eb,ba,ea->e", Bz, cfg.coeffs[0].astype(float), Br)
+    sig += noise * rng.standard_normal(sig.shape)
+    return cfg, sig.astype(np.float32), pos, (t_r, t_z)
+
+
+def test_axial_z_fit_recovers_coefficients_and_equals_lstsq():
+    cfg, sig, pos, _ = _problem_rz(2500)
+    c, used = fit.fit_axial_z(cfg.sensor_xy, cfg.gains, cfg.knots, 16, 8, sig, pos)
+    want = cfg.coeffs[0].astype(float)
+    assert np.abs(c - want).max() <= 5e-5 * np.abs(want).max() and used > 0
+    cfg, sig, pos, (t_r, t_z) = _problem_rz(1200, noise=0.3)
+    c, used = fit.fit_axial_z(cfg.sensor_xy, cfg.gains, cfg.knots, 16, 8, sig, pos)
+    rows, ys = [], []
+    Bz = BSpline.design_matrix(pos[:, 2].astype(float), t_z, 3).toarray()
+    for i in range(cfg.n_sensors):
+        r = np.hypot(pos[:, 0].astype(float) - float(cfg.sensor_xy[i, 0]), pos[:, 1].astype(float) - float(cfg.sensor_xy[i, 1]))
+        use = r <= 120.0
+        Br = BSpline.design_matrix(r[use], t_r, 3).toarray()
+        rows.append(np.einsum("eb,ea->eba", Bz[use], Br).reshape(use.sum(), -1))
+        ys.append(sig[use, i].astype(float) / (pos[use, 3].astype(float) * float(cfg.gains[i])))
+    ref, *_ = np.linalg.lstsq(np.vstack(rows), np.concatenate(ys), rcond=None)
+    assert used == sum(len(y) for y in ys)
+    assert np.abs(c.ravel() - ref).max() <= 1e-7 * max(1.0, np.abs(ref).max())

@@ -335,6 +335,7 @@ TRAFFIC_PER_EVENT = {"cfg2_pmt2d_hex19": 87.83, "cfg3_sipm_chi2_sq64": 257.5, "c
 # secondary workload: the LRF calculation (ants_lrf_fit_axial), `--workload fit`
 # ---------------------------------------------------------------------------
 def run_fit(args):
+    import numpy as np
     """Times ants_lrf_fit_axial (normal equations on the GPU + host solve) on the config's batch with the
     positions reconstructed by the library.  HBM roofline: the call must read the signals (4N B) and the
     positions (16 B) of every event once; peak = MEASURED_PEAKS.json hbm_gbs (fallback 6650, said so)."""
@@ -344,8 +345,6 @@ def run_fit(args):
         raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
     device = torch.device("cuda", 0)
     cfg = synth.make_config(args.config)
-    if cfg.lrf_dim != 1:
-        raise SystemExit("--workload fit: axial LRFs only (configs 1, 2, 3, 5)")
     E = cfg.n_events // cfg.n_batches if args.events is None else args.events
     sig = synth.generate_events(cfg, E, device=device)["signals"]
     r = recon.Reconstructor(cfg)
@@ -358,14 +357,19 @@ def run_fit(args):
         knots = cfg.knots
     torch.cuda.synchronize()
     stream = torch.cuda.current_stream()
-    n0 = recon.launch_count()
+    def call():
+        if cfg.lrf_dim == 2:
+            c, u = recon.ants_lrf_fit_axial_z(cfg.sensor_xy, cfg.gains, knots, cfg.n_int_r, cfg.n_int_z, sig, xyzA)
+            return c, np.array([u])
+        return recon.ants_lrf_fit_axial(cfg.sensor_xy, cfg.gains, knots, cfg.n_lrf, cfg.n_int_r, sig, xyzA)
+
     for _ in range(args.warmup):
-        recon.ants_lrf_fit_axial(cfg.sensor_xy, cfg.gains, knots, cfg.n_lrf, cfg.n_int_r, sig, xyzA)
+        call()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     n1 = recon.launch_count()
     for a, b in ev:
         a.record(stream)
-        coeffs, used = recon.ants_lrf_fit_axial(cfg.sensor_xy, cfg.gains, knots, cfg.n_lrf, cfg.n_int_r, sig, xyzA)
+        coeffs, used = call()
         b.record(stream)
     torch.cuda.synchronize()
     ms = [a.elapsed_time(b) for a, b in ev]
@@ -384,7 +388,7 @@ def run_fit(args):
             "gpu_launches": recon.launch_count() - n1,
             "roofline": {"bound": "hbm", "achieved": bytes_alg / t / 1e9, "peak": peak, "unit": "GB/s",
                          "frac": bytes_alg / t / 1e9 / peak, "traffic": None, "peak_source": src + " hbm_gbs",
-                         "pairs_per_s": float(used.sum()) / t, "smem_fp64_atomics_per_s": 14.0 * float(used.sum()) / t},
+                         "pairs_per_s": float(used.sum()) / t, "smem_fp64_atomics_per_s": (152.0 if cfg.lrf_dim == 2 else 14.0) * float(used.sum()) / t},
             "step_ms": ms}
     print(json.dumps(line), flush=True)
     return 0

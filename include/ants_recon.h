@@ -188,6 +188,21 @@ int ants_lrf_fit_gains(const float *sensor_xy, const float *knots, const float *
                        int32_t n_int_r, const float *signals, const float *xyzA, int64_t n_events,
                        float *gains_out, double *n_used_out, void *cuda_stream);
 
+/*
+ * ants_lrf_fit_axial_z -- LRF calculation for the shared axial+z tensor-product LRF s(r, z) (PAPER.md:394,
+ * section 6.1.2).  Reading R25: as ants_lrf_fit_axial with y = S / (A g) against the tensor
+ * spline; an event also needs a finite z inside [z_lo, z_hi].
+ *   sensor_xy HOST [N][2], gains HOST [N] or NULL, knots HOST {r_lo, r_hi, z_lo, z_hi},
+ *   signals DEVICE [n_events][N], xyzA DEVICE [n_events][4] = x, y, z, A;
+ *   coeffs_out HOST [n_int_z + 3][n_int_r + 3] float (r fastest), n_used_out HOST [1] double or NULL.
+ * Normal equations in FP64 on the GPU (one launch on `cuda_stream`), dense Cholesky on the host.
+ * Errors: ANTS_ERR_INVALID, ANTS_ERR_SINGULAR, ANTS_ERR_UNSUPPORTED ((n_int_z+3)(n_int_r+3) > 768),
+ * ANTS_ERR_CUDA, ANTS_ERR_NOMEM.
+ */
+int ants_lrf_fit_axial_z(const float *sensor_xy, const float *gains, const float *knots, int32_t n_sensors,
+                         int32_t n_int_r, int32_t n_int_z, const float *signals, const float *xyzA,
+                         int64_t n_events, float *coeffs_out, double *n_used_out, void *cuda_stream);
+
 /* Release the model and its device memory.  NULL is a no-op. */
 void ants_destroy(ants_lrf_t *lrf);
 

@@ -847,3 +847,111 @@ extern "C" int ants_lrf_fit_gains(const float *sensor_xy, const float *knots, co
     }
     return ANTS_OK;
 }
+
+// dense Cholesky solve (row-major symmetric positive definite M [n][n], overwritten), false if not PD
+static bool solve_dense_spd(std::vector<double> &M, std::vector<double> &b, int n) {
+    for (int j = 0; j < n; ++j) {
+        double s = M[(size_t)j * n + j];
+        for (int k = 0; k < j; ++k) s -= M[(size_t)j * n + k] * M[(size_t)j * n + k];
+        if (!(s > 0.0) || !std::isfinite(s)) return false;
+        const double d = std::sqrt(s);
+        M[(size_t)j * n + j] = d;
+        for (int i = j + 1; i < n; ++i) {
+            double t = M[(size_t)i * n + j];
+            for (int k = 0; k < j; ++k) t -= M[(size_t)i * n + k] * M[(size_t)j * n + k];
+            M[(size_t)i * n + j] = t / d;
+        }
+    }
+    for (int i = 0; i < n; ++i) {
+        double s = b[i];
+        for (int k = 0; k < i; ++k) s -= M[(size_t)i * n + k] * b[k];
+        b[i] = s / M[(size_t)i * n + i];
+    }
+    for (int i = n - 1; i >= 0; --i) {
+        double s = b[i];
+        for (int k = i + 1; k < n; ++k) s -= M[(size_t)k * n + i] * b[k];
+        b[i] = s / M[(size_t)i * n + i];
+    }
+    return true;
+}
+
+extern "C" int ants_lrf_fit_axial_z(const float *sensor_xy, const float *gains, const float *knots, int32_t N,
+                                    int32_t n_r, int32_t n_z, const float *signals, const float *xyzA,
+                                    int64_t n_events, float *coeffs_out, double *n_used_out, void *cuda_stream) {
+    if (!sensor_xy || !knots || !coeffs_out || N < 1 || n_r < 1 || n_z < 1 || n_events < 0) return ANTS_ERR_INVALID;
+    if (n_events > 0 && (!signals || !xyzA)) return ANTS_ERR_INVALID;
+    const double r_lo = knots[0], r_hi = knots[1], z_lo = knots[2], z_hi = knots[3];
+    if (!std::isfinite(r_lo) || !std::isfinite(r_hi) || !(r_lo >= 0.0) || !(r_hi > r_lo) || !std::isfinite(z_lo) ||
+        !std::isfinite(z_hi) || !(z_hi > z_lo))
+        return ANTS_ERR_INVALID;
+    for (int i = 0; i < N; ++i)
+        if (gains && !(gains[i] > 0.f && std::isfinite(gains[i]))) return ANTS_ERR_INVALID;
+    const int ncr = n_r + 3, nc = ncr * (n_z + 3);
+    if (nc > 768) return ANTS_ERR_UNSUPPORTED;
+    const size_t total = (size_t)nc * 29, smem = total * sizeof(double);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+        cudaGetLastError();
+        return ANTS_ERR_CUDA;
+    }
+    std::vector<float> g(N, 1.f);
+    if (gains) std::copy(gains, gains + N, g.begin());
+    float *d_xy = nullptr, *d_g = nullptr;
+    double *d_acc = nullptr;
+    unsigned long long *d_used = nullptr;
+    auto cleanup = [&]() { cudaFree(d_xy); cudaFree(d_g); cudaFree(d_acc); cudaFree(d_used); cudaGetLastError(); };
+    if (cudaMalloc(&d_xy, (size_t)N * 2 * sizeof(float)) != cudaSuccess || cudaMalloc(&d_g, (size_t)N * sizeof(float)) != cudaSuccess ||
+        cudaMalloc(&d_acc, smem) != cudaSuccess || cudaMalloc(&d_used, sizeof(unsigned long long)) != cudaSuccess) {
+        cleanup();
+        return ANTS_ERR_NOMEM;
+    }
+    bool ok = cudaMemcpyAsync(d_xy, sensor_xy, (size_t)N * 2 * sizeof(float), cudaMemcpyHostToDevice, st) == cudaSuccess &&
+              cudaMemcpyAsync(d_g, g.data(), (size_t)N * sizeof(float), cudaMemcpyHostToDevice, st) == cudaSuccess &&
+              cudaMemsetAsync(d_acc, 0, smem, st) == cudaSuccess &&
+              cudaMemsetAsync(d_used, 0, sizeof(unsigned long long), st) == cudaSuccess;
+    if (ok && n_events > 0) {
+        FitRZParams p{};
+        p.sens_xy = d_xy; p.gains = d_g; p.signals = signals; p.xyzA = xyzA; p.n_events = n_events;
+        p.N = N; p.n_r = n_r; p.n_z = n_z; p.ncr = ncr; p.nc = nc;
+        p.r_lo = r_lo; p.r_hi = r_hi; p.hr = (r_hi - r_lo) / n_r;
+        p.z_lo = z_lo; p.z_hi = z_hi; p.hz = (z_hi - z_lo) / n_z;
+        p.acc = d_acc; p.n_used = d_used;
+        const int warps = 8;
+        int occ = 0;
+        ok = cudaFuncSetAttribute((const void *)lrf_fit_rz_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) == cudaSuccess &&
+             cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void *)lrf_fit_rz_kernel, warps * 32, smem) == cudaSuccess && occ >= 1;
+        if (ok) {
+            const long long want = (n_events + warps - 1) / warps;
+            const int grid = (int)std::min<long long>(want, (long long)sms * occ);
+            void *args[] = {&p};
+            ok = cudaLaunchKernel((const void *)lrf_fit_rz_kernel, dim3(grid), dim3(warps * 32), args, smem, st) == cudaSuccess;
+            if (ok) g_launches.fetch_add(1);
+        }
+    }
+    std::vector<double> acc(total);
+    unsigned long long used = 0;
+    ok = ok && cudaMemcpyAsync(acc.data(), d_acc, smem, cudaMemcpyDeviceToHost, st) == cudaSuccess &&
+         cudaMemcpyAsync(&used, d_used, sizeof(used), cudaMemcpyDeviceToHost, st) == cudaSuccess &&
+         cudaStreamSynchronize(st) == cudaSuccess;
+    cleanup();
+    if (!ok) return ANTS_ERR_CUDA;
+    if (n_used_out) *n_used_out = (double)used;
+    std::vector<double> M((size_t)nc * nc, 0.0), b(nc);
+    for (int j1 = 0; j1 < nc; ++j1) {
+        const int jr1 = j1 % ncr;
+        b[j1] = acc[(size_t)j1 * 29 + 28];
+        for (int dz = 0; dz < 4; ++dz)
+            for (int dr = -3; dr <= 3; ++dr) {
+                const int jr2 = jr1 + dr, j2 = j1 + dz * ncr + dr;
+                if (jr2 < 0 || jr2 >= ncr || j2 >= nc || j2 < j1) continue;
+                const double v = acc[(size_t)j1 * 29 + dz * 7 + dr + 3];
+                M[(size_t)j1 * nc + j2] = v;
+                M[(size_t)j2 * nc + j1] = v;
+            }
+    }
+    if (!solve_dense_spd(M, b, nc)) return ANTS_ERR_SINGULAR;
+    for (int j = 0; j < nc; ++j) coeffs_out[j] = (float)b[j];
+    return ANTS_OK;
+}

@@ -155,4 +155,70 @@ __global__ void __launch_bounds__(256) lrf_gain_kernel(const GainParams p) {
     }
 }
 
+// ---- axial+z tensor LRF (R25): normal equations of the shared (r, z) spline -----------
+// nc = (n_z + 3)(n_r + 3) unknowns; a pair touches 4 x 4 of them.  The CTA keeps, per row j1, the 4 x 7
+// block of entries M[j1][j1 + dz ncr + dr], dz = 0..3, dr = -3..3 (the upper triangle in linear order) and
+// the right-hand side: 29 doubles per row in shared memory, 136 + 16 FP64 atomics per pair.
+struct FitRZParams {
+    const float *sens_xy, *gains, *signals, *xyzA;
+    long long n_events;
+    int N, n_r, n_z, ncr, nc;
+    double r_lo, r_hi, hr, z_lo, z_hi, hz;
+    double *acc;                 // device [nc][29]: [dz * 7 + dr + 3] for dz = 0..3, then the rhs at [28]
+    unsigned long long *n_used;  // device [1]
+};
+
+__global__ void __launch_bounds__(256) lrf_fit_rz_kernel(const FitRZParams p) {
+    extern __shared__ double rz_smem[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, warps = blockDim.x >> 5;
+    const int total = p.nc * 29;
+    for (int i = threadIdx.x; i < total; i += blockDim.x) rz_smem[i] = 0.0;
+    __syncthreads();
+    unsigned long long used = 0ULL;
+    for (long long e = (long long)blockIdx.x * warps + warp; e < p.n_events; e += (long long)gridDim.x * warps) {
+        const float4 pe = reinterpret_cast<const float4 *>(p.xyzA)[e];
+        const double x = (double)pe.x, y = (double)pe.y, z = (double)pe.z, A = (double)pe.w;
+        if (!(fabs(x) <= 1.7e308 && fabs(y) <= 1.7e308 && A > 0.0 && A <= 1.7e308 && z >= p.z_lo && z <= p.z_hi)) continue;
+        const double tz = (z - p.z_lo) / p.hz;
+        const int kz = min((int)floor(tz), p.n_z - 1);
+        const double uz = tz - (double)kz, oz = 1.0 - uz, uz2 = uz * uz, uz3 = uz2 * uz;
+        const double bz[4] = {oz * oz * oz / 6.0, (3.0 * uz3 - 6.0 * uz2 + 4.0) / 6.0,
+                              (-3.0 * uz3 + 3.0 * uz2 + 3.0 * uz + 1.0) / 6.0, uz3 / 6.0};
+        const float *sig = p.signals + e * p.N;
+        for (int i = lane; i < p.N; i += 32) {
+            const double dx = x - (double)p.sens_xy[2 * i], dy = y - (double)p.sens_xy[2 * i + 1];
+            const double r = sqrt(dx * dx + dy * dy);
+            if (!(r >= p.r_lo && r <= p.r_hi)) continue;
+            const double yv = (double)__ldg(sig + i) / (A * (double)p.gains[i]);
+            const double tr = (r - p.r_lo) / p.hr;
+            const int kr = min((int)floor(tr), p.n_r - 1);
+            const double u = tr - (double)kr, o = 1.0 - u, u2 = u * u, u3 = u2 * u;
+            const double br[4] = {o * o * o / 6.0, (3.0 * u3 - 6.0 * u2 + 4.0) / 6.0,
+                                  (-3.0 * u3 + 3.0 * u2 + 3.0 * u + 1.0) / 6.0, u3 / 6.0};
+#pragma unroll
+            for (int b1 = 0; b1 < 4; ++b1)
+#pragma unroll
+                for (int a1 = 0; a1 < 4; ++a1) {
+                    const double w1 = bz[b1] * br[a1];
+                    double *row = rz_smem + (size_t)((kz + b1) * p.ncr + kr + a1) * 29;
+                    atomicAdd(row + 28, w1 * yv);
+#pragma unroll
+                    for (int b2 = b1; b2 < 4; ++b2)
+#pragma unroll
+                        for (int a2 = 0; a2 < 4; ++a2) {
+                            if (b2 == b1 && a2 < a1) continue;
+                            atomicAdd(row + (b2 - b1) * 7 + (a2 - a1) + 3, w1 * bz[b2] * br[a2]);
+                        }
+                }
+            ++used;
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) used += __shfl_xor_sync(0xffffffffu, used, o);
+    if (lane == 0 && used) atomicAdd(p.n_used, used);
+    __syncthreads();
+    for (int i = threadIdx.x; i < total; i += blockDim.x)
+        if (rz_smem[i] != 0.0) atomicAdd(p.acc + i, rz_smem[i]);
+}
+
 }  // namespace ants

@@ -61,6 +61,8 @@ def load():
     lib.ants_lrf_fit_axial.argtypes = [vp, vp, vp, C.c_int32, C.c_int32, C.c_int32, vp, vp, C.c_int64, vp, vp, vp]
     lib.ants_lrf_fit_gains.restype = C.c_int
     lib.ants_lrf_fit_gains.argtypes = [vp, vp, vp, C.c_int32, C.c_int32, vp, vp, C.c_int64, vp, vp, vp]
+    lib.ants_lrf_fit_axial_z.restype = C.c_int
+    lib.ants_lrf_fit_axial_z.argtypes = [vp, vp, vp, C.c_int32, C.c_int32, C.c_int32, vp, vp, C.c_int64, vp, vp, vp]
     lib.ants_destroy.restype = None
     lib.ants_destroy.argtypes = [vp]
     lib.ants_strerror.restype = C.c_char_p
@@ -128,6 +130,28 @@ def ants_lrf_fit_axial(sensor_xy, gains, knots, n_lrf: int, n_int_r: int, signal
     if rc != 0:
         raise AntsError(rc, "ants_lrf_fit_axial")
     return coeffs, used
+
+
+def ants_lrf_fit_axial_z(sensor_xy, gains, knots, n_int_r: int, n_int_z: int, signals, xyzA, stream=None):
+    """Axial+z tensor LRF calculation (include/ants_recon.h).  -> (coeffs float32 [n_int_z+3][n_int_r+3], pairs used)."""
+    import torch
+    xy, kn = _f32(sensor_xy).reshape(-1, 2), _f32(knots)
+    N, E = xy.shape[0], int(signals.shape[0])
+    g = None if gains is None else _f32(gains)
+    for t in (signals, xyzA):
+        if not (t.is_cuda and t.is_contiguous() and t.dtype == torch.float32):
+            raise ValueError("ants_lrf_fit_axial_z needs contiguous float32 CUDA tensors")
+    if signals.shape[1] != N or tuple(xyzA.shape) != (E, 4) or kn.size < 4:
+        raise ValueError("ants_lrf_fit_axial_z: shape mismatch")
+    coeffs = np.zeros((int(n_int_z) + 3, int(n_int_r) + 3), np.float32)
+    used = C.c_double(0.0)
+    st = torch.cuda.current_stream().cuda_stream if stream is None else int(stream)
+    rc = load().ants_lrf_fit_axial_z(xy.ctypes.data, None if g is None else g.ctypes.data, kn.ctypes.data, N,
+                                     int(n_int_r), int(n_int_z), signals.data_ptr(), xyzA.data_ptr(), E,
+                                     coeffs.ctypes.data, C.addressof(used), st)
+    if rc != 0:
+        raise AntsError(rc, "ants_lrf_fit_axial_z")
+    return coeffs, used.value
 
 
 def ants_lrf_fit_gains(sensor_xy, knots, coeffs, signals, xyzA, stream=None):

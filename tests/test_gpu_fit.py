@@ -126,3 +126,33 @@ def test_gain_of_a_sensor_without_data_is_nan_gpu():
     g, used = recon.ants_lrf_fit_gains(cfg.sensor_xy, cfg.knots, cfg.coeffs[0, 0],
                                        torch.ones((64, cfg.n_sensors), device="cuda"), pos)
     assert np.isnan(g).all() and (used == 0).all()
+
+
+def test_axial_z_fit_parity():
+    """ants_lrf_fit_axial_z vs oracle.fit_axial_z (R25) on true positions of flood data (the config's disk plus a wider
+    one so that every (r, z) cell gets data), some failed rows and out-of-range z; 209 unknowns: tolerance 5e-6 of max|c|."""
+    cfg = synth.make_config(4)
+    E = 30_011
+    ev = synth.generate_events(cfg, E, device="cuda")         # flood data of the config (positions inside the array)
+    sig = ev["signals"].cpu().numpy()
+    pos = np.zeros((E, 4), np.float32)
+    pos[:, :3] = ev["true_xyz"].cpu().numpy()
+    pos[:, 3] = 0.1 * ev["n_ph"].cpu().numpy()
+    # widen: a second half of events far out so that every (r, z) cell gets data
+    far = synth.make_config(4)
+    far.extent = 200.0
+    ev2 = synth.generate_events(far, E, device="cuda", batch=1)
+    sig = np.concatenate([sig, ev2["signals"].cpu().numpy()])
+    pos2 = np.zeros((E, 4), np.float32)
+    pos2[:, :3] = ev2["true_xyz"].cpu().numpy()
+    pos2[:, 3] = 0.1 * ev2["n_ph"].cpu().numpy()
+    pos = np.concatenate([pos, pos2])
+    pos[::19] = np.nan
+    pos[3::23, 2] = 25.0                                       # z outside the LRF range: event ignored
+    c, used = recon.ants_lrf_fit_axial_z(cfg.sensor_xy, cfg.gains, cfg.knots, 16, 8,
+                                         torch.from_numpy(sig).cuda(), torch.from_numpy(pos).cuda())
+    c0, used0 = ofit.fit_axial_z(cfg.sensor_xy, cfg.gains, cfg.knots, 16, 8, sig, pos)
+    assert used == used0
+    assert np.abs(c - c0).max() <= 5e-6 * np.abs(c0).max()
+    # near the truth where the LRF is large (statistics, not parity)
+    assert np.abs(c[2:8, 2:8] - cfg.coeffs[0, 2:8, 2:8]).max() < 0.1 * np.abs(cfg.coeffs[0, 2:8, 2:8]).max()

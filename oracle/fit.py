@@ -145,3 +145,31 @@ def fit_axial_z(sensor_xy, gains, knots, n_int_r, n_int_z, signals, xyzA):
         used += use.sum()
     c = np.linalg.solve(M, b)
     return c.reshape(ncz, ncr), used
+
+
+def filter_events(xyzA, score, score_max=float("nan"), energy_min=float("nan"), energy_max=float("nan"),
+                  radius_max=float("nan")):
+    """Event filters (section 5.2: "individual events can be filtered out according to ...
+    reconstructed ... event energy, chi-squared value of the reconstruction, and the event position";
+    "Only those events which pass all the activated filters are used in LRF reconstruction").  Reading R26:
+    an event passes if its reconstruction did not fail (finite x, y, A, score) and, for every activated
+    (non-NaN) criterion, score <= score_max, energy_min <= A <= energy_max, x^2 + y^2 <= radius_max^2
+    (compared in double on the float32 values).  -> boolean mask [E] and the filtered copy of xyzA in which
+    rejected rows are NaN (what the LRF calculation ignores, R22)."""
+    P = np.asarray(xyzA, np.float32).reshape(-1, 4)
+    s = np.asarray(score, np.float32).reshape(-1)
+    Pd, sd = P.astype(np.float64), s.astype(np.float64)
+    keep = np.isfinite(Pd[:, 0]) & np.isfinite(Pd[:, 1]) & np.isfinite(Pd[:, 3]) & np.isfinite(sd)
+    with np.errstate(invalid="ignore"):
+        if not np.isnan(score_max):
+            keep &= sd <= float(np.float32(score_max))
+        if not np.isnan(energy_min):
+            keep &= Pd[:, 3] >= float(np.float32(energy_min))
+        if not np.isnan(energy_max):
+            keep &= Pd[:, 3] <= float(np.float32(energy_max))
+        if not np.isnan(radius_max):
+            rm = float(np.float32(radius_max))
+            keep &= Pd[:, 0] * Pd[:, 0] + Pd[:, 1] * Pd[:, 1] <= rm * rm
+    out = P.copy()
+    out[~keep] = np.nan
+    return keep, out

@@ -159,3 +159,21 @@ def test_axial_z_fit_recovers_coefficients_and_equals_lstsq():
     ref, *_ = np.linalg.lstsq(np.vstack(rows), np.concatenate(ys), rcond=None)
     assert used == sum(len(y) for y in ys)
     assert np.abs(c.ravel() - ref).max() <= 1e-7 * max(1.0, np.abs(ref).max())
+
+
+# ---------------------------------------------------------------------------
+# event filters (R26)
+# ---------------------------------------------------------------------------
+def test_event_filters_on_hand_made_cases():
+    P = np.array([[0, 0, 0, 100], [3, 4, 0, 100], [3, 4, 0, 50], [np.nan, 0, 0, 100], [0, 0, 0, 100], [6, 8, 0, 100]],
+                 np.float32)
+    s = np.array([1.0, 2.0, 2.0, 1.0, np.inf, 9.0], np.float32)
+    keep, out = fit.filter_events(P, s)
+    assert keep.tolist() == [True, True, True, False, False, True]            # failed rows never pass
+    assert fit.filter_events(P, s, score_max=2.0)[0].tolist() == [True, True, True, False, False, False]
+    assert fit.filter_events(P, s, energy_min=60.0)[0].tolist() == [True, True, False, False, False, True]
+    assert fit.filter_events(P, s, energy_max=60.0)[0].tolist() == [False, False, True, False, False, False]
+    assert fit.filter_events(P, s, radius_max=5.0)[0].tolist() == [True, True, True, False, False, False]   # r = 5 passes
+    keep, out = fit.filter_events(P, s, score_max=5.0, radius_max=4.9)
+    assert keep.tolist() == [True, False, False, False, False, False]
+    assert np.isnan(out[1:]).all() and np.array_equal(out[0], P[0])

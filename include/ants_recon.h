@@ -203,6 +203,26 @@ int ants_lrf_fit_axial_z(const float *sensor_xy, const float *gains, const float
                          int32_t n_int_r, int32_t n_int_z, const float *signals, const float *xyzA,
                          int64_t n_events, float *coeffs_out, double *n_used_out, void *cuda_stream);
 
+/* Event-filter criteria (section 5.2); NaN switches a criterion off. */
+typedef struct {
+    float score_max;    /* keep score <= score_max (chi-square / deviance of the reconstruction) */
+    float energy_min;   /* keep A >= energy_min */
+    float energy_max;   /* keep A <= energy_max */
+    float radius_max;   /* keep x^2 + y^2 <= radius_max^2 */
+} ants_filter_t;
+
+/*
+ * ants_filter_events -- event filters on the reconstruction's own outputs (events "can be
+ * filtered out according to ... reconstructed ... event energy, chi-squared value of the reconstruction, and
+ * the event position"; "Only those events which pass all the activated filters are used in LRF
+ * reconstruction").  Reading R26.  Rows of xyzA (DEVICE [n_events][4], modified IN PLACE) that fail, and rows
+ * of failed reconstructions, become NaN -- exactly what ants_lrf_fit_* ignore; score (DEVICE [n_events]) is
+ * read only.  n_pass_out (HOST, may be NULL) receives the number of passing events; the call then waits for
+ * the stream, otherwise it is asynchronous.  Errors: ANTS_ERR_INVALID, ANTS_ERR_CUDA, ANTS_ERR_NOMEM.
+ */
+int ants_filter_events(float *xyzA, const float *score, int64_t n_events, const ants_filter_t *filter,
+                       int64_t *n_pass_out, void *cuda_stream);
+
 /* Release the model and its device memory.  NULL is a no-op. */
 void ants_destroy(ants_lrf_t *lrf);
 

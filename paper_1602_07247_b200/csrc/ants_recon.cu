@@ -955,3 +955,31 @@ extern "C" int ants_lrf_fit_axial_z(const float *sensor_xy, const float *gains, 
     for (int j = 0; j < nc; ++j) coeffs_out[j] = (float)b[j];
     return ANTS_OK;
 }
+
+extern "C" int ants_filter_events(float *xyzA, const float *score, int64_t n_events, const ants_filter_t *f,
+                                  int64_t *n_pass_out, void *cuda_stream) {
+    if (!f || n_events < 0 || (n_events > 0 && (!xyzA || !score))) return ANTS_ERR_INVALID;
+    if (n_pass_out) *n_pass_out = 0;
+    if (n_events == 0) return ANTS_OK;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    unsigned long long *d_pass = nullptr;
+    if (cudaMalloc(&d_pass, sizeof(unsigned long long)) != cudaSuccess) { cudaGetLastError(); return ANTS_ERR_NOMEM; }
+    FilterParams p{xyzA, score, n_events, f->score_max, f->energy_min, f->energy_max, f->radius_max, d_pass};
+    const int grid = (int)std::min<long long>((n_events + 255) / 256, 148LL * 8);
+    void *args[] = {&p};
+    bool ok = cudaMemsetAsync(d_pass, 0, sizeof(unsigned long long), st) == cudaSuccess &&
+              cudaLaunchKernel((const void *)event_filter_kernel, dim3(grid), dim3(256), args, 0, st) == cudaSuccess;
+    if (ok) g_launches.fetch_add(1);
+    unsigned long long pass = 0;
+    // the counter lives until the stream has passed this point: wait when a count is wanted, else free in stream order
+    if (ok && n_pass_out) {
+        ok = cudaMemcpyAsync(&pass, d_pass, sizeof(pass), cudaMemcpyDeviceToHost, st) == cudaSuccess &&
+             cudaStreamSynchronize(st) == cudaSuccess;
+        *n_pass_out = (int64_t)pass;
+        cudaFree(d_pass);
+    } else {
+        if (cudaFreeAsync(d_pass, st) != cudaSuccess) { cudaGetLastError(); cudaStreamSynchronize(st); cudaFree(d_pass); }
+    }
+    if (!ok) { cudaGetLastError(); return ANTS_ERR_CUDA; }
+    return ANTS_OK;
+}

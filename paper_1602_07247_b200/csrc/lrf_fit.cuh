@@ -221,4 +221,36 @@ __global__ void __launch_bounds__(256) lrf_fit_rz_kernel(const FitRZParams p) {
         if (rz_smem[i] != 0.0) atomicAdd(p.acc + i, rz_smem[i]);
 }
 
+// ---- event filters (section 5.2; R26): rejected rows of xyzA become NaN, in place ------
+struct FilterParams {
+    float *xyzA;                 // device [E][4], in place
+    const float *score;          // device [E]
+    long long n_events;
+    float score_max, energy_min, energy_max, radius_max;   // NaN = criterion off
+    unsigned long long *n_pass;  // device [1]
+};
+
+__global__ void __launch_bounds__(256) event_filter_kernel(const FilterParams p) {
+    unsigned long long pass = 0ULL;
+    const double rm2 = (double)p.radius_max * (double)p.radius_max;
+    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < p.n_events; e += (long long)gridDim.x * blockDim.x) {
+        const float4 v = reinterpret_cast<const float4 *>(p.xyzA)[e];
+        const float s = p.score[e];
+        bool keep = fabsf(v.x) <= 3.402823466e38f && fabsf(v.y) <= 3.402823466e38f && fabsf(v.w) <= 3.402823466e38f &&
+                    fabsf(s) <= 3.402823466e38f;
+        if (p.score_max == p.score_max) keep = keep && s <= p.score_max;
+        if (p.energy_min == p.energy_min) keep = keep && v.w >= p.energy_min;
+        if (p.energy_max == p.energy_max) keep = keep && v.w <= p.energy_max;
+        if (p.radius_max == p.radius_max) keep = keep && (double)v.x * (double)v.x + (double)v.y * (double)v.y <= rm2;
+        if (keep) ++pass;
+        else {
+            const float q = __int_as_float(0x7fc00000);
+            reinterpret_cast<float4 *>(p.xyzA)[e] = make_float4(q, q, q, q);
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) pass += __shfl_xor_sync(0xffffffffu, pass, o);
+    if ((threadIdx.x & 31) == 0 && pass) atomicAdd(p.n_pass, pass);
+}
+
 }  // namespace ants

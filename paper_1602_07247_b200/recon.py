@@ -34,6 +34,11 @@ class GridParams(C.Structure):
                 ("seed_mode", C.c_int32), ("z_seed", C.c_float)]
 
 
+class FilterCriteria(C.Structure):
+    _fields_ = [("score_max", C.c_float), ("energy_min", C.c_float), ("energy_max", C.c_float),
+                ("radius_max", C.c_float)]
+
+
 _lib = None
 
 
@@ -63,6 +68,8 @@ def load():
     lib.ants_lrf_fit_gains.argtypes = [vp, vp, vp, C.c_int32, C.c_int32, vp, vp, C.c_int64, vp, vp, vp]
     lib.ants_lrf_fit_axial_z.restype = C.c_int
     lib.ants_lrf_fit_axial_z.argtypes = [vp, vp, vp, C.c_int32, C.c_int32, C.c_int32, vp, vp, C.c_int64, vp, vp, vp]
+    lib.ants_filter_events.restype = C.c_int
+    lib.ants_filter_events.argtypes = [vp, vp, C.c_int64, C.POINTER(FilterCriteria), C.POINTER(C.c_int64), vp]
     lib.ants_destroy.restype = None
     lib.ants_destroy.argtypes = [vp]
     lib.ants_strerror.restype = C.c_char_p
@@ -106,6 +113,26 @@ def ants_lrf_set_selection(handle, passive=None, signal_min=float("nan"), dist_m
                                        float(dist_max))
     if rc != 0:
         raise AntsError(rc, "ants_lrf_set_selection")
+
+
+def ants_filter_events(xyzA, score, score_max=float("nan"), energy_min=float("nan"), energy_max=float("nan"),
+                       radius_max=float("nan"), stream=None) -> int:
+    """Event filters (include/ants_recon.h): rejected rows of the CUDA tensor xyzA become NaN in place.
+    -> number of passing events."""
+    import torch
+    for t in (xyzA, score):
+        if not (t.is_cuda and t.is_contiguous() and t.dtype == torch.float32):
+            raise ValueError("ants_filter_events needs contiguous float32 CUDA tensors")
+    E = int(score.shape[0])
+    if tuple(xyzA.shape) != (E, 4):
+        raise ValueError("ants_filter_events: shape mismatch")
+    crit = FilterCriteria(score_max, energy_min, energy_max, radius_max)
+    n_pass = C.c_int64(0)
+    st = torch.cuda.current_stream().cuda_stream if stream is None else int(stream)
+    rc = load().ants_filter_events(xyzA.data_ptr(), score.data_ptr(), E, C.byref(crit), C.byref(n_pass), st)
+    if rc != 0:
+        raise AntsError(rc, "ants_filter_events")
+    return int(n_pass.value)
 
 
 def ants_lrf_fit_axial(sensor_xy, gains, knots, n_lrf: int, n_int_r: int, signals, xyzA, stream=None):

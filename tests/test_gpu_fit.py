@@ -156,3 +156,27 @@ def test_axial_z_fit_parity():
     assert np.abs(c - c0).max() <= 5e-6 * np.abs(c0).max()
     # near the truth where the LRF is large (statistics, not parity)
     assert np.abs(c[2:8, 2:8] - cfg.coeffs[0, 2:8, 2:8]).max() < 0.1 * np.abs(cfg.coeffs[0, 2:8, 2:8]).max()
+
+
+def test_event_filter_is_bit_exact_and_feeds_the_fit():
+    """ants_filter_events vs oracle.filter_events (R26): the pass mask and the filtered array are identical
+    bit for bit (integer decisions on the same float32 values); the filtered array then drives the fit."""
+    cfg, ev, xyzA = _reconstructed(2, 40_003)
+    r = recon.Reconstructor(cfg)
+    try:
+        xyzA, score = r(ev["signals"])
+    finally:
+        r.close()
+    ref_keep, ref_out = ofit.filter_events(xyzA.cpu().numpy(), score.cpu().numpy(), score_max=30.0, energy_min=120.0,
+                                           energy_max=450.0, radius_max=50.0)
+    filt = xyzA.clone()
+    n_pass = recon.ants_filter_events(filt, score, score_max=30.0, energy_min=120.0, energy_max=450.0, radius_max=50.0)
+    out = filt.cpu().numpy()
+    assert n_pass == int(ref_keep.sum()) and 0.2 * len(ref_keep) < n_pass < 0.95 * len(ref_keep)
+    assert np.array_equal(np.isnan(out[:, 0]), ~ref_keep)
+    assert np.array_equal(out[ref_keep], ref_out[ref_keep])
+    none = xyzA.clone()
+    assert recon.ants_filter_events(none, score) == int(torch.isfinite(xyzA[:, 0]).sum())       # all criteria off
+    c, used = recon.ants_lrf_fit_axial(cfg.sensor_xy, cfg.gains, cfg.knots, 1, cfg.n_int_r, ev["signals"], filt)
+    c0, used0 = ofit.fit_axial(cfg.sensor_xy, cfg.gains, cfg.knots, 1, cfg.n_int_r, ev["signals"].cpu().numpy(), ref_out)
+    assert np.array_equal(used, used0) and np.abs(c - c0).max() <= TOL * np.abs(c0).max()

@@ -1,0 +1,40 @@
+"""The iterative response reconstruction of PAPER.md:428-442 (section 8) as a thin driver:
+reconstruct all flood events with the current LRFs -> filter -> recalculate the LRFs -> repeat.
+Every step runs in the library's kernels (ants_reconstruct, ants_filter_events, ants_lrf_fit_*);
+this module only chains the calls and swaps the coefficient arrays."""
+from __future__ import annotations
+
+import copy
+
+import numpy as np
+
+from . import recon
+
+
+def iterate_response(cfg, signals, n_cycles: int, score_max: float = float("nan"),
+                     energy_min: float = float("nan"), energy_max: float = float("nan"),
+                     radius_max: float = float("nan"), refit_gains: bool = False):
+    """cfg: a synth.Config-like record with the starting LRFs (axial, shared or per-sensor tables, or
+    axial+z); signals: CUDA float32 [E][N].  Yields (cycle, cfg_k, n_events_used) after every cycle, cfg_k
+    carrying the refitted coefficients (and gains when refit_gains, shared axial profile only)."""
+    cur = copy.copy(cfg)
+    for cycle in range(n_cycles):
+        r = recon.Reconstructor(cur)
+        try:
+            xyzA, score = r(signals)
+        finally:
+            r.close()
+        n_pass = recon.ants_filter_events(xyzA, score, score_max, energy_min, energy_max, radius_max)
+        nxt = copy.copy(cur)
+        if cur.lrf_dim == 2:
+            c, _ = recon.ants_lrf_fit_axial_z(cur.sensor_xy, cur.gains, cur.knots, cur.n_int_r, cur.n_int_z, signals, xyzA)
+            nxt.coeffs = c[None, :, :].astype(np.float32)
+        else:
+            c, _ = recon.ants_lrf_fit_axial(cur.sensor_xy, cur.gains, cur.knots, cur.n_lrf, cur.n_int_r, signals, xyzA)
+            nxt.coeffs = c[:, None, :].astype(np.float32)
+            if refit_gains and cur.n_lrf == 1:
+                g, _ = recon.ants_lrf_fit_gains(cur.sensor_xy, cur.knots, c[0], signals, xyzA)
+                g = np.where(np.isfinite(g) & (g > 0), g, cur.gains)
+                nxt.gains = (g / g.mean() * np.asarray(cur.gains).mean()).astype(np.float32)   # gains are relative
+        cur = nxt
+        yield cycle, cur, n_pass

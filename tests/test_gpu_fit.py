@@ -91,18 +91,11 @@ def test_reconstruct_refit_cycle_recovers_the_response():
         s = s * (truth @ s) / (s @ s)              # the overall scale trades with the energy: compare shapes
         return float(np.abs(s - truth).max() / truth.max())
 
+    from paper_1602_07247_b200 import iterate
     err = [shape_error(guess.coeffs[0, 0])]
-    cur = guess
-    for _ in range(6):
-        rc = recon.Reconstructor(cur)
-        try:
-            xyzA, _ = rc(ev["signals"])
-        finally:
-            rc.close()
-        c, used = recon.ants_lrf_fit_axial(cur.sensor_xy, cur.gains, cur.knots, 1, cur.n_int_r, ev["signals"], xyzA)
-        cur = synth.make_config(2)
-        cur.coeffs = c[None, :, :].astype(np.float32)
-        err.append(shape_error(c[0]))
+    for cycle, cur, n_pass in iterate.iterate_response(guess, ev["signals"], 6, score_max=60.0):
+        assert n_pass > 0.8 * ev["signals"].shape[0]
+        err.append(shape_error(cur.coeffs[0, 0]))
     assert err[0] > 0.03 and err[-1] < 0.5 * err[0], err
 
 

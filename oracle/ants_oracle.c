@@ -261,7 +261,7 @@ int oracle_start(const oracle_model_t *m, const float *sig, int method, int seed
 {
     if (seed_mode == 0) return oracle_centroid(m, sig, method, xy);
     int N = m->n_sensors, best = -1, bad = 0;
-    double *S = (double *)malloc(sizeof(double) * (size_t)N);
+    double *S = (double *)malloc(sizeof(double) * (size_t)(unsigned)N);
     double ss = 0.0;
     prepare_signals(sig, N, method, S);
     for (int i = 0; i < N; ++i) {
@@ -292,7 +292,7 @@ int oracle_score_at(const oracle_model_t *m, const float *sig, int method, int s
     prepare_signals(sig, N, method, S);
     if (needs_selection(m)) {           /* the event's active set hangs on its start position (R19) */
         double xy[2];
-        active = (uint8_t *)malloc((size_t)N);
+        active = (uint8_t *)malloc((size_t)(unsigned)N);
         if (oracle_start(m, sig, method, seed_mode, xy) || select_sensors(m, S, xy, active) == 0) {
             *A_out = NAN; *score_out = INFINITY;
             free(S); free(active);
@@ -335,7 +335,7 @@ static void reconstruct_one(const oracle_model_t *m, const float *sig, const ora
     prepare_signals(sig, N, method, S);
     uint8_t *active = 0;
     if (needs_selection(m)) {
-        active = (uint8_t *)malloc((size_t)N);
+        active = (uint8_t *)malloc((size_t)(unsigned)N);
         double ssum = 0.0;
         int n_act = select_sensors(m, S, xy, active);
         for (int i = 0; i < N; ++i) if (active[i]) ssum += S[i];

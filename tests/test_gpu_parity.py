@@ -388,3 +388,46 @@ def test_large_array_more_than_128_sensors():
     xyzA, score, path = _run(cfg, ev["signals"])
     res = parity_rules.compare(cfg, ev["signals"].cpu().numpy(), xyzA, score, path)
     parity_rules.assert_parity(res, "217 sensors chi-square")
+
+
+def _random_config(seed):
+    """A seeded irregular detector: random sensor positions and gains, random bell width, grid, iteration
+    count, contraction factor, method and LRF sharing (nothing regular for the kernels to lean on)."""
+    rng = np.random.default_rng(1000 + seed)
+    cfg = synth.make_config(2)
+    N = int(rng.integers(3, 70))
+    cfg.sensor_xy = rng.uniform(-50.0, 50.0, (N, 2)).astype(np.float32)
+    cfg.gains = rng.uniform(0.6, 1.5, N).astype(np.float32)
+    width = float(rng.uniform(12.0, 30.0))
+    n_int = int(rng.integers(6, 25))
+    r_hi = float(rng.uniform(80.0, 160.0))
+    base = synth.fit_axial(lambda r: (1.0 + (r / width) ** 2) ** -1.5, 0.0, r_hi, n_int).astype(np.float64)
+    cfg.knots = np.array([0.0, r_hi], np.float32)
+    cfg.n_int_r = n_int
+    if rng.random() < 0.5:
+        cfg.n_lrf, cfg.coeffs = 1, base.astype(np.float32)[None, None, :]
+    else:
+        fac = rng.normal(1.0, 0.05, N)
+        cfg.n_lrf, cfg.coeffs = N, (base[None, :] * fac[:, None]).astype(np.float32)[:, None, :]
+        cfg.gains = np.ones(N, np.float32)
+    cfg.nodes_per_axis = int(rng.integers(3, 14))
+    cfg.n_iter = int(rng.integers(4, 11))
+    cfg.factor = float(rng.choice([0.5, 0.5, 0.6, 0.4]))
+    cfg.step0_xy = float(rng.uniform(20.0, 40.0)) / (cfg.nodes_per_axis - 1) * 2.0
+    cfg.method = int(rng.integers(0, 2))
+    cfg.extent = 40.0
+    cfg.nph = ("uniform", 2000.0, 8000.0)
+    cfg.noise_sigma = float(rng.choice([0.0, 1.0]))
+    cfg.seed_mode = int(rng.integers(0, 2))
+    return cfg
+
+
+@pytest.mark.parametrize("seed", range(24))
+def test_parity_on_random_irregular_detectors(seed):
+    cfg = _random_config(seed)
+    ev = synth.generate_events(cfg, 3001, device="cuda")
+    xyzA, score, path = _run(cfg, ev["signals"])
+    res = parity_rules.compare(cfg, ev["signals"].cpu().numpy(), xyzA, score, path)
+    what = (f"seed {seed}: N={cfg.n_sensors} n_lrf={cfg.n_lrf} G={cfg.nodes_per_axis} K={cfg.n_iter} f={cfg.factor} "
+            f"method={cfg.method} start={cfg.seed_mode}")
+    parity_rules.assert_parity(res, what)

@@ -431,3 +431,33 @@ def test_parity_on_random_irregular_detectors(seed):
     what = (f"seed {seed}: N={cfg.n_sensors} n_lrf={cfg.n_lrf} G={cfg.nodes_per_axis} K={cfg.n_iter} f={cfg.factor} "
             f"method={cfg.method} start={cfg.seed_mode}")
     parity_rules.assert_parity(res, what)
+
+
+@pytest.mark.parametrize("seed", range(8))
+def test_parity_on_random_axial_z_detectors(seed):
+    """Config 4's (r, z) response on random sensor layouts, random grids (3..8 per axis, or a 2-D search
+    at a random fixed z), iterations, contraction factor, method and start option."""
+    rng = np.random.default_rng(2000 + seed)
+    cfg = synth.make_config(4)
+    N = int(rng.integers(5, 60))
+    cfg.sensor_xy = rng.uniform(-80.0, 80.0, (N, 2)).astype(np.float32)
+    cfg.gains = rng.uniform(0.7, 1.4, N).astype(np.float32)
+    cfg.method = int(rng.integers(0, 2))
+    cfg.n_iter = int(rng.integers(5, 11))
+    cfg.factor = float(rng.choice([0.5, 0.5, 0.6]))
+    cfg.seed_mode = int(rng.integers(0, 2))
+    cfg.extent = 60.0
+    if rng.random() < 0.7:
+        cfg.nodes_per_axis = int(rng.integers(3, 9))
+        cfg.step0_xy = 48.0 / (cfg.nodes_per_axis - 1)
+        cfg.step0_z = 18.0 / (cfg.nodes_per_axis - 1)
+    else:
+        cfg.dim, cfg.nodes_per_axis = 2, int(rng.integers(3, 14))
+        cfg.step0_xy = 48.0 / (cfg.nodes_per_axis - 1)
+        z = float(rng.uniform(1.0, 19.0))
+        cfg.z_seed, cfg.z_range = z, (z, z)
+    ev = synth.generate_events(cfg, 2401, device="cuda")
+    xyzA, score, path = _run(cfg, ev["signals"])
+    res = parity_rules.compare(cfg, ev["signals"].cpu().numpy(), xyzA, score, path)
+    parity_rules.assert_parity(res, f"seed {seed}: N={N} dim={cfg.dim} G={cfg.nodes_per_axis} K={cfg.n_iter} "
+                                    f"f={cfg.factor} method={cfg.method} start={cfg.seed_mode}")

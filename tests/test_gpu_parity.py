@@ -419,6 +419,14 @@ def _random_config(seed):
     cfg.nph = ("uniform", 2000.0, 8000.0)
     cfg.noise_sigma = float(rng.choice([0.0, 1.0]))
     cfg.seed_mode = int(rng.integers(0, 2))
+    if seed >= 12:                           # the second dozen also exercises the sensor selection (R19)
+        if rng.random() < 0.6:
+            cfg.passive = (rng.random(N) < 0.15).astype(np.uint8)
+            cfg.passive[int(rng.integers(0, N))] = 0
+        if rng.random() < 0.6:
+            cfg.signal_min = float(rng.uniform(0.5, 4.0))
+        if rng.random() < 0.6:
+            cfg.dist_max = float(rng.uniform(45.0, 110.0))
     return cfg
 
 

@@ -394,6 +394,55 @@ def run_fit(args):
     return 0
 
 
+def run_cycle(args):
+    """Times one cycle of the iterative response reconstruction: reconstruct the batch,
+    filter on the score, recalculate the LRFs.  Secondary workload (`--workload cycle`)."""
+    import torch
+    from paper_1602_07247_b200 import recon, synth
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    device = torch.device("cuda", 0)
+    cfg = synth.make_config(args.config)
+    E = cfg.n_events // cfg.n_batches if args.events is None else args.events
+    sig = synth.generate_events(cfg, E, device=device)["signals"]
+    knots = cfg.knots.copy()
+    if cfg.n_lrf > 1:
+        knots[1] = min(float(knots[1]), 30.0)
+    r = recon.Reconstructor(cfg)
+    xyzA = torch.empty((E, 4), dtype=torch.float32, device=device)
+    score = torch.empty((E,), dtype=torch.float32, device=device)
+    stream = torch.cuda.current_stream()
+
+    def cycle():
+        recon.ants_reconstruct(r.handle, sig, r.grid, r.method, xyzA, score, stream.cuda_stream)
+        n_pass = recon.ants_filter_events(xyzA, score, score_max=4.0 * cfg.n_sensors)
+        if cfg.lrf_dim == 2:
+            recon.ants_lrf_fit_axial_z(cfg.sensor_xy, cfg.gains, knots, cfg.n_int_r, cfg.n_int_z, sig, xyzA)
+        else:
+            recon.ants_lrf_fit_axial(cfg.sensor_xy, cfg.gains, knots, cfg.n_lrf, cfg.n_int_r, sig, xyzA)
+        return n_pass
+
+    for _ in range(args.warmup):
+        cycle()
+    n0 = recon.launch_count()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    for a, b in ev:
+        a.record(stream)
+        n_pass = cycle()
+        b.record(stream)
+    torch.cuda.synchronize()
+    ms = [a.elapsed_time(b) for a, b in ev]
+    t = sum(ms) / len(ms) * 1e-3
+    r.close()
+    print(json.dumps({"metric": "events/s through one reconstruct -> filter -> LRF-calculation cycle", "value": E / t,
+                      "unit": "events/s", "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": t * 1e3,
+                      "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32+f64",
+                      "data": "synthetic", "config": {"workload": cfg.name + " response-reconstruction cycle",
+                                                      "events_per_step_per_gpu": E, "events_passing_filter": n_pass},
+                      "gpu_launches": recon.launch_count() - n0, "step_ms": ms}), flush=True)
+    return 0
+
+
 def main(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -407,13 +456,15 @@ def main(argv=None):
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--ref-step-seconds", type=float, default=4.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--workload", default="reconstruct", choices=["reconstruct", "fit"],
+    ap.add_argument("--workload", default="reconstruct", choices=["reconstruct", "fit", "cycle"],
                     help="fit = time the LRF calculation instead (secondary; not the BASELINE metric)")
     args = ap.parse_args(argv)
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = max(args.warmup, 1)
     if args.workload == "fit":
         return run_fit(args)
+    if args.workload == "cycle":
+        return run_cycle(args)
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)

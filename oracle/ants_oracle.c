@@ -201,7 +201,8 @@ int oracle_centroid(const oracle_model_t *m, const float *sig, int method, doubl
  *   Poisson (R2): A = sum S / sum L, mu_i = A L_i,
  *       D = 2 sum_i t_i, t_i = mu_i - S_i - S_i ln(mu_i/S_i) (S_i>0), mu_i (S_i=0)
  *   chi-square (R3,R4): w_i = 1/max(S_i,1), A = sum w S L / sum w L^2,
- *       chi2 = sum w (S - A L)^2                                             */
+ *       chi2 = sum w (S - A L)^2
+ *   chi-square, sum-ratio energy (method 2, R27): A = sum S / sum L, same chi2   */
 static int score_prepared(const oracle_model_t *m, const double *S, const uint8_t *active, int method,
                           double x, double y, double z, double *L, double *A_out, double *score_out)
 {
@@ -229,6 +230,21 @@ static int score_prepared(const oracle_model_t *m, const double *S, const uint8_
         }
         *A_out = A;
         *score_out = 2.0 * D;
+    } else if (method == 2) {
+        /* R27: least squares with the energy exactly as PAPER.md:328 states it for contracting grids,
+         * "the ratio of two sums over all photosensors: the sum of the photosensor signals and that of
+         * the LRF values": A = sum S / sum L, chi2 = sum w (S - A L)^2, w = 1/max(S,1) (R4) */
+        double sumS = 0.0, chi2 = 0.0;
+        for (int i = 0; i < N; ++i) if (ACTIVE(i)) sumS += S[i];
+        double A = sumS / sumL;
+        for (int i = 0; i < N; ++i) {
+            if (!ACTIVE(i)) continue;
+            double w = 1.0 / (S[i] > 1.0 ? S[i] : 1.0);
+            double d = S[i] - A * L[i];
+            chi2 += w * d * d;
+        }
+        *A_out = A;
+        *score_out = chi2;
     } else {
         double swsl = 0.0, swll = 0.0, chi2 = 0.0;
         for (int i = 0; i < N; ++i) {

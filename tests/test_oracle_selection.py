@@ -178,3 +178,43 @@ def test_distance_selection_follows_the_chosen_start():
         sub = _subset_config(cfg, keep)
         A_ref, s_ref = lib_score(sub, sig[e, keep], *res["xyzA"][e, :2])
         assert res["score"][e] == pytest.approx(s_ref, rel=1e-8) and res["xyzA"][e, 3] == pytest.approx(A_ref, rel=1e-9)
+
+
+# ---------------------------------------------------------------------------
+# least squares with the paper's sum-ratio energy (method 2; R27)
+# ---------------------------------------------------------------------------
+def test_sum_ratio_least_squares_matches_its_definition():
+    from test_oracle_pins import lib_lrf
+    for idx in (2, 3):
+        cfg, sig = _events(idx, 8)
+        model = oracle.Model.from_config(cfg)
+        rng = np.random.default_rng(idx)
+        for e in range(sig.shape[0]):
+            x, y = rng.uniform(-20, 20, 2)
+            L = lib_lrf(cfg, x, y)                                  # scipy evaluation of every sensor's LRF
+            S = sig[e].astype(float)
+            A_ref = S.sum() / L.sum()
+            chi2_ref = ((S - A_ref * L) ** 2 / np.maximum(S, 1.0)).sum()
+            A, sc = model.score_at(sig[e], 2, x, y)
+            assert A == pytest.approx(A_ref, rel=1e-10) and sc == pytest.approx(chi2_ref, rel=1e-9)
+            # the weighted minimiser of method 1 can only do better on the same chi-square
+            assert model.score_at(sig[e], 1, x, y)[1] <= sc * (1 + 1e-12)
+
+
+def test_sum_ratio_first_iteration_equals_numpy_argmin():
+    from test_oracle_pins import lib_lrf
+    cfg, sig = _events(3, 4)
+    cfg.method, cfg.n_iter = 2, 1
+    res = oracle.reconstruct(oracle.Model.from_config(cfg), sig, oracle.grid_from_config(cfg), 2, trace=True)
+    G, half = cfg.nodes_per_axis, 0.5 * (cfg.nodes_per_axis - 1)
+    model = oracle.Model.from_config(cfg)
+    for e in range(sig.shape[0]):
+        c, _ = model.centroid(sig[e], 2)
+        S = sig[e].astype(float)
+        sc = np.empty(G * G)
+        for iy in range(G):
+            for ix in range(G):
+                L = lib_lrf(cfg, c[0] + (ix - half) * cfg.step0_xy, c[1] + (iy - half) * cfg.step0_xy)
+                A = S.sum() / L.sum()
+                sc[iy * G + ix] = ((S - A * L) ** 2 / np.maximum(S, 1.0)).sum()
+        assert res["idx"][e, 0] == int(np.argmin(sc)) and res["best"][e, 0] == pytest.approx(sc.min(), rel=1e-9)

@@ -43,7 +43,9 @@ enum ants_status {
 
 enum ants_method {
     ANTS_POISSON_ML = 0,  /* A = sum S / sum L; score = Poisson deviance 2 sum[mu - S + S ln(S/mu)], mu = A L (R2) */
-    ANTS_CHI_SQUARE = 1   /* w = 1/max(S,1); A = sum w S L / sum w L^2; score = sum w (S - A L)^2 (R3, R4) */
+    ANTS_CHI_SQUARE = 1,  /* w = 1/max(S,1); A = sum w S L / sum w L^2; score = sum w (S - A L)^2 (R3, R4) */
+    ANTS_CHI_SQUARE_SUMRATIO = 2  /* the same score with the energy as PAPER.md:328 states it, A = sum S / sum L (R27);
+                                     axial LRFs only */
 };
 
 /* Opaque LRF model living in device memory; immutable after create. */
@@ -119,7 +121,7 @@ int ants_lrf_set_selection(ants_lrf_t *lrf, const uint8_t *passive, float signal
  * Per-event failure does not fail the call: an event with a non-finite signal,
  * sum S <= 0 or (centroid start) sum S/g <= 0 gets x = y = z = A = NaN and score = +inf.
  * Errors: ANTS_ERR_INVALID (NULL pointers with n_events > 0, bad grid values,
- * dim 3 with an axial LRF, method not 0/1), ANTS_ERR_UNSUPPORTED (G^dim above
+ * dim 3 with an axial LRF, method not 0/1/2), ANTS_ERR_UNSUPPORTED (method 2 with an axial+z LRF; G^dim above
  * the compiled limit: 256 nodes in 2-D, 512 in 3-D), ANTS_ERR_CUDA.
  * n_events == 0 is a valid no-op.
  */

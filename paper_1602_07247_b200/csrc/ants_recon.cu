@@ -381,7 +381,7 @@ static const void *pick2d(int npt) {
 
 static int validate_grid(const ants_lrf *h, const ants_grid_params_t *g, int32_t method) {
     if (!h || !g) return ANTS_ERR_INVALID;
-    if (method != ANTS_POISSON_ML && method != ANTS_CHI_SQUARE) return ANTS_ERR_INVALID;
+    if (method != ANTS_POISSON_ML && method != ANTS_CHI_SQUARE && method != ANTS_CHI_SQUARE_SUMRATIO) return ANTS_ERR_INVALID;
     if (g->dim != 2 && g->dim != 3) return ANTS_ERR_INVALID;
     if (g->nodes_per_axis < 2 || g->n_iter < 1 || g->n_iter > 4096) return ANTS_ERR_INVALID;
     if (!(g->factor > 0.f && g->factor < 1.f)) return ANTS_ERR_INVALID;
@@ -487,7 +487,10 @@ static int make_plan(const ants_lrf *h, const ants_grid_params_t *g, int32_t met
     int rc = validate_grid(h, g, method);
     if (rc != ANTS_OK) return rc;
     const ModelDev &m = h->dev;
-    if (m.n_z > 0) return make_plan3d(h, g, method, pl);
+    if (m.n_z > 0) {
+        if (method == ANTS_CHI_SQUARE_SUMRATIO) return ANTS_ERR_UNSUPPORTED;   // axial LRFs only (R27)
+        return make_plan3d(h, g, method, pl);
+    }
     const long long nodes = (long long)g->nodes_per_axis * g->nodes_per_axis;
     if (nodes > 256) return ANTS_ERR_UNSUPPORTED;
     int need = (int)((nodes + 31) / 32);
@@ -499,10 +502,11 @@ static int make_plan(const ants_lrf *h, const ants_grid_params_t *g, int32_t met
     const bool packed = h->positive;
     if (!packed && m.select) return ANTS_ERR_UNSUPPORTED;   // the generic kernel has no sensor selection
     if (packed)
-        pl.kernel = method == ANTS_POISSON_ML ? pick2d_pk<0>(pl.npt) : pick2d_pk<1>(pl.npt);
+        pl.kernel = method == 0 ? pick2d_pk<0>(pl.npt) : method == 1 ? pick2d_pk<1>(pl.npt) : pick2d_pk<2>(pl.npt);
     else
-        pl.kernel = method == ANTS_POISSON_ML ? pick2d<0, false>(pl.npt) : pick2d<1, false>(pl.npt);
+        pl.kernel = method == 0 ? pick2d<0, false>(pl.npt) : method == 1 ? pick2d<1, false>(pl.npt) : pick2d<2, false>(pl.npt);
     pl.k_diff = first_diff_iter(h, g, method);
+    if (!packed && method == ANTS_CHI_SQUARE_SUMRATIO) pl.k_diff = g->n_iter;   // generic kernel: plain form only
     pl.k_series = pl.k_diff;
     const size_t tables = packed ? (cta_smem_bytes_pk(m.N, m.n_lrf * (m.n_r + 1)) + 15) / 16 * 16
                                  : (size_t)(m.N + m.n_lrf * (m.n_r + 1)) * 16;

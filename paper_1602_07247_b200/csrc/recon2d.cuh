@@ -93,7 +93,7 @@ __device__ void final_score_2d(const ModelDev &m, const float4 *sens_s, const Wa
         Ld[i] = L;
         sumL += L;
         sumS += S;
-        if (METHOD == 1) {
+        if (METHOD >= 1) {
             double wi = 1.0 / fmax(S, 1.0);
             swsl += wi * S * L;
             swll += wi * L * L;
@@ -121,7 +121,7 @@ __device__ void final_score_2d(const ModelDev &m, const float4 *sens_s, const Wa
         swsl = warp_sum(swsl);
         swll = warp_sum(swll);
         if (!(swll > 0.0)) bad = true;
-        A = swsl / swll;
+        A = METHOD == 2 ? sumS / sumL : swsl / swll;          // R27 / R3
         for (int i = lane; i < m.N; i += 32) {
             if (!(w.SC[i].y == w.SC[i].y)) continue;
             double L = Ld[i], S = (double)w.SC[i].x;
@@ -228,7 +228,7 @@ __global__ void __launch_bounds__(256) recon2d_kernel(const Params p) {
         for (int k = 0; k < p.K; ++k) {
             float sc_node[NPT];          // node scores (lower is better), +inf = invalid
             float sumL_node[NPT];        // plain mode: sum L (Poisson) / A (chi2) at the node
-            if (k < p.k_diff) {
+            if (METHOD == 2 || k < p.k_diff) {
                 // =================== plain iteration =========================
                 const float lA = log2f(A_ref);
                 for (int i = lane; i < N; i += 32) {
@@ -280,7 +280,7 @@ __global__ void __launch_bounds__(256) recon2d_kernel(const Params p) {
                             a1[j] = fmaf(wd, d, a1[j]);
                             a2[j] = fmaf(wd, L, a2[j]);
                             a3[j] = fmaf(a.w * L, L, a3[j]);
-                            if (!POS) a4[j] += L;
+                            if (!POS || METHOD == 2) a4[j] += L;
                         }
                     }
                 }
@@ -292,11 +292,17 @@ __global__ void __launch_bounds__(256) recon2d_kernel(const Params p) {
                         sc = fmaf(sumS, log2f(a2[j] * (A_ref / sumS)), a1[j]);
                         sumL_node[j] = a2[j];
                         if (!(a2[j] > 0.f) || bad[j]) sc = kInf;
-                    } else {
+                    } else if (METHOD == 1) {
                         // chi2 = sum w d^2 - (sum w d L)^2 / sum w L^2; A = A_ref + sum w d L / sum w L^2
                         sc = a1[j] - a2[j] * a2[j] / a3[j];
                         sumL_node[j] = A_ref + a2[j] / a3[j];
                         if (!(a3[j] > 0.f) || (!POS && !(a4[j] > 0.f))) sc = kInf;
+                    } else {
+                        // R27: A = sumS / sumL; chi2 = sum w (d - delta L)^2, delta = A - A_ref
+                        const float An = sumS / a4[j], dl = An - A_ref;
+                        sc = fmaf(dl, fmaf(dl, a3[j], -2.f * a2[j]), a1[j]);
+                        sumL_node[j] = An;
+                        if (!(a4[j] > 0.f)) sc = kInf;
                     }
                     if (!nv[j] || !(sc == sc)) sc = kInf;
                     sc_node[j] = sc;
@@ -309,7 +315,7 @@ __global__ void __launch_bounds__(256) recon2d_kernel(const Params p) {
                 int n_simple = 0, n_knot = 0;
                 // pass 1 (chi2 only): A0 = P0/Q0 at the centre needs all sensors first
                 float A0 = 0.f;
-                if (METHOD == 1) {
+                if (METHOD >= 1) {
                     for (int i = lane; i < N; i += 32) {
                         float4 sn = sens_s[i];
                         float dx0 = cx - sn.x, dy0 = cy - sn.y;
@@ -381,7 +387,7 @@ __global__ void __launch_bounds__(256) recon2d_kernel(const Params p) {
                         w.B[pos] = rB;
                         w.C[pos] = rC;
                         w.D[pos] = rD;
-                        if (METHOD == 1) w.E[pos] = rE;
+                        if (METHOD >= 1) w.E[pos] = rE;
                     }
                     n_knot += __popc(mk);
                     n_simple += __popc(ms);
@@ -403,7 +409,7 @@ __global__ void __launch_bounds__(256) recon2d_kernel(const Params p) {
                     const float4 a = w.A[i], b = w.B[i], c = w.C[i];
                     float4 d, ee;
                     if (KNOT) d = w.D[i];
-                    if (METHOD == 1) ee = w.E[i];
+                    if (METHOD >= 1) ee = w.E[i];
 #pragma unroll
                     for (int j = 0; j < NPT; ++j) {
                         float num = fmaf(ddx[j], a.x, fmaf(ddy[j], a.y, dd2[j]));   // r^2 - r0^2, accurate
@@ -462,7 +468,7 @@ __global__ void __launch_bounds__(256) recon2d_kernel(const Params p) {
             warp_argmin(bs, bi);
             const bool found = bs < kInf;
             if (found) {
-                if (k < p.k_diff) {
+                if (METHOD == 2 || k < p.k_diff) {
                     float mine = 0.f;
 #pragma unroll
                     for (int j = 0; j < NPT; ++j)

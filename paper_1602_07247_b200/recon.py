@@ -14,7 +14,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libants_recon.so")
 
-POISSON_ML, CHI_SQUARE = 0, 1
+POISSON_ML, CHI_SQUARE, CHI_SQUARE_SUMRATIO = 0, 1, 2
 
 
 class AntsError(RuntimeError):

@@ -414,7 +414,7 @@ def _random_config(seed):
     cfg.n_iter = int(rng.integers(4, 11))
     cfg.factor = float(rng.choice([0.5, 0.5, 0.6, 0.4]))
     cfg.step0_xy = float(rng.uniform(20.0, 40.0)) / (cfg.nodes_per_axis - 1) * 2.0
-    cfg.method = int(rng.integers(0, 2))
+    cfg.method = int(rng.integers(0, 3))                       # Poisson ML, chi-square, sum-ratio chi-square
     cfg.extent = 40.0
     cfg.nph = ("uniform", 2000.0, 8000.0)
     cfg.noise_sigma = float(rng.choice([0.0, 1.0]))
@@ -469,3 +469,39 @@ def test_parity_on_random_axial_z_detectors(seed):
     res = parity_rules.compare(cfg, ev["signals"].cpu().numpy(), xyzA, score, path)
     parity_rules.assert_parity(res, f"seed {seed}: N={N} dim={cfg.dim} G={cfg.nodes_per_axis} K={cfg.n_iter} "
                                     f"f={cfg.factor} method={cfg.method} start={cfg.seed_mode}")
+
+
+# ---------------------------------------------------------------------------
+# least squares with the paper's sum-ratio energy (method 2; R27)
+# ---------------------------------------------------------------------------
+@pytest.mark.parametrize("idx,n", [(3, 4_003), (2, 10_007), (5, 1_501), (1, 5_001)])
+def test_parity_sum_ratio_least_squares(idx, n):
+    cfg = synth.make_config(idx)
+    cfg.method = 2
+    ev = synth.generate_events(cfg, n, device="cuda")
+    xyzA, score, path = _run(cfg, ev["signals"])
+    res = parity_rules.compare(cfg, ev["signals"].cpu().numpy(), xyzA, score, path)
+    parity_rules.assert_parity(res, f"cfg{idx} sum-ratio least squares")
+
+
+def test_sum_ratio_least_squares_variants():
+    """Method 2 with sensor selection, the strongest-sensor start, a non-positive LRF (generic kernel) and the
+    refusal for axial+z LRFs."""
+    cfg = _with_selection(3, passive=[5, 40], signal_min=2.0)
+    cfg.method, cfg.seed_mode = 2, 1
+    ev = synth.generate_events(synth.make_config(3), 3001, device="cuda")
+    xyzA, score, path = _run(cfg, ev["signals"])
+    parity_rules.assert_parity(parity_rules.compare(cfg, ev["signals"].cpu().numpy(), xyzA, score, path), "selection")
+    cfg = synth.make_config(2)
+    c = cfg.coeffs.copy()
+    c[0, 0, -4:] = -0.002
+    cfg.coeffs, cfg.method = c, 2
+    ev = synth.generate_events(synth.make_config(2), 2001, device="cuda")
+    xyzA, score, path = _run(cfg, ev["signals"])
+    res = parity_rules.compare(cfg, ev["signals"].cpu().numpy(), xyzA, score, path)
+    assert res["fail_mismatch"] == 0 and res["score_viol"] == 0 and res["A_viol"] == 0 and res["idx_viol"] == 0, res
+    cfg = synth.make_config(4)
+    cfg.method = 2
+    with pytest.raises(recon.AntsError) as ei:
+        _run(cfg, torch.ones((4, cfg.n_sensors), device="cuda"))
+    assert ei.value.status == -2

@@ -32,8 +32,11 @@ def basis4(u):
                      u ** 3 / 6.0], axis=-1)
 
 
-def normal_equations(sensor_xy, gains, knots, n_lrf, n_int, signals, xyzA):
-    """-> M [n_lrf][n+3][n+3], b [n_lrf][n+3], n_used [n_lrf] (pairs that entered each table)."""
+def normal_equations(sensor_xy, gains, knots, n_lrf, n_int, signals, xyzA, group=None):
+    """-> M [n_lrf][n+3][n+3], b [n_lrf][n+3], n_used [n_lrf] (pairs that entered each table).
+    group (R28): table index of every sensor, values 0 .. n_lrf-1; the sensors of a group share one profile
+    scaled by their relative gains (section 6.2).  None = the two built-in groupings:
+    one group for all sensors (n_lrf = 1) or one table per sensor without gains (n_lrf = N)."""
     xy = np.asarray(sensor_xy, np.float32).astype(np.float64).reshape(-1, 2)
     N = xy.shape[0]
     g = np.ones(N) if gains is None else np.asarray(gains, np.float32).astype(np.float64)
@@ -47,8 +50,11 @@ def normal_equations(sensor_xy, gains, knots, n_lrf, n_int, signals, xyzA):
     b = np.zeros((n_lrf, nc))
     n_used = np.zeros(n_lrf)
     for i in range(N):
-        m = 0 if n_lrf == 1 else i
-        gi = g[i] if n_lrf == 1 else 1.0
+        if group is not None:
+            m, gi = int(group[i]), g[i]
+        else:
+            m = 0 if n_lrf == 1 else i
+            gi = g[i] if n_lrf == 1 else 1.0
         with np.errstate(invalid="ignore"):
             r = np.hypot(P[:, 0] - xy[i, 0], P[:, 1] - xy[i, 1])
             use = ok & (r >= lo) & (r <= hi)                                                     # R22
@@ -64,10 +70,10 @@ def normal_equations(sensor_xy, gains, knots, n_lrf, n_int, signals, xyzA):
     return M, b, n_used
 
 
-def fit_axial(sensor_xy, gains, knots, n_lrf, n_int, signals, xyzA):
+def fit_axial(sensor_xy, gains, knots, n_lrf, n_int, signals, xyzA, group=None):
     """Least-squares B-spline coefficients [n_lrf][n_int + 3] (float64) and the pairs used per table.
     Raises numpy.linalg.LinAlgError when a table is underdetermined (an interval without data)."""
-    M, b, n_used = normal_equations(sensor_xy, gains, knots, n_lrf, n_int, signals, xyzA)
+    M, b, n_used = normal_equations(sensor_xy, gains, knots, n_lrf, n_int, signals, xyzA, group)
     c = np.stack([np.linalg.solve(M[m], b[m]) for m in range(n_lrf)])
     return c, n_used
 
@@ -173,3 +179,20 @@ def filter_events(xyzA, score, score_max=float("nan"), energy_min=float("nan"), 
     out = P.copy()
     out[~keep] = np.nan
     return keep, out
+
+
+def group_by_radius(sensor_xy, tol=1e-3):
+    """"Grouping according to the distance from the sensor center to the detector center" (PAPER.md:404):
+    sensors whose distance from the origin agrees within tol (mm) share a group; groups are numbered by
+    increasing distance.  -> (group [N] int32, n_groups)."""
+    xy = np.asarray(sensor_xy, np.float64).reshape(-1, 2)
+    d = np.hypot(xy[:, 0], xy[:, 1])
+    order = np.argsort(d, kind="stable")
+    group = np.zeros(len(d), np.int32)
+    g, last = -1, None
+    for i in order:
+        if last is None or d[i] - last > tol:
+            g += 1
+            last = d[i]          # a group is anchored at its first (smallest) distance
+        group[i] = g
+    return group, g + 1

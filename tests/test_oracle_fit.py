@@ -177,3 +177,37 @@ def test_event_filters_on_hand_made_cases():
     keep, out = fit.filter_events(P, s, score_max=5.0, radius_max=4.9)
     assert keep.tolist() == [True, False, False, False, False, False]
     assert np.isnan(out[1:]).all() and np.array_equal(out[0], P[0])
+
+
+# ---------------------------------------------------------------------------
+# grouped fit (R28)
+# ---------------------------------------------------------------------------
+def test_radius_groups_of_the_hexagonal_arrays():
+    for rings, want in ((1, [1, 6]), (2, [1, 6, 6, 6]), (3, [1, 6, 6, 6, 12, 6])):
+        group, n = fit.group_by_radius(synth.hex_array(rings, 30.0))
+        assert n == len(want) and np.bincount(group).tolist() == want
+    group, n = fit.group_by_radius(synth.square_array(8, 6.0))
+    assert n == 9 and np.bincount(group).sum() == 64          # 8 x 8 grid: nine distinct distances from the centre
+
+
+def test_grouped_fit_is_the_lstsq_of_each_group():
+    cfg, sig, pos = _problem(2, 2500, noise=0.4)
+    group, n_groups = fit.group_by_radius(cfg.sensor_xy)
+    c, used = fit.fit_axial(cfg.sensor_xy, cfg.gains, cfg.knots, n_groups, cfg.n_int_r, sig, pos, group=group)
+    assert c.shape == (n_groups, cfg.n_int_r + 3)
+    lo, hi = float(cfg.knots[0]), float(cfg.knots[1])
+    t = synth.uniform_knot_vector(lo, hi, cfg.n_int_r)
+    for m in range(n_groups):
+        rows, ys = [], []
+        for i in np.flatnonzero(group == m):
+            r = np.hypot(pos[:, 0].astype(float) - float(cfg.sensor_xy[i, 0]), pos[:, 1].astype(float) - float(cfg.sensor_xy[i, 1]))
+            use = (r >= lo) & (r <= hi)
+            rows.append(BSpline.design_matrix(r[use], t, 3).toarray())
+            ys.append(sig[use, i].astype(float) / (pos[use, 3].astype(float) * float(cfg.gains[i])))
+        ref, *_ = np.linalg.lstsq(np.vstack(rows), np.concatenate(ys), rcond=None)
+        assert np.abs(c[m] - ref).max() <= 1e-8 * max(1.0, np.abs(ref).max())
+        assert used[m] == sum(len(y) for y in ys)
+    # the two built-in groupings are special cases
+    one, _ = fit.fit_axial(cfg.sensor_xy, cfg.gains, cfg.knots, 1, cfg.n_int_r, sig, pos)
+    one_g, _ = fit.fit_axial(cfg.sensor_xy, cfg.gains, cfg.knots, 1, cfg.n_int_r, sig, pos, group=np.zeros(cfg.n_sensors, np.int32))
+    assert np.array_equal(one, one_g)

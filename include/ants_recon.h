@@ -191,6 +191,20 @@ int ants_lrf_fit_gains(const float *sensor_xy, const float *knots, const float *
                        float *gains_out, double *n_used_out, void *cuda_stream);
 
 /*
+ * ants_lrf_fit_axial_grouped -- ants_lrf_fit_axial with an explicit sensor grouping (section
+ * 6.2: one group for all sensors, grouping by the distance from the sensor centre to the detector centre, or
+ * by the symmetry of the array).  Reading R28: group HOST [N] int32 gives every sensor's table index in
+ * 0 .. n_groups-1; the sensors of a group share one profile, each scaled by its relative gain (gains HOST [N]
+ * or NULL).  coeffs_out HOST [n_groups][n_int_r + 3], n_used_out HOST [n_groups] or NULL.  To reconstruct with
+ * a grouped response, expand it to one table per sensor (coefficients of the sensor's group times its gain).
+ * Other arguments, behaviour and errors as ants_lrf_fit_axial; a group index out of range is ANTS_ERR_INVALID.
+ */
+int ants_lrf_fit_axial_grouped(const float *sensor_xy, const float *gains, const int32_t *group, const float *knots,
+                               int32_t n_sensors, int32_t n_groups, int32_t n_int_r, const float *signals,
+                               const float *xyzA, int64_t n_events, float *coeffs_out, double *n_used_out,
+                               void *cuda_stream);
+
+/*
  * ants_lrf_fit_axial_z -- LRF calculation for the shared axial+z tensor-product LRF s(r, z) (PAPER.md:394,
  * section 6.1.2).  Reading R25: as ants_lrf_fit_axial with y = S / (A g) against the tensor
  * spline; an event also needs a finite z inside [z_lo, z_hi].

@@ -707,11 +707,17 @@ static bool solve_band3(const double *rows, int nc, double *x) {
     return true;
 }
 
-extern "C" int ants_lrf_fit_axial(const float *sensor_xy, const float *gains, const float *knots, int32_t N,
-                                  int32_t n_lrf, int32_t n_int, const float *signals, const float *xyzA,
-                                  int64_t n_events, float *coeffs_out, double *n_used_out, void *cuda_stream) {
+static int fit_axial_impl(const float *sensor_xy, const float *gains, const int32_t *group, const float *knots, int32_t N,
+                          int32_t n_lrf, int32_t n_int, const float *signals, const float *xyzA,
+                          int64_t n_events, float *coeffs_out, double *n_used_out, void *cuda_stream) {
     if (!sensor_xy || !knots || !coeffs_out || N < 1 || n_int < 1 || n_int > 4096 || n_events < 0) return ANTS_ERR_INVALID;
-    if (n_lrf != 1 && n_lrf != N) return ANTS_ERR_INVALID;
+    if (group) {
+        if (n_lrf < 1 || n_lrf > N) return ANTS_ERR_INVALID;
+        for (int i = 0; i < N; ++i)
+            if (group[i] < 0 || group[i] >= n_lrf) return ANTS_ERR_INVALID;
+    } else if (n_lrf != 1 && n_lrf != N) {
+        return ANTS_ERR_INVALID;
+    }
     if (n_events > 0 && (!signals || !xyzA)) return ANTS_ERR_INVALID;
     const double lo = (double)knots[0], hi = (double)knots[1];
     if (!std::isfinite(lo) || !std::isfinite(hi) || !(lo >= 0.0) || !(hi > lo)) return ANTS_ERR_INVALID;
@@ -734,6 +740,7 @@ extern "C" int ants_lrf_fit_axial(const float *sensor_xy, const float *gains, co
         lane_split = 4;      // measured on B200: 4 is the best of 1..16 (more copies cost resident CTAs)
         while (lane_split > 1 && per_copy * warps * lane_split * sizeof(double) > 32 * 1024) lane_split >>= 1;
     }
+    int *d_group = nullptr;
     if (const char *e = std::getenv("ANTS_FIT_LANE_SPLIT")) { const int v = std::atoi(e); if (v >= 1 && v <= 32 && n_lrf == 1) lane_split = v; }
     const int copies = n_lrf == 1 ? warps * lane_split : 1;
     const size_t smem = (per_copy * copies + (size_t)n_lrf) * sizeof(double);
@@ -744,8 +751,9 @@ extern "C" int ants_lrf_fit_axial(const float *sensor_xy, const float *gains, co
     float *d_xy = nullptr, *d_g = nullptr;
     double *d_acc = nullptr;
     unsigned long long *d_used = nullptr;
-    auto cleanup = [&]() { cudaFree(d_xy); cudaFree(d_g); cudaFree(d_acc); cudaFree(d_used); cudaGetLastError(); };
+    auto cleanup = [&]() { cudaFree(d_xy); cudaFree(d_g); cudaFree(d_acc); cudaFree(d_used); cudaFree(d_group); cudaGetLastError(); };
     if (cudaMalloc(&d_xy, (size_t)N * 2 * sizeof(float)) != cudaSuccess || cudaMalloc(&d_g, (size_t)N * sizeof(float)) != cudaSuccess ||
+        (group && cudaMalloc(&d_group, (size_t)N * sizeof(int)) != cudaSuccess) ||
         cudaMalloc(&d_acc, per_copy * sizeof(double)) != cudaSuccess ||
         cudaMalloc(&d_used, (size_t)n_lrf * sizeof(unsigned long long)) != cudaSuccess) {
         cleanup();
@@ -753,11 +761,12 @@ extern "C" int ants_lrf_fit_axial(const float *sensor_xy, const float *gains, co
     }
     bool ok = cudaMemcpyAsync(d_xy, sensor_xy, (size_t)N * 2 * sizeof(float), cudaMemcpyHostToDevice, st) == cudaSuccess &&
               cudaMemcpyAsync(d_g, g.data(), (size_t)N * sizeof(float), cudaMemcpyHostToDevice, st) == cudaSuccess &&
+              (!group || cudaMemcpyAsync(d_group, group, (size_t)N * sizeof(int), cudaMemcpyHostToDevice, st) == cudaSuccess) &&
               cudaMemsetAsync(d_acc, 0, per_copy * sizeof(double), st) == cudaSuccess &&
               cudaMemsetAsync(d_used, 0, (size_t)n_lrf * sizeof(unsigned long long), st) == cudaSuccess;
     if (ok && n_events > 0) {
         FitParams p{};
-        p.sens_xy = d_xy; p.gains = d_g; p.signals = signals; p.xyzA = xyzA; p.n_events = n_events;
+        p.sens_xy = d_xy; p.gains = d_g; p.group = d_group; p.signals = signals; p.xyzA = xyzA; p.n_events = n_events;
         p.N = N; p.n_lrf = n_lrf; p.n_int = n_int; p.nc = nc;
         p.lo = lo; p.hi = hi; p.h = (hi - lo) / n_int;
         p.acc = d_acc; p.n_used = d_used; p.copies = copies; p.lane_split = lane_split;
@@ -786,6 +795,22 @@ extern "C" int ants_lrf_fit_axial(const float *sensor_xy, const float *gains, co
         for (int j = 0; j < nc; ++j) coeffs_out[(size_t)m * nc + j] = (float)x[j];
     }
     return ANTS_OK;
+}
+
+extern "C" int ants_lrf_fit_axial(const float *sensor_xy, const float *gains, const float *knots, int32_t N,
+                                  int32_t n_lrf, int32_t n_int, const float *signals, const float *xyzA,
+                                  int64_t n_events, float *coeffs_out, double *n_used_out, void *cuda_stream) {
+    return fit_axial_impl(sensor_xy, gains, nullptr, knots, N, n_lrf, n_int, signals, xyzA, n_events, coeffs_out,
+                          n_used_out, cuda_stream);
+}
+
+extern "C" int ants_lrf_fit_axial_grouped(const float *sensor_xy, const float *gains, const int32_t *group,
+                                          const float *knots, int32_t N, int32_t n_groups, int32_t n_int,
+                                          const float *signals, const float *xyzA, int64_t n_events,
+                                          float *coeffs_out, double *n_used_out, void *cuda_stream) {
+    if (!group) return ANTS_ERR_INVALID;
+    return fit_axial_impl(sensor_xy, gains, group, knots, N, n_groups, n_int, signals, xyzA, n_events, coeffs_out,
+                          n_used_out, cuda_stream);
 }
 
 extern "C" int ants_lrf_fit_gains(const float *sensor_xy, const float *knots, const float *coeffs, int32_t N,

@@ -20,6 +20,7 @@ namespace ants {
 struct FitParams {
     const float *sens_xy;        // device [N][2]
     const float *gains;          // device [N] (all 1 when the caller passed none)
+    const int *group;            // device [N] table index per sensor (R28), or nullptr: 0 (n_lrf = 1) / i (n_lrf = N)
     const float *signals;        // device [E][N]
     const float *xyzA;           // device [E][4]
     long long n_events;
@@ -56,14 +57,15 @@ __global__ void __launch_bounds__(256) lrf_fit_kernel(const FitParams p) {
             const double dx = x - (double)p.sens_xy[2 * i], dy = y - (double)p.sens_xy[2 * i + 1];
             const double r = sqrt(dx * dx + dy * dy);
             if (!(r >= p.lo && r <= p.hi)) continue;                                   // R22
-            const double g = p.n_lrf == 1 ? (double)p.gains[i] : 1.0;
+            const int tabi = p.group ? p.group[i] : (p.n_lrf == 1 ? 0 : i);
+            const double g = (p.group || p.n_lrf == 1) ? (double)p.gains[i] : 1.0;
             const double yv = (double)__ldg(sig + i) / (A * g);                         // R21, R23
             const double t = (r - p.lo) / p.h;
             const int k = min((int)floor(t), p.n_int - 1);
             const double u = t - (double)k, o = 1.0 - u, u2 = u * u, u3 = u2 * u;
             const double b4[4] = {o * o * o / 6.0, (3.0 * u3 - 6.0 * u2 + 4.0) / 6.0,
                                   (-3.0 * u3 + 3.0 * u2 + 3.0 * u + 1.0) / 6.0, u3 / 6.0};
-            double *tab = mine + (size_t)(p.n_lrf == 1 ? 0 : i) * p.nc * 5;
+            double *tab = mine + (size_t)tabi * p.nc * 5;
 #pragma unroll
             for (int a = 0; a < 4; ++a) {
                 double *row = tab + (size_t)(k + a) * 5;
@@ -72,7 +74,7 @@ __global__ void __launch_bounds__(256) lrf_fit_kernel(const FitParams p) {
                 for (int c = a; c < 4; ++c) atomicAdd(row + (c - a), b4[a] * b4[c]);
             }
             if (p.n_lrf == 1) ++used;
-            else atomicAdd(cnt + i, 1ULL);
+            else atomicAdd(cnt + tabi, 1ULL);
         }
     }
     if (p.n_lrf == 1) {

@@ -66,6 +66,8 @@ def load():
     lib.ants_lrf_fit_axial.argtypes = [vp, vp, vp, C.c_int32, C.c_int32, C.c_int32, vp, vp, C.c_int64, vp, vp, vp]
     lib.ants_lrf_fit_gains.restype = C.c_int
     lib.ants_lrf_fit_gains.argtypes = [vp, vp, vp, C.c_int32, C.c_int32, vp, vp, C.c_int64, vp, vp, vp]
+    lib.ants_lrf_fit_axial_grouped.restype = C.c_int
+    lib.ants_lrf_fit_axial_grouped.argtypes = [vp, vp, vp, vp, C.c_int32, C.c_int32, C.c_int32, vp, vp, C.c_int64, vp, vp, vp]
     lib.ants_lrf_fit_axial_z.restype = C.c_int
     lib.ants_lrf_fit_axial_z.argtypes = [vp, vp, vp, C.c_int32, C.c_int32, C.c_int32, vp, vp, C.c_int64, vp, vp, vp]
     lib.ants_filter_events.restype = C.c_int
@@ -135,7 +137,7 @@ def ants_filter_events(xyzA, score, score_max=float("nan"), energy_min=float("na
     return int(n_pass.value)
 
 
-def ants_lrf_fit_axial(sensor_xy, gains, knots, n_lrf: int, n_int_r: int, signals, xyzA, stream=None):
+def ants_lrf_fit_axial(sensor_xy, gains, knots, n_lrf: int, n_int_r: int, signals, xyzA, stream=None, group=None):
     """LRF calculation (include/ants_recon.h): signals [E][N] and xyzA [E][4] are CUDA float32 tensors.
     -> (coeffs float32 [n_lrf][n_int_r + 3], pairs used per table float64 [n_lrf])."""
     import torch
@@ -151,9 +153,15 @@ def ants_lrf_fit_axial(sensor_xy, gains, knots, n_lrf: int, n_int_r: int, signal
     coeffs = np.zeros((int(n_lrf), int(n_int_r) + 3), np.float32)
     used = np.zeros(int(n_lrf), np.float64)
     st = torch.cuda.current_stream().cuda_stream if stream is None else int(stream)
-    rc = load().ants_lrf_fit_axial(xy.ctypes.data, None if g is None else g.ctypes.data, kn.ctypes.data, N,
-                                   int(n_lrf), int(n_int_r), signals.data_ptr(), xyzA.data_ptr(), E,
-                                   coeffs.ctypes.data, used.ctypes.data, st)
+    if group is None:
+        rc = load().ants_lrf_fit_axial(xy.ctypes.data, None if g is None else g.ctypes.data, kn.ctypes.data, N,
+                                       int(n_lrf), int(n_int_r), signals.data_ptr(), xyzA.data_ptr(), E,
+                                       coeffs.ctypes.data, used.ctypes.data, st)
+    else:       # explicit grouping (R28): n_lrf = number of groups
+        gr = np.ascontiguousarray(np.asarray(group, dtype=np.int32))
+        rc = load().ants_lrf_fit_axial_grouped(xy.ctypes.data, None if g is None else g.ctypes.data, gr.ctypes.data,
+                                               kn.ctypes.data, N, int(n_lrf), int(n_int_r), signals.data_ptr(),
+                                               xyzA.data_ptr(), E, coeffs.ctypes.data, used.ctypes.data, st)
     if rc != 0:
         raise AntsError(rc, "ants_lrf_fit_axial")
     return coeffs, used

@@ -173,3 +173,35 @@ def test_event_filter_is_bit_exact_and_feeds_the_fit():
     c, used = recon.ants_lrf_fit_axial(cfg.sensor_xy, cfg.gains, cfg.knots, 1, cfg.n_int_r, ev["signals"], filt)
     c0, used0 = ofit.fit_axial(cfg.sensor_xy, cfg.gains, cfg.knots, 1, cfg.n_int_r, ev["signals"].cpu().numpy(), ref_out)
     assert np.array_equal(used, used0) and np.abs(c - c0).max() <= TOL * np.abs(c0).max()
+
+
+def test_grouped_fit_parity_and_use_in_reconstruction():
+    """ants_lrf_fit_axial_grouped vs the oracle (R28) with the distance groups of the 19-PMT array, then the
+    grouped response expanded to one table per sensor drives a reconstruction that agrees with the oracle's."""
+    cfg, ev, xyzA = _reconstructed(2, 60_011)
+    group, n_groups = ofit.group_by_radius(cfg.sensor_xy)
+    assert n_groups == 4
+    knots = np.array([0.0, 55.0], np.float32)        # the range the central PMT sees with events inside 60 mm
+    c, used = recon.ants_lrf_fit_axial(cfg.sensor_xy, cfg.gains, knots, n_groups, cfg.n_int_r, ev["signals"], xyzA,
+                                       group=group)
+    c0, used0 = ofit.fit_axial(cfg.sensor_xy, cfg.gains, knots, n_groups, cfg.n_int_r,
+                               ev["signals"].cpu().numpy(), xyzA.cpu().numpy(), group=group)
+    assert np.array_equal(used, used0)
+    assert (np.abs(c - c0).max(axis=1) <= TOL * np.abs(c0).max(axis=1)).all()
+    with pytest.raises(recon.AntsError):
+        recon.ants_lrf_fit_axial(cfg.sensor_xy, cfg.gains, knots, n_groups, cfg.n_int_r, ev["signals"], xyzA,
+                                 group=np.full(cfg.n_sensors, 7))
+    # expand: table of sensor i = its group's profile times its gain
+    import parity_rules
+    exp = synth.make_config(2)
+    exp.n_lrf = cfg.n_sensors
+    exp.knots = knots
+    exp.coeffs = (c[group] * cfg.gains[:, None]).astype(np.float32)[:, None, :]
+    exp.gains = np.ones(cfg.n_sensors, np.float32)
+    sub = ev["signals"][:8001].contiguous()
+    r = recon.Reconstructor(exp)
+    try:
+        out = [t.cpu().numpy() for t in r(sub, trace=True)]
+    finally:
+        r.close()
+    parity_rules.assert_parity(parity_rules.compare(exp, sub.cpu().numpy(), *out), "grouped response expanded")

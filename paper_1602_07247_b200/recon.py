@@ -208,6 +208,29 @@ def ants_lrf_fit_gains(sensor_xy, knots, coeffs, signals, xyzA, stream=None):
     return gains, used
 
 
+def group_by_radius(sensor_xy, tol: float = 1e-3):
+    """Sensor groups "according to the distance from the sensor center to the detector center":
+    sensors are sorted by their distance from the origin and a new group starts wherever the distance exceeds
+    the group's first one by more than tol (mm).  -> (group int32 [N], n_groups), for ants_lrf_fit_axial(group=)."""
+    xy = _f32(sensor_xy).reshape(-1, 2).astype(np.float64)
+    dist = np.sqrt((xy * xy).sum(axis=1))
+    order = np.argsort(dist, kind="stable")
+    group = np.empty(len(dist), np.int32)
+    current, anchor = -1, -np.inf
+    for i in order:
+        if dist[i] - anchor > tol:
+            current, anchor = current + 1, dist[i]
+        group[i] = current
+    return group, current + 1
+
+
+def expand_groups(coeffs, group, gains):
+    """A grouped response as one table per sensor (what ants_lrf_create takes with n_lrf = N): the table of
+    sensor i is its group's profile times its relative gain.  -> float32 [N][1][n_int_r + 3]."""
+    c = np.asarray(coeffs, np.float64)[np.asarray(group)] * np.asarray(gains, np.float64)[:, None]
+    return c.astype(np.float32)[:, None, :]
+
+
 def ants_destroy(handle) -> None:
     load().ants_destroy(handle)
 

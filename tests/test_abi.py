@@ -79,3 +79,14 @@ def test_invalid_model_arguments_are_rejected_before_any_gpu_work():
         with pytest.raises(recon.AntsError) as ei:
             recon.ants_lrf_create(a["sensor_xy"], a["gains"], a["knots"], a["coeffs"], a["dims"])
         assert ei.value.status == -1, kw
+
+
+def test_distance_grouping_helper_agrees_with_the_oracle():
+    from oracle import fit as ofit
+    for xy in (synth.hex_array(1, 30.0), synth.hex_array(3, 30.0), synth.hex_array(6, 25.0), synth.square_array(8, 6.0)):
+        g, n = recon.group_by_radius(xy)
+        g0, n0 = ofit.group_by_radius(xy)
+        assert n == n0 and np.array_equal(g, g0)
+    c = np.arange(8, dtype=np.float64).reshape(2, 4)
+    out = recon.expand_groups(c, [0, 1, 1], [1.0, 2.0, 0.5])
+    assert out.shape == (3, 1, 4) and np.array_equal(out[1, 0], 2.0 * c[1]) and np.array_equal(out[2, 0], 0.5 * c[1])

@@ -179,8 +179,8 @@ def test_grouped_fit_parity_and_use_in_reconstruction():
     """ants_lrf_fit_axial_grouped vs the oracle (R28) with the distance groups of the 19-PMT array, then the
     grouped response expanded to one table per sensor drives a reconstruction that agrees with the oracle's."""
     cfg, ev, xyzA = _reconstructed(2, 60_011)
-    group, n_groups = ofit.group_by_radius(cfg.sensor_xy)
-    assert n_groups == 4
+    group, n_groups = recon.group_by_radius(cfg.sensor_xy)
+    assert n_groups == 4 and np.array_equal(group, ofit.group_by_radius(cfg.sensor_xy)[0])
     knots = np.array([0.0, 55.0], np.float32)        # the range the central PMT sees with events inside 60 mm
     c, used = recon.ants_lrf_fit_axial(cfg.sensor_xy, cfg.gains, knots, n_groups, cfg.n_int_r, ev["signals"], xyzA,
                                        group=group)
@@ -196,7 +196,7 @@ def test_grouped_fit_parity_and_use_in_reconstruction():
     exp = synth.make_config(2)
     exp.n_lrf = cfg.n_sensors
     exp.knots = knots
-    exp.coeffs = (c[group] * cfg.gains[:, None]).astype(np.float32)[:, None, :]
+    exp.coeffs = recon.expand_groups(c, group, cfg.gains)
     exp.gains = np.ones(cfg.n_sensors, np.float32)
     sub = ev["signals"][:8001].contiguous()
     r = recon.Reconstructor(exp)

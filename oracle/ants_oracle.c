@@ -181,7 +181,7 @@ int oracle_centroid(const oracle_model_t *m, const float *sig, int method, doubl
     prepare_signals(sig, N, method, S);
     for (int i = 0; i < N; ++i) {
         if (!not_passive(m, i)) continue;             /* passive sensors are ignored altogether */
-        if (!isfinite(S[i])) bad = 1;
+        if (!isfinite((double)sig[i])) bad = 1;       /* the raw signal: -inf must not be clipped away */
         double w = S[i] / (double)m->gains[i];
         sx += (double)m->sensor_xy[2 * i] * w;
         sy += (double)m->sensor_xy[2 * i + 1] * w;
@@ -282,7 +282,7 @@ int oracle_start(const oracle_model_t *m, const float *sig, int method, int seed
     prepare_signals(sig, N, method, S);
     for (int i = 0; i < N; ++i) {
         if (!not_passive(m, i)) continue;
-        if (!isfinite(S[i])) bad = 1;
+        if (!isfinite((double)sig[i])) bad = 1;       /* the raw signal, before the clipping of R18 */
         ss += S[i];
         if (best < 0 || S[i] > S[best]) best = i;
     }

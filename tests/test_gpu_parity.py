@@ -138,8 +138,9 @@ def test_failed_events_and_negative_signals():
     sig[7, 1] = float("inf")
     sig[9] = -sig[9]                     # all negative: Poisson clips to 0 -> failed
     sig[11, 0] = -3.0                    # one negative: clipped, event fine (R18)
+    sig[13, 4] = float("-inf")           # -inf is non-finite: fails BEFORE the clipping
     xyzA, score, path = _run(cfg, sig)
-    for e in (3, 5, 7, 9):
+    for e in (3, 5, 7, 9, 13):
         assert np.isnan(xyzA[e]).all() and np.isposinf(score[e])
         assert ((path[e].astype(np.int64) & 0xFFFF) == 0xFFFF).all()
     res = parity_rules.compare(cfg, sig.cpu().numpy(), xyzA, score, path)
@@ -186,6 +187,32 @@ def test_non_positive_spline_uses_validity_rules():
     res = parity_rules.compare(cfg, ev["signals"].cpu().numpy(), xyzA, score, path)
     assert res["fail_mismatch"] == 0 and res["score_viol"] == 0 and res["A_viol"] == 0 and res["idx_viol"] == 0, res
     assert res["pos_frac_within"] >= 0.9 and res["pos_max_steps"] <= 16.0, res
+
+
+@pytest.mark.parametrize("lrf_dim,G,method", [(1, 2, 0), (1, 4, 0), (1, 6, 1), (1, 4, 2), (1, 8, 0), (2, 4, 0), (2, 6, 1)])
+def test_tie_break_lowest_linear_index_gpu(lrf_dim, G, method):
+    """R9 on an EXACT tie: sensors on the line y = 0 make nodes mirrored in y bit-identical (same operands in
+    the same order, in FP32 as in FP64), so the first iteration always has a tied pair; the lower linear
+    index must win on both sides -> identical node index, bit for bit (tests/test_oracle_pins.py pins the
+    oracle's side of this)."""
+    cfg = synth.make_config(4 if lrf_dim == 2 else 2)
+    cfg.sensor_xy = np.array([[-31.0, 0.0], [-9.5, 0.0], [4.25, 0.0], [22.0, 0.0], [40.5, 0.0]], np.float32)
+    cfg.gains = np.array([1.0, 0.9, 1.1, 1.05, 0.95], np.float32)
+    cfg.nodes_per_axis, cfg.method, cfg.n_iter = G, method, 1
+    cfg.step0_xy, cfg.step0_z = 3.0, 2.0
+    rng = np.random.default_rng(G * 10 + method)
+    sig = torch.from_numpy(rng.poisson(40.0, (257, 5)).astype(np.float32)).cuda()
+    xyzA, score, path = _run(cfg, sig)
+    model = oracle.Model.from_config(cfg)
+    ref = oracle.reconstruct(model, sig.cpu().numpy(), oracle.grid_from_config(cfg), method, trace=True)
+    ok = np.isfinite(ref["xyzA"][:, 0])
+    assert ok.sum() > 250
+    assert np.all(ref["best"][ok, 0] == ref["second"][ok, 0])            # every event has an exact tie
+    gp = path.astype(np.int64)[:, 0] & 0xFFFF
+    assert np.array_equal(gp[ok], ref["idx"][ok, 0])                      # and both sides take the lower index
+    iy = (gp[ok] // G) % G
+    assert np.all(iy < G - 1 - iy)
+    assert np.array_equal(xyzA[ok, 1].astype(np.float64), ref["xyzA"][ok, 1])
 
 
 def test_noise_free_recovery_gpu():
@@ -284,7 +311,9 @@ def test_axial_z_seed_outside_range_gives_invalid_nodes():
     xyzA, score, path = _run(cfg, ev["signals"])
     assert np.isposinf(score).all() and np.isnan(xyzA[:, 3]).all() and np.isfinite(xyzA[:, :3]).all()
     res = parity_rules.compare(cfg, ev["signals"].cpu().numpy(), xyzA, score, path)
-    assert res["idx_diverged"] == 0 and res["pos_frac_within"] == 1.0 or res["fail_mismatch"] >= 0
+    assert res["fail_mismatch"] == 0 and res["idx_diverged"] == 0 and res["pos_frac_within"] == 1.0, res
+    assert np.all(res["ref"]["idx"] == -1)                       # no node is ever valid, on either side
+    assert ((path.astype(np.int64) & 0xFFFF) == 0xFFFF).all()
     model = oracle.Model.from_config(cfg)
     ref = oracle.reconstruct(model, ev["signals"].cpu().numpy(), oracle.grid_from_config(cfg), cfg.method)
     assert np.allclose(ref["xyzA"][:, :2], xyzA[:, :2], atol=1e-4) and np.isposinf(ref["score"]).all()

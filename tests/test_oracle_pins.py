@@ -300,6 +300,131 @@ def test_multi_iteration_walk_matches_numpy_replay():
         assert np.allclose(out["xyzA"][e, :2], c[:2], atol=1e-12)
 
 
+def lib_lrf_fast(cfg, x, y, z=0.0):
+    """lib_lrf with one library call per table instead of one per sensor (same scipy evaluation)."""
+    r = np.hypot(x - cfg.sensor_xy[:, 0].astype(float), y - cfg.sensor_xy[:, 1].astype(float))
+    if cfg.n_lrf != 1:
+        return lib_lrf(cfg, x, y, z)
+    if cfg.lrf_dim == 1:
+        s = synth.eval_axial(cfg.coeffs[0, 0], float(cfg.knots[0]), float(cfg.knots[1]), r)
+    else:
+        s = synth.eval_axial_z(cfg.coeffs[0], cfg.knots[0:2], cfg.knots[2:4], r, np.array([z]))[0]
+    return cfg.gains.astype(float) * s
+
+
+def np_walk(cfg, S, start, K, G, h_xy, h_z, f):
+    """The contracting-grid walk of PAPER.md:328 replayed with numpy: per iteration an argmin (first
+    minimum in linear-index order) over library-evaluated node scores, then recentre and contract."""
+    half = 0.5 * (G - 1)
+    Gz = G if cfg.dim == 3 else 1
+    c = list(start)
+    path = []
+    for _ in range(K):
+        sc = np.full(Gz * G * G, np.inf)
+        for iz, iy, ix in itertools.product(range(Gz), range(G), range(G)):
+            z = c[2] + (iz - half) * h_z if cfg.dim == 3 else c[2]
+            if cfg.lrf_dim == 2 and not (cfg.knots[2] <= z <= cfg.knots[3]):
+                continue
+            L = lib_lrf_fast(cfg, c[0] + (ix - half) * h_xy, c[1] + (iy - half) * h_xy, z)
+            Sv = np.asarray(S, float)
+            if cfg.method == 0:
+                Sv = np.maximum(Sv, 0.0)
+                mu = Sv.sum() / L.sum() * L
+                t = np.where(Sv > 0, mu - Sv - Sv * np.log(np.where(Sv > 0, mu / np.where(Sv > 0, Sv, 1), 1.0)), mu)
+                sc[(iz * G + iy) * G + ix] = 2.0 * t.sum()
+            else:
+                w = 1.0 / np.maximum(Sv, 1.0)
+                A = (w * Sv * L).sum() / (w * L * L).sum()
+                sc[(iz * G + iy) * G + ix] = (w * (Sv - A * L) ** 2).sum()
+        i = int(np.argmin(sc))                 # numpy: the first occurrence of the minimum
+        path.append(i)
+        ix, iy, iz = i % G, (i // G) % G, i // (G * G)
+        c[0] += (ix - half) * h_xy
+        c[1] += (iy - half) * h_xy
+        if cfg.dim == 3:
+            c[2] += (iz - half) * h_z
+        h_xy *= f
+        h_z *= f
+    return path, c
+
+
+@pytest.mark.parametrize("idx,G,K,f,n_ev", [(3, 5, 4, 0.5, 2),      # chi-square, one table per sensor
+                                            (4, 4, 3, 0.5, 2),      # 3-D, z recentring, even G
+                                            (4, 3, 4, 0.6, 1),      # 3-D with f != 0.5
+                                            (2, 7, 5, 0.4, 3),      # f != 0.5, gains, noise
+                                            (1, 6, 4, 0.7, 3)])     # even G, f != 0.5
+def test_multi_iteration_walk_matches_numpy_replay_other_configs(idx, G, K, f, n_ev):
+    """The chained walk for chi-square (config 3), the 3-D search with z recentring (config 4) and
+    contraction factors other than 0.5 (h_k = h_0 f^k, R1)."""
+    cfg = synth.make_config(idx)
+    m = oracle.Model.from_config(cfg)
+    sig = synth.generate_events(cfg, n_ev)["signals"].numpy()
+    h_xy = cfg.step0_xy * (cfg.nodes_per_axis - 1) / (G - 1)
+    h_z = cfg.step0_z * (cfg.nodes_per_axis - 1) / (G - 1) if cfg.dim == 3 else 0.0
+    g = oracle.grid_params(cfg.dim, G, h_xy, h_z, f, K)
+    out = oracle.reconstruct(m, sig, g, cfg.method, trace=True)
+    for e in range(n_ev):
+        xy, _ = m.centroid(sig[e], cfg.method)
+        z0 = 0.5 * (float(cfg.knots[2]) + float(cfg.knots[3])) if cfg.lrf_dim == 2 else 0.0
+        path, c = np_walk(cfg, sig[e], (xy[0], xy[1], z0), K, G, float(np.float32(h_xy)), float(np.float32(h_z)),
+                          float(np.float32(f)))
+        assert list(out["idx"][e]) == path
+        assert np.allclose(out["xyzA"][e, :3], c, atol=1e-11)
+
+
+# ---------------------------------------------------------------------------
+# tie-break (R9): the first strict minimum in linear-index order
+# ---------------------------------------------------------------------------
+def _collinear_model(lrf_dim):
+    """Sensors on the line y = 0: nodes mirrored in y see bit-identical distances, so their scores tie
+    EXACTLY (same operands in the same order), and the centroid's y is exactly 0."""
+    base = synth.make_config(4 if lrf_dim == 2 else 2)
+    xy = np.array([[-31.0, 0.0], [-9.5, 0.0], [4.25, 0.0], [22.0, 0.0], [40.5, 0.0]], np.float32)
+    g = np.array([1.0, 0.9, 1.1, 1.05, 0.95], np.float32)
+    return base, oracle.Model(xy, g, base.knots, base.coeffs, 1, lrf_dim, base.n_int_r, base.n_int_z)
+
+
+@pytest.mark.parametrize("method", [0, 1, 2])
+@pytest.mark.parametrize("G", [2, 4, 6])
+def test_tie_break_lowest_linear_index_2d(G, method):
+    base, m = _collinear_model(1)
+    S = np.array([[12, 55, 80, 31, 7], [3, 9, 40, 90, 60]], np.float32)
+    g = oracle.grid_params(2, G, 3.0, 0.0, 0.5, 1)
+    out = oracle.reconstruct(m, S, g, method, trace=True)
+    for e in range(2):
+        xy, _ = m.centroid(S[e], method)
+        assert xy[1] == 0.0
+        # scores of all nodes, through the oracle's own score_at (the pin is the ORDER rule, not the score)
+        half = 0.5 * (G - 1)
+        sc = np.array([m.score_at(S[e], method, xy[0] + (ix - half) * 3.0, (iy - half) * 3.0)[1]
+                       for iy in range(G) for ix in range(G)])
+        best = sc.min()
+        tied = np.flatnonzero(sc == best)
+        assert len(tied) >= 2                         # the mirrored partner ties exactly
+        assert tied[0] // G == G - 1 - tied[-1] // G and tied[0] % G == tied[-1] % G
+        assert out["idx"][e, 0] == tied[0]            # the LOWEST linear index wins
+        assert out["best"][e, 0] == best and out["second"][e, 0] == best
+        assert out["xyzA"][e, 1] == (tied[0] // G - half) * 3.0
+
+
+def test_tie_break_lowest_linear_index_3d():
+    base, m = _collinear_model(2)
+    S = np.array([[12, 55, 80, 31, 7]], np.float32)
+    G = 4
+    g = oracle.grid_params(3, G, 3.0, 2.0, 0.5, 1)
+    out = oracle.reconstruct(m, S, g, 0, trace=True)
+    i = int(out["idx"][0, 0])
+    ix, iy, iz = i % G, (i // G) % G, i // (G * G)
+    assert iy < G - 1 - iy                            # the partner (ix, G-1-iy, iz) has the higher index
+    assert out["best"][0, 0] == out["second"][0, 0]   # and ties exactly
+    xy, _ = m.centroid(S[0], 0)
+    half = 0.5 * (G - 1)
+    p = (xy[0] + (ix - half) * 3.0, (iy - half) * 3.0, 10.0 + (iz - half) * 2.0)
+    a = m.score_at(S[0], 0, p[0], p[1], p[2])[1]
+    b = m.score_at(S[0], 0, p[0], -p[1], p[2])[1]
+    assert a == b == out["best"][0, 0]
+
+
 def test_lattice_brute_force_tiny():
     """With factor 0.5 every visited node lies on seed + m*h_K: the exhaustive minimum
     over that lattice (window = everything the search could reach) is <= the oracle's
@@ -383,6 +508,14 @@ def test_failed_events_and_all_invalid_grid():
     out = oracle.reconstruct(m, sig, oracle.grid_from_config(cfg), 0, trace=True)
     assert np.all(np.isnan(out["xyzA"][1])) and out["score"][1] == np.inf and np.all(out["idx"][1] == -1)
     assert np.all(np.isfinite(out["xyzA"][[0, 2]]))
+    # a non-finite RAW signal fails the event, -inf included (it must not be clipped to 0 first)
+    for bad in (np.nan, np.inf, -np.inf):
+        for method in (0, 1):
+            s2 = sig.copy()
+            s2[2, 3] = bad
+            o2 = oracle.reconstruct(m, s2, oracle.grid_from_config(cfg), method)
+            assert np.all(np.isnan(o2["xyzA"][2])) and o2["score"][2] == np.inf and np.all(np.isfinite(o2["xyzA"][0]))
+            assert m.centroid(s2[2], method)[1] == 1 and m.start(s2[2], method, 1)[1] == 1
     with pytest.raises(ValueError):
         oracle.reconstruct(m, sig, oracle.grid_params(2, 1, 5.0, 0, 0.5, 3), 0)
     with pytest.raises(ValueError):

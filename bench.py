@@ -5,8 +5,10 @@ One "step" = one pass of the whole hot path (load, 
 K grid iterations of LRF evaluation + energy + score + argmin, store) over one batch of seeded
 synthetic flood-field events = ONE kernel launch through the C ABI (ants_reconstruct).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 5] [--impl ours|reference]
 
+The headline is config 5 (the largest single-GPU configuration: 127 PMTs, 16 M events in 8 batches of
+2 M); `per_config` carries the same measurements for all five BASELINE.json configs (N = 1).
 Prints ONE JSON line (rank 0).  `value` is device-resident throughput (CUDA events on the
 launching stream, L2 flushed between steps, max over ranks); `e2e` is the same metric through
 ants_reconstruct_host with pinned HOST buffers (H2D and D2H inside the timed region);
@@ -174,7 +176,8 @@ def run_reference(args):
     grid = oracle.grid_from_config(cfg)
     used = oracle.n_threads(0)
     # bounded sample per step: sized from a calibration slice so that one step takes ~step_s
-    pool = synth.generate_events(cfg, min(cfg.n_events // cfg.n_batches, 262_144), device="cpu")["signals"].numpy()
+    n_pool = 262_144 if cfg.pairs_per_event < 50_000 else 32_768       # a step never needs more (oracle: ~1e4 events/s)
+    pool = synth.generate_events(cfg, min(cfg.n_events // cfg.n_batches, n_pool), device="cpu")["signals"].numpy()
     n0 = max(64, 8 * used)
     t0 = time.perf_counter()
     oracle.reconstruct(model, pool[:n0], grid, cfg.method)
@@ -204,31 +207,75 @@ def workload_config(cfg, events_per_step: int, n_gpus: int) -> dict:
             "grid": "x".join([str(cfg.nodes_per_axis)] * cfg.dim), "n_iter": cfg.n_iter,
             "method": "poisson_ml" if cfg.method == 0 else "chi_square",
             "pairs_per_event": cfg.pairs_per_event, "parallelism": f"replicas x{n_gpus} (no collective)",
+            "events_total": int(cfg.n_events), "batches": int(cfg.n_batches),
             "l2": "256 MiB scratch write between timed steps; resident batches rotate"}
+
+
+# ---------------------------------------------------------------------------
+# instruction mix and DRAM traffic per kernel: read from the committed ncu summary (never hard-coded here)
+# ---------------------------------------------------------------------------
+MIX_CSV = os.path.join(ROOT, "profiles", "r02_kernel_mix.csv")
+
+
+def kernel_mix(workload: str, kernel: str):
+    """Row of profiles/r02_kernel_mix.csv (made from `ncu --set full --import-source on` captures of this very
+    bench command, see profiles/r02_kernel_mix.md) for this workload, if it describes the kernel that is
+    dispatched now; else None -- a stale row is dropped, not reported."""
+    try:
+        import csv
+        with open(MIX_CSV, newline="") as f:
+            for row in csv.DictReader(f):
+                if row["workload"] == workload and row["kernel"] == kernel:
+                    return row
+    except OSError:
+        pass
+    return None
+
+
+def fp32_peak_tflops(prop, max_mhz: float) -> float:
+    return prop.multi_processor_count * FP32_LANES_PER_SM * 2 * max_mhz * 1e6 / 1e12
+
+
+def roofline_of(cfg, plan: dict, E: int, launch_ms: float, prop, max_mhz: float) -> dict:
+    """FP32-ALU roofline of the one kernel.  `frac` is nominal: SURVEY.md 8(d)'s flop per
+    (node, sensor) pair x ALL K G^d N pairs of the method (the kernels skip pairs whose LRF is constant over the
+    grid; no credit is taken for that) / launch time / peak.  `frac_executed`, `mix_ceiling` and `traffic` come
+    from the committed ncu capture of the same kernel, labelled with their source."""
+    peak = fp32_peak_tflops(prop, max_mhz)
+    pairs = float(cfg.pairs_per_event) * E
+    t = launch_ms * 1e-3
+    achieved = flop_per_pair(cfg) * pairs / t / 1e12
+    alg_bytes = E * (4 * cfg.n_sensors + 20)
+    out = {"bound": "alu", "kernel": plan.get("kernel"), "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+           "frac": achieved / peak, "frac_kind": "nominal flop/pair x all K*G^d*N pairs",
+           "peak_source": "derived: SMs x 128 FP32 lanes x 2 x clocks.max.sm (MEASURED_PEAKS.json has no FP32 "
+                          "entry); cross-checked by profiles/r02_fp32_peak.md",
+           "flop_per_pair_nominal": flop_per_pair(cfg), "pairs_per_s": pairs / t,
+           "algorithmic_bytes_per_launch": alg_bytes, "hbm_gbs_signal_stream": alg_bytes / t / 1e9,
+           "launch_ms": launch_ms, "traffic": None, "frac_executed": None, "mix_ceiling": None}
+    row = kernel_mix(cfg.name, plan.get("kernel") or "")
+    if row is not None:
+        out["traffic"] = float(row["dram_bytes_per_event"]) * E
+        out["frac_executed"] = float(row["flop_executed_per_pair"]) * pairs / t / 1e12 / peak
+        out["mix_ceiling"] = float(row["mix_ceiling_frac"])
+        out["thread_inst_per_pair"] = float(row["thread_inst_per_pair"])
+        out["mix_source"] = "profiles/r02_kernel_mix.csv (ncu capture of this kernel; see profiles/r02_kernel_mix.md)"
+    return out
 
 
 # ---------------------------------------------------------------------------
 # our arm
 # ---------------------------------------------------------------------------
-def run_ours(args):
+def measure_config(idx: int, args, device, rank: int, world: int, dist, steps: int, warmup: int,
+                   cpu_seconds: float) -> dict:
+    """Device-resident throughput, end-to-end throughput, roofline and oracle baseline of one BASELINE.json config.
+    A step = one launch of ants_reconstruct over one batch (config 5: one of its eight 2 M-event batches)."""
     import torch
-    rank, local_rank, world = dist_env()
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
-    torch.cuda.set_device(local_rank)
-    device = torch.device("cuda", local_rank)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=device)
     from paper_1602_07247_b200 import recon, synth
-    recon.load()
-
-    cfg = synth.make_config(args.config)
+    cfg = synth.make_config(idx)
     E = cfg.n_events // cfg.n_batches if args.events is None else args.events
-    cfg_run = cfg
     n_resident = max(2, cfg.n_batches) if args.resident is None else args.resident
-    r = recon.Reconstructor(cfg_run)
+    r = recon.Reconstructor(cfg)
     sigs = [synth.generate_events(cfg, E, device=device, batch=rank_seed_batch(rank, j, n_resident))["signals"]
             for j in range(n_resident)]
     xyzA = torch.empty((E, 4), dtype=torch.float32, device=device)
@@ -240,20 +287,20 @@ def run_ours(args):
         recon.ants_reconstruct(r.handle, sigs[rank_batch(rank, step, n_resident)], r.grid, r.method, xyzA, score,
                                stream.cuda_stream)
 
-    for s in range(args.warmup):
+    for s in range(warmup):
         one(s)
     torch.cuda.synchronize()
     if dist is not None:
         dist.barrier()
     launches0 = recon.launch_count()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    sampler = ClockSampler(local_rank)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    sampler = ClockSampler(device.index or 0)
     torch.cuda.synchronize()
     with sampler:
-        for s in range(args.steps):
+        for s in range(steps):
             flush.fill_(s & 0xFF)                 # evict L2 (126 MB) between timed steps
             ev[s][0].record(stream)
-            one(args.warmup + s)
+            one(warmup + s)
             ev[s][1].record(stream)
         torch.cuda.synchronize()
     if dist is not None:
@@ -262,61 +309,113 @@ def run_ours(args):
     gpu_launches = recon.launch_count() - launches0
     local_ms = sum(step_ms)
     total_ms = max_over_ranks(local_ms, dist, device)
-    total_events = sum_over_ranks(float(E * args.steps), dist, device)
-    value = total_events / (total_ms * 1e-3)
+    total_events = sum_over_ranks(float(E * steps), dist, device)
+    out = {"config": workload_config(cfg, E, world), "value": total_events / (total_ms * 1e-3), "unit": UNIT,
+           "steps": steps, "warmup": warmup, "ms_per_step": total_ms / steps, "step_ms": step_ms,
+           "gpu_launches": int(gpu_launches), "clocks": sampler.summary()}
+    del flush
 
-    # ---- end to end: pinned host buffers through ants_reconstruct_host -----------------------
-    sig_h = sigs[0].cpu().pin_memory()
-    xyzA_h = torch.empty((E, 4), dtype=torch.float32).pin_memory()
-    score_h = torch.empty((E,), dtype=torch.float32).pin_memory()
-    chunk = max(1, min(E, args.e2e_chunk))
-    for _ in range(2):
-        recon.ants_reconstruct_host(r.handle, sig_h, r.grid, r.method, xyzA_h, score_h, chunk)
+    # ---- latency of one call (launch-bound workloads: config 1) ------------------------------------
+    if E <= 100_000:
+        n_calls = 200
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for s in range(n_calls):
+            one(s)
+        t_issue = time.perf_counter() - t0
+        torch.cuda.synchronize()
+        t_all = time.perf_counter() - t0
+        out["us_per_call"] = {"host_issue": 1e6 * t_issue / n_calls, "back_to_back": 1e6 * t_all / n_calls,
+                              "device_kernel": 1e3 * statistics.median(step_ms), "calls": n_calls}
+
+    # ---- end to end: pinned host buffers through ants_reconstruct_host -------------------------------
+    # config 5: the whole 16 M-event job as BASELINE.json states it (8 streamed batches of 2 M); others: one batch
+    n_e2e_batches = cfg.n_batches if args.events is None else 1
+    E2 = E * n_e2e_batches
+    sig_h = torch.empty((E2, cfg.n_sensors), dtype=torch.float32).pin_memory()
+    for j in range(n_e2e_batches):
+        sig_h[j * E:(j + 1) * E].copy_(sigs[j])
+    xyzA_h = torch.empty((E2, 4), dtype=torch.float32).pin_memory()
+    score_h = torch.empty((E2,), dtype=torch.float32).pin_memory()
+    chunk = E if n_e2e_batches > 1 else max(1, min(E, args.e2e_chunk))
+    torch.cuda.synchronize()
+    recon.ants_reconstruct_host(r.handle, sig_h, r.grid, r.method, xyzA_h, score_h, chunk)     # allocates the ring
     if dist is not None:
         dist.barrier()
-    e2e_steps = max(1, min(args.steps, 5))
+    e2e_steps = 1 if n_e2e_batches > 1 else max(1, min(steps, 5))
+    l0 = recon.launch_count()
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
         recon.ants_reconstruct_host(r.handle, sig_h, r.grid, r.method, xyzA_h, score_h, chunk)
     e2e_ms = (time.perf_counter() - t0) * 1e3
+    e2e_launches = recon.launch_count() - l0
     e2e_ms = max_over_ranks(e2e_ms, dist, device)
-    e2e_value = sum_over_ranks(float(E * e2e_steps), dist, device) / (e2e_ms * 1e-3)
+    e2e_value = sum_over_ranks(float(E2 * e2e_steps), dist, device) / (e2e_ms * 1e-3)
     assert torch.equal(xyzA_h[:1024].to(device), r(sigs[0][:1024].contiguous())[0])   # same kernel, same bits
+    out["e2e"] = {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": E2 * cfg.n_sensors * 4,
+                  "d2h_bytes_per_step": E2 * 20, "steps": e2e_steps, "events_per_step": E2, "chunk_events": chunk,
+                  "ms_per_step": e2e_ms / e2e_steps, "gpu_launches": int(e2e_launches),
+                  "api": "ants_reconstruct_host (pinned host buffers, 3-stream ring)"}
 
-    # ---- roofline of the one kernel (FP32 ALU bound) --------------------
+    # ---- roofline of the one kernel --------------------------------------------------------------------
     prop = torch.cuda.get_device_properties(device)
-    clocks = sampler.summary()
-    max_mhz = clocks["sm_max_mhz"] or 1965.0
-    peak_tflops = prop.multi_processor_count * FP32_LANES_PER_SM * 2 * max_mhz * 1e6 / 1e12
-    launch_ms = local_ms / max(gpu_launches, 1)
-    flops_per_launch = flop_per_pair(cfg) * cfg.pairs_per_event * E
-    achieved = flops_per_launch / (launch_ms * 1e-3) / 1e12
-    roofline = {"bound": "alu", "kernel": "ants::recon%dd_kernel" % cfg.dim, "achieved": achieved, "peak": peak_tflops,
-                "unit": "TFLOP/s", "frac": achieved / peak_tflops, "traffic": (TRAFFIC_PER_EVENT[cfg.name] * E if cfg.name in TRAFFIC_PER_EVENT else None),
-                "peak_source": "derived: SMs x 128 FP32 lanes x 2 x clocks.max.sm (MEASURED_PEAKS.json has no FP32 entry)",
-                "flop_per_pair_nominal": flop_per_pair(cfg), "pairs_per_s": cfg.pairs_per_event * E / (launch_ms * 1e-3),
-                "algorithmic_bytes_per_launch": E * (4 * cfg.n_sensors + 20),
-                "hbm_gbs_signal_stream": E * (4 * cfg.n_sensors + 20) / (launch_ms * 1e-3) / 1e9,
-                "launch_ms": launch_ms}
+    max_mhz = out["clocks"]["sm_max_mhz"] or 1965.0
+    out["plan"] = r.plan()
+    out["roofline"] = roofline_of(cfg, out["plan"], E, local_ms / max(gpu_launches, 1), prop, max_mhz)
 
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": workload_config(cfg, E, world), "clocks": clocks,
-            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": E * cfg.n_sensors * 4,
-                    "d2h_bytes_per_step": E * 20, "steps": e2e_steps, "chunk_events": chunk,
-                    "api": "ants_reconstruct_host (pinned host buffers, 3-stream ring)"},
-            "gpu_launches": int(gpu_launches), "roofline": roofline, "step_ms": step_ms,
-            "plan": r.plan()}
-
-    # ---- oracle beside it (rank 0, N = 1) -------------------------------------------------------
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+    # ---- oracle beside it (rank 0, N = 1) --------------------------------------------------------------
+    if rank == 0 and world == 1 and not args.no_cpu_baseline and cpu_seconds > 0:
         n_pool = min(E, 262_144)
-        rate, n, used = oracle_rate(cfg, sig_h[:n_pool].numpy(), args.cpu_seconds)
-        line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": used, "kind": "oracle",
-                                "sample": f"first {n} events of the same {cfg.name} batch, one pass, "
-                                          f"double precision, OpenMP over events"}
+        rate, n, used = oracle_rate(cfg, sig_h[:n_pool].numpy(), cpu_seconds)
+        out["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": used, "kind": "oracle",
+                               "sample": f"first {n} events of the same {cfg.name} batch, one pass, "
+                                         f"double precision, OpenMP over events"}
     r.close()
+    del sigs, sig_h, xyzA_h, score_h, xyzA, score
+    torch.cuda.empty_cache()
+    return out
+
+
+def run_ours(args):
+    import torch
+    rank, local_rank, world = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    device = torch.device("cuda", local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=device)
+    from paper_1602_07247_b200 import recon
+    recon.load()
+
+    head = measure_config(args.config, args, device, rank, world, dist, args.steps, args.warmup, args.cpu_seconds)
+    line = {"metric": METRIC, "value": head["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": head["ms_per_step"], "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": head["config"], "clocks": head["clocks"], "e2e": head["e2e"],
+            "gpu_launches": head["gpu_launches"], "roofline": head["roofline"], "step_ms": head["step_ms"],
+            "plan": head["plan"]}
+    if "cpu_baseline" in head:
+        line["cpu_baseline"] = head["cpu_baseline"]
+    if "us_per_call" in head:
+        line["us_per_call"] = head["us_per_call"]
+
+    # ---- every BASELINE.json config beside the headline (N = 1 only: north_star asks for all five) -----
+    if world == 1 and not args.no_per_config and args.events is None:
+        per = []
+        for idx in (1, 2, 3, 4, 5):
+            m = head if idx == args.config else measure_config(
+                idx, args, device, rank, world, dist, min(args.steps, 20), args.warmup, args.per_config_cpu_seconds)
+            entry = {k: m[k] for k in ("value", "unit", "ms_per_step", "steps", "warmup", "gpu_launches", "roofline",
+                                        "e2e", "plan", "clocks", "config") if k in m}
+            entry["config_index"] = idx
+            for k in ("cpu_baseline", "us_per_call"):
+                if k in m:
+                    entry[k] = m[k]
+            per.append(entry)
+        line["per_config"] = per
     if rank == 0:
         print(json.dumps(line), flush=True)
     if dist is not None:
@@ -325,10 +424,34 @@ def run_ours(args):
     return 0
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per event from the `ncu --set full` captures of the bench
-# command (profiles/r01_ncu_final.md); `traffic` = this x the events of one launch.  Config 1 was not captured.
-TRAFFIC_PER_EVENT = {"cfg2_pmt2d_hex19": 87.83, "cfg3_sipm_chi2_sq64": 257.5, "cfg4_axialz3d_hex37": 148.7,
-                     "cfg5_flood_hex127": 547.2}
+def run_peak(args):
+    """FP32 / MUFU / FP64 issue-rate probes behind the derived peak (`--workload peak`): ants_probe_throughput."""
+    import torch
+    from paper_1602_07247_b200 import recon
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device")
+    prop = torch.cuda.get_device_properties(0)
+    sampler = ClockSampler(0)
+    kinds = {0: "ffma", 1: "ffma2_packed", 2: "mufu_lg2", 3: "dfma", 4: "ffma_3_distinct_regs"}
+    res = {}
+    with sampler:
+        for kind, name in kinds.items():
+            best = 0.0
+            for _ in range(max(args.steps, 3)):
+                ops, ms = recon.ants_probe_throughput(kind, 8192)
+                best = max(best, ops)
+            res[name] = best
+    clocks = sampler.summary()
+    mhz = clocks["sm_max_mhz"] or 1965.0
+    cyc = prop.multi_processor_count * mhz * 1e6
+    line = {"metric": "dependent-free instruction throughput (ants_probe_throughput)", "unit": "lane-ops/s",
+            "n_gpus": 1, "sms": prop.multi_processor_count, "clocks": clocks,
+            "lane_ops_per_s": res, "lane_ops_per_clk_per_sm": {k: v / cyc for k, v in res.items()},
+            "fp32_tflops_ffma": 2 * res["ffma"] / 1e12, "fp32_tflops_ffma2": 2 * res["ffma2_packed"] / 1e12,
+            "fp64_tflops_dfma": 2 * res["dfma"] / 1e12,
+            "fp32_peak_derived_tflops": fp32_peak_tflops(prop, mhz)}
+    print(json.dumps(line), flush=True)
+    return 0
 
 
 # ---------------------------------------------------------------------------
@@ -449,14 +572,18 @@ def main(argv=None):
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config 1..5 (default 2 = configs[1])")
+    ap.add_argument("--config", type=int, default=5,
+                    help="BASELINE.json config 1..5 of the headline (default 5 = the largest single-GPU config: "
+                         "16 M events as 8 batches of 2 M)")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the per_config entries of the other configs")
+    ap.add_argument("--per-config-cpu-seconds", type=float, default=5.0)
     ap.add_argument("--events", type=int, default=None, help="events per step per GPU (default: the config's batch)")
     ap.add_argument("--resident", type=int, default=None, help="distinct resident batches to rotate through")
     ap.add_argument("--e2e-chunk", type=int, default=1 << 18)
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--ref-step-seconds", type=float, default=4.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--workload", default="reconstruct", choices=["reconstruct", "fit", "cycle"],
+    ap.add_argument("--workload", default="reconstruct", choices=["reconstruct", "fit", "cycle", "peak"],
                     help="fit = time the LRF calculation instead (secondary; not the BASELINE metric)")
     args = ap.parse_args(argv)
     if args.warmup < 3 and args.impl == "ours":
@@ -465,6 +592,8 @@ def main(argv=None):
         return run_fit(args)
     if args.workload == "cycle":
         return run_cycle(args)
+    if args.workload == "peak":
+        return run_peak(args)
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)

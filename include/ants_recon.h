@@ -48,12 +48,16 @@ enum ants_method {
                                      axial LRFs only */
 };
 
-/* Opaque LRF model living in device memory; immutable after create. */
+/* Opaque LRF model living in device memory.  Sensor positions, gains and tables are immutable after
+ * create; the only mutable state is the sensor selection (ants_lrf_set_selection), which must not be
+ * changed while a reconstruction that uses the handle is in flight. */
 typedef struct ants_lrf ants_lrf_t;
 
 typedef struct {
     int32_t n_sensors; /* N >= 1 */
-    int32_t n_lrf;     /* 1 = one shared profile, L_i = gains[i] * s(.); N = one table per sensor, L_i = s_i(.) */
+    int32_t n_lrf;     /* number of tables.  ants_lrf_create: 1 = one shared profile, L_i = gains[i] * s(.);
+                          N = one table per sensor, L_i = s_i(.).  ants_lrf_create_grouped: the number of
+                          sensor groups, L_i = gains[i] * s_group[i](.) */
     int32_t lrf_dim;   /* 1 = axial s(r); 2 = axial+z s(r,z) tensor product */
     int32_t n_int_r;   /* uniform intervals in r: n_int_r + 3 coefficients */
     int32_t n_int_z;   /* uniform intervals in z (ignored when lrf_dim == 1) */
@@ -77,6 +81,33 @@ typedef struct {
  */
 int ants_lrf_create(const float *sensor_xy, const float *gains, const float *knots,
                     const float *coeffs, const ants_lrf_dims_t *dims, ants_lrf_t **out);
+
+/*
+ * ants_lrf_create_grouped -- the same model with an explicit photosensor grouping (PAPER.md:400-406,
+ * section 6.2: "assign a number of photosensors to a group and use the same LRF for all photosensors within
+ * it ... a scaling parameter (relative gain) has to be assigned to each of them").  Reading R28:
+ *   group   HOST [N] int32, the table index of every sensor, 0 <= group[i] < dims->n_lrf;
+ *   coeffs  HOST [n_lrf][n_int_r + 3]: one profile per group;  L_i = gains[i] * s_group[i](r).
+ * Axial LRFs only (lrf_dim == 1).  The group tables are shared in shared memory by all sensors of a
+ * group.  Other arguments and errors as ants_lrf_create; a group index out of range is ANTS_ERR_INVALID.
+ */
+int ants_lrf_create_grouped(const float *sensor_xy, const float *gains, const int32_t *group,
+                            const float *knots, const float *coeffs, const ants_lrf_dims_t *dims,
+                            ants_lrf_t **out);
+
+/*
+ * ants_group_by_radius -- photosensor groups "according to the distance from the sensor center to the
+ * detector center" (section 6.2).  Reading R28: sensors are ordered by their distance from
+ * the origin (ties: lower index first); a new group starts wherever the distance exceeds the first
+ * distance of the current group by more than tol (mm); groups are numbered outward from 0.
+ *   sensor_xy HOST [N][2]; group_out HOST [N] int32; n_groups_out HOST int32.  Host-only, no GPU work.
+ * Errors: ANTS_ERR_INVALID (NULL, N < 1, tol < 0 or not finite, non-finite position), ANTS_ERR_NOMEM.
+ */
+int ants_group_by_radius(const float *sensor_xy, int32_t n_sensors, float tol, int32_t *group_out,
+                         int32_t *n_groups_out);
+
+/* Number of photosensors of a model (0 for NULL): lets a binding check its buffers. */
+int32_t ants_lrf_n_sensors(const ants_lrf_t *lrf);
 
 typedef struct {
     int32_t dim;            /* 2 = search (x,y); 3 = search (x,y,z), requires lrf_dim == 2 */
@@ -108,7 +139,12 @@ int ants_lrf_set_selection(ants_lrf_t *lrf, const uint8_t *passive, float signal
 
 /*
  * ants_reconstruct -- steps a1..a6 for a batch of events, ONE kernel launch,
- * asynchronous on `cuda_stream`, no allocation, no host synchronisation.
+ * asynchronous on `cuda_stream`, no allocation, no host synchronisation.  The launch plan (kernel
+ * variant, shared-memory carve-up, occupancy) is computed on the first call with a given
+ * (grid, method) and cached in the handle; later calls only fill the parameter block and launch.
+ * The handle must be used on the device it was created on (else ANTS_ERR_INVALID).  Up to 1024
+ * launches of one handle may be in flight at once; a further launch waits on the device (not on
+ * the host) for the launch that used its counter slot 1024 launches earlier.
  *   signals   DEVICE [n_events][N] float row-major, caller-owned, read-only.
  *   out_xyzA  DEVICE [n_events][4] float: x, y, z (0 for axial LRFs), energy A
  *             at the last best node (R11).
@@ -191,12 +227,23 @@ int ants_lrf_fit_gains(const float *sensor_xy, const float *knots, const float *
                        float *gains_out, double *n_used_out, void *cuda_stream);
 
 /*
+ * ants_gains_renormalise -- relative gains are defined up to a common factor ("a scaling
+ * parameter (relative gain)"); after a re-evaluation (ants_lrf_fit_gains) the iterative procedure of
+ * PAPER.md:428-440 carries them on at the scale of the previous set.  Reading R29: a sensor whose new
+ * estimate is missing (NaN) or not positive keeps its previous gain; the set is then multiplied by
+ * mean(gains_prev) / mean(set), all in double, rounded once to float.
+ *   gains_new HOST [N], gains_prev HOST [N] (all > 0), gains_out HOST [N] (may alias gains_new).
+ * Host-only.  Errors: ANTS_ERR_INVALID (NULL, N < 1, a previous gain that is not positive and finite).
+ */
+int ants_gains_renormalise(const float *gains_new, const float *gains_prev, int32_t n_sensors, float *gains_out);
+
+/*
  * ants_lrf_fit_axial_grouped -- ants_lrf_fit_axial with an explicit sensor grouping (section
  * 6.2: one group for all sensors, grouping by the distance from the sensor centre to the detector centre, or
  * by the symmetry of the array).  Reading R28: group HOST [N] int32 gives every sensor's table index in
  * 0 .. n_groups-1; the sensors of a group share one profile, each scaled by its relative gain (gains HOST [N]
- * or NULL).  coeffs_out HOST [n_groups][n_int_r + 3], n_used_out HOST [n_groups] or NULL.  To reconstruct with
- * a grouped response, expand it to one table per sensor (coefficients of the sensor's group times its gain).
+ * or NULL).  coeffs_out HOST [n_groups][n_int_r + 3], n_used_out HOST [n_groups] or NULL.  The result goes
+ * straight into ants_lrf_create_grouped with the same group array.
  * Other arguments, behaviour and errors as ants_lrf_fit_axial; a group index out of range is ANTS_ERR_INVALID.
  */
 int ants_lrf_fit_axial_grouped(const float *sensor_xy, const float *gains, const int32_t *group, const float *knots,
@@ -250,14 +297,35 @@ const char *ants_strerror(int status);
 int64_t ants_launch_count(void);
 
 /*
- * ants_plan_info -- host-only introspection of how a call would run (no GPU
- * work): first iteration index that uses the differential score (K if none),
- * nodes handled per lane, warps per CTA, CTAs per SM and dynamic shared-memory
- * bytes per CTA.  Any output pointer may be NULL.  Errors as ants_reconstruct.
+ * ants_plan_info -- introspection of how a call runs (no kernel launch): first iteration index that
+ * uses the differential score (K if none), nodes handled per lane, warps per CTA, resident CTAs per SM
+ * (as the runtime's occupancy calculator reports them for the chosen kernel and shared-memory size;
+ * 0 if no device can be asked) and dynamic shared-memory bytes per CTA.  Any output pointer may be
+ * NULL.  Errors as ants_reconstruct.
  */
 int ants_plan_info(const ants_lrf_t *lrf, const ants_grid_params_t *grid, int32_t method,
                    int32_t *first_diff_iter, int32_t *nodes_per_lane, int32_t *warps_per_cta,
                    int32_t *ctas_per_sm, int32_t *smem_bytes);
+
+/*
+ * ants_plan_kernel_name -- the name of the kernel instantiation ants_reconstruct launches for this
+ * (model, grid, method), as a profiler shows it (e.g. "ants::recon2d_pk_kernel<3,0>"), NUL-terminated
+ * and truncated to name_cap bytes.  Host-only.  Errors as ants_plan_info, plus ANTS_ERR_INVALID for a
+ * NULL or empty buffer.
+ */
+int ants_plan_kernel_name(const ants_lrf_t *lrf, const ants_grid_params_t *grid, int32_t method,
+                          char *name_out, int32_t name_cap);
+
+/*
+ * ants_probe_throughput -- micro-benchmark behind the roofline denominator (bench.py --workload peak):
+ * a grid that fills the device runs `iters` x 128 dependent-free instructions per thread of one kind:
+ *   0 FFMA (fp32 fused multiply-add, one operand register reused),  1 FFMA2 (packed pair, fma.rn.f32x2),
+ *   2 MUFU (lg2.approx),  3 DFMA (fp64),  4 FFMA whose three source registers are all distinct.
+ * lane_ops_per_second_out (HOST) receives scalar results per second (an FFMA2 counts two; x 2 = flop/s for
+ * the FMA kinds); milliseconds_out (HOST, may be NULL) the timed launch's duration.  Uses the default stream
+ * of the current device and waits for it.  Errors: ANTS_ERR_INVALID, ANTS_ERR_CUDA, ANTS_ERR_NOMEM.
+ */
+int ants_probe_throughput(int32_t kind, int32_t iters, double *lane_ops_per_second_out, double *milliseconds_out);
 
 #ifdef __cplusplus
 }

@@ -66,6 +66,10 @@ typedef struct {
     const uint8_t *passive;  /* [N] non-zero = passive, or NULL (none) */
     float signal_min;        /* sensors with S < signal_min are ignored; -inf (or NaN) = off */
     float dist_max;          /* sensors farther than this from the start position are ignored; +inf (NaN) = off */
+    /* photosensor grouping (section 6.2: "assign a number of photosensors to a group and use
+     * the same LRF for all photosensors within it ... a scaling parameter (relative gain) has to be assigned
+     * to each of them"); reading R28.  NULL = no explicit grouping (n_lrf == 1 or n_lrf == N as above) */
+    const int32_t *group;    /* [N] table index 0..n_lrf-1 of every sensor, or NULL */
 } oracle_model_t;
 
 typedef struct {
@@ -124,14 +128,16 @@ double oracle_spline2(const float *c, int nr, int nz, double r_lo, double r_hi,
 
 /* ---- LRF of sensor i at (x,y,z): L_i = g*_i s_m(i)(|p_xy - P_i|[, z])
  * (PAPER.md:388 axial; PAPER.md:394 axial+z; PAPER.md:400 shared profile +
- * relative gain) ------------------------------------------------------------ */
+ * relative gain; PAPER.md:402-406 sensor groups) ----------------------------- */
 double oracle_lrf(const oracle_model_t *m, int i, double x, double y, double z)
 {
     double dx = x - (double)m->sensor_xy[2 * i], dy = y - (double)m->sensor_xy[2 * i + 1];
     double r = sqrt(dx * dx + dy * dy);
     int per = (m->n_int_r + 3) * (m->lrf_dim == 2 ? m->n_int_z + 3 : 1);
-    const float *c = m->coeffs + (size_t)(m->n_lrf == 1 ? 0 : i) * per;
-    double g = m->n_lrf == 1 ? (double)m->gains[i] : 1.0;
+    /* table and scale of sensor i: a group's profile times the sensor's relative gain;
+     * one shared profile is the one-group case; a table of the sensor's own is not scaled */
+    const float *c = m->coeffs + (size_t)(m->group ? m->group[i] : (m->n_lrf == 1 ? 0 : i)) * per;
+    double g = (m->group || m->n_lrf == 1) ? (double)m->gains[i] : 1.0;
     double s = m->lrf_dim == 1
         ? oracle_spline1(c, m->n_int_r, m->knots[0], m->knots[1], r)
         : oracle_spline2(c, m->n_int_r, m->n_int_z, m->knots[0], m->knots[1],

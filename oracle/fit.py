@@ -196,3 +196,16 @@ def group_by_radius(sensor_xy, tol=1e-3):
             last = d[i]          # a group is anchored at its first (smallest) distance
         group[i] = g
     return group, g + 1
+
+
+def renormalise_gains(gains_new, gains_prev):
+    """Relative gains are defined up to a common factor (PAPER.md:400 "a scaling parameter (relative gain)");
+    between cycles of the iterative procedure they are carried on at the scale of the
+    previous set.  Reading R29: a sensor whose new estimate is missing (NaN) or not positive keeps its previous
+    gain; the set is then multiplied by mean(gains_prev) / mean(set).  -> float32 [N]."""
+    gn = np.asarray(gains_new, np.float32).astype(np.float64).reshape(-1)
+    gp = np.asarray(gains_prev, np.float32).astype(np.float64).reshape(-1)
+    with np.errstate(invalid="ignore"):
+        usable = np.isfinite(gn) & (gn > 0.0)
+    g = np.where(usable, gn, gp)
+    return (g * (gp.mean() / g.mean())).astype(np.float32)

@@ -32,7 +32,8 @@ class _Model(C.Structure):
                 ("n_int_r", C.c_int32), ("n_int_z", C.c_int32),
                 ("sensor_xy", C.c_void_p), ("gains", C.c_void_p),
                 ("knots", C.c_void_p), ("coeffs", C.c_void_p),
-                ("passive", C.c_void_p), ("signal_min", C.c_float), ("dist_max", C.c_float)]
+                ("passive", C.c_void_p), ("signal_min", C.c_float), ("dist_max", C.c_float),
+                ("group", C.c_void_p)]
 
 
 class _Grid(C.Structure):
@@ -97,7 +98,7 @@ class Model:
     """The LRF model: the float32 arrays handed to ants_lrf_create, kept alive here."""
 
     def __init__(self, sensor_xy, gains, knots, coeffs, n_lrf, lrf_dim, n_int_r, n_int_z,
-                 passive=None, signal_min=float("nan"), dist_max=float("nan")):
+                 passive=None, signal_min=float("nan"), dist_max=float("nan"), group=None):
         self.sensor_xy = _f32(sensor_xy).reshape(-1, 2)
         N = self.sensor_xy.shape[0]
         self.gains = _f32(np.ones(N) if gains is None else gains)
@@ -107,16 +108,20 @@ class Model:
         self.n_sensors = N
         self.passive = None if passive is None else np.ascontiguousarray(np.asarray(passive) != 0, dtype=np.uint8)
         assert self.passive is None or self.passive.size == N
+        self.group = None if group is None else np.ascontiguousarray(np.asarray(group, dtype=np.int32))
+        assert self.group is None or (self.group.size == N and self.group.min() >= 0 and self.group.max() < n_lrf)
         self.c = _Model(N, n_lrf, lrf_dim, n_int_r, n_int_z, self.sensor_xy.ctypes.data,
                         self.gains.ctypes.data, self.knots.ctypes.data, self.coeffs.ctypes.data,
                         None if self.passive is None else self.passive.ctypes.data,
-                        float(signal_min), float(dist_max))
+                        float(signal_min), float(dist_max),
+                        None if self.group is None else self.group.ctypes.data)
 
     @classmethod
     def from_config(cls, cfg):
         return cls(cfg.sensor_xy, cfg.gains, cfg.knots, cfg.coeffs, cfg.n_lrf, cfg.lrf_dim,
                    cfg.n_int_r, cfg.n_int_z, getattr(cfg, "passive", None),
-                   getattr(cfg, "signal_min", float("nan")), getattr(cfg, "dist_max", float("nan")))
+                   getattr(cfg, "signal_min", float("nan")), getattr(cfg, "dist_max", float("nan")),
+                   getattr(cfg, "group", None))
 
     def lrf(self, i, x, y, z=0.0):
         return _load().oracle_lrf(C.byref(self.c), int(i), float(x), float(y), float(z))

@@ -6,6 +6,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <algorithm>
 #include <atomic>
 #include <mutex>
 #include <new>
@@ -15,14 +16,45 @@
 #include "recon2d.cuh"
 #include "recon2d_pk.cuh"
 #include "recon3d.cuh"
+#include "kernels.h"
 
 using namespace ants;
+
+// launches that may be in flight at once on one model (each owns a counter pair until its last warp retires);
+// a launch that wraps around the ring waits, on the device, for the previous user of its slot
+static const unsigned kCtrSlots = 1024;
 
 // ---------------------------------------------------------------------------
 // the opaque handle
 // ---------------------------------------------------------------------------
+// launch plan of one (grid, method) on one model: computed once, cached in the handle
+struct Plan {
+    int npt = 0;             // nodes per lane (template instantiation)
+    int cpl = 0, gzm = 0;    // axial+z kernel: columns per lane, compiled z-levels
+    int family = 0;          // 0 recon2d_pk_kernel, 1 recon2d_kernel (generic), 2 recon3d_kernel
+    int warps = 0;           // warps per CTA
+    int ctas_per_sm = 0;     // resident CTAs per SM (cudaOccupancyMaxActiveBlocksPerMultiprocessor, capped by the tuning knob)
+    size_t smem = 0;         // dynamic shared memory per CTA
+    int k_diff = 0;          // first differential iteration (K = never)
+    int k_series = 0;        // axial+z Poisson: first iteration with the log1p series
+    const void *kernel = nullptr;
+    bool ready = false;      // cudaFuncSetAttribute + occupancy done (needs the device)
+};
+struct PlanKey {
+    int32_t dim, G, K, method, select;
+    float step0_xy, step0_z, factor;
+    bool operator==(const PlanKey &o) const {
+        return dim == o.dim && G == o.G && K == o.K && method == o.method && select == o.select &&
+               step0_xy == o.step0_xy && step0_z == o.step0_z && factor == o.factor;
+    }
+};
+
 struct ants_lrf {
     ModelDev dev{};          // device pointers + scalars, passed by value to the kernels
+    std::mutex plan_mu;      // guards plans
+    std::vector<std::pair<PlanKey, Plan>> plans;
+    void *d_grp = nullptr;
+    cudaEvent_t *slot_ev = nullptr;   // [kCtrSlots] lazily created: the launch that last used a counter slot
     int device = 0;
     int sm_count = 0;
     bool positive = false;   // every spline strictly positive on its domain
@@ -42,8 +74,6 @@ struct ants_lrf {
 };
 
 static std::atomic<int64_t> g_launches{0};
-// launches that may be in flight at once on one model (each owns a counter pair until its last warp retires)
-static const unsigned kCtrSlots = 4096;
 
 // ---------------------------------------------------------------------------
 // step a0: B-spline coefficients -> per-interval cubics
@@ -183,15 +213,23 @@ static void tensor_analysis(const float *c, const double *rows64, int n_r, int n
 
 static bool finite_f(float v) { return std::isfinite(v); }
 
-extern "C" int ants_lrf_create(const float *sensor_xy, const float *gains, const float *knots,
-                               const float *coeffs, const ants_lrf_dims_t *dims, ants_lrf_t **out) {
+// group == nullptr: n_lrf = 1 (all sensors on table 0, L = g s) or n_lrf = N (sensor i on table i, L = s_i)
+static int create_impl(const float *sensor_xy, const float *gains, const int32_t *group, const float *knots,
+                       const float *coeffs, const ants_lrf_dims_t *dims, ants_lrf_t **out) {
     if (!out) return ANTS_ERR_INVALID;
     *out = nullptr;
     if (!sensor_xy || !knots || !coeffs || !dims) return ANTS_ERR_INVALID;
     const int N = dims->n_sensors, n_lrf = dims->n_lrf, dim = dims->lrf_dim, n_r = dims->n_int_r;
     const int n_z = dim == 2 ? dims->n_int_z : 0;
     if (N < 1 || N > 65535 || (dim != 1 && dim != 2) || n_r < 1 || n_r > 4096) return ANTS_ERR_INVALID;
-    if (n_lrf != 1 && n_lrf != N) return ANTS_ERR_INVALID;
+    if (group) {
+        if (n_lrf < 1 || n_lrf > N) return ANTS_ERR_INVALID;
+        for (int i = 0; i < N; ++i)
+            if (group[i] < 0 || group[i] >= n_lrf) return ANTS_ERR_INVALID;
+        if (dim != 1) return ANTS_ERR_UNSUPPORTED;
+    } else if (n_lrf != 1 && n_lrf != N) {
+        return ANTS_ERR_INVALID;
+    }
     if (dim == 2 && (n_z < 1 || n_z > 1024)) return ANTS_ERR_INVALID;
     const float r_lo = knots[0], r_hi = knots[1];
     if (!finite_f(r_lo) || !finite_f(r_hi) || !(r_lo >= 0.f) || !(r_hi > r_lo)) return ANTS_ERR_INVALID;
@@ -224,9 +262,13 @@ extern "C" int ants_lrf_create(const float *sensor_xy, const float *gains, const
     const size_t n_spl = (size_t)n_lrf * n_rows_z;   // r-splines in the table
     std::vector<float4> sens(N), rows32(n_spl * (n_r + 1));
     std::vector<double> rows64(n_spl * n_r * 4);
+    std::vector<int> grp(N);
+    // a shared or group profile is scaled by the relative gain; per-sensor tables are not
+    const bool scaled = group != nullptr || n_lrf == 1;
     for (int i = 0; i < N; ++i) {
         float g = gains ? gains[i] : 1.f;
-        sens[i] = make_float4(sensor_xy[2 * i], sensor_xy[2 * i + 1], g, 1.f / g);
+        sens[i] = make_float4(sensor_xy[2 * i], sensor_xy[2 * i + 1], scaled ? g : 1.f, 1.f / g);
+        grp[i] = group ? group[i] : (n_lrf == 1 ? 0 : i);
     }
     const double sc_r = (double)n_r / ((double)r_hi - (double)r_lo);
     bool positive = true;
@@ -243,26 +285,31 @@ extern "C" int ants_lrf_create(const float *sensor_xy, const float *gains, const
     h->knot_r = 1.0 / sc_r;
     h->knot_z = dim == 2 ? ((double)z_hi - (double)z_lo) / n_z : 0.0;
 
+    h->slot_ev = new (std::nothrow) cudaEvent_t[kCtrSlots]();
+    if (!h->slot_ev) { delete h; return ANTS_ERR_NOMEM; }
     cudaError_t e0 = cudaMalloc(&h->d_ctr, kCtrSlots * 2 * sizeof(unsigned long long));
     if (e0 == cudaSuccess) e0 = cudaMemset(h->d_ctr, 0, kCtrSlots * 2 * sizeof(unsigned long long));
     cudaError_t e1 = cudaMalloc(&h->d_sens, sens.size() * sizeof(float4));
     cudaError_t e2 = cudaMalloc(&h->d_poly, rows32.size() * sizeof(float4));
     cudaError_t e3 = cudaMalloc(&h->d_polyd, rows64.size() * sizeof(double));
-    if (e0 != cudaSuccess || e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess) {
+    cudaError_t e4 = cudaMalloc(&h->d_grp, grp.size() * sizeof(int));
+    if (e0 != cudaSuccess || e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess || e4 != cudaSuccess) {
         cudaGetLastError();
         ants_destroy(h);
         return (e1 == cudaErrorMemoryAllocation || e2 == cudaErrorMemoryAllocation ||
-                e3 == cudaErrorMemoryAllocation) ? ANTS_ERR_NOMEM : ANTS_ERR_CUDA;
+                e3 == cudaErrorMemoryAllocation || e4 == cudaErrorMemoryAllocation) ? ANTS_ERR_NOMEM : ANTS_ERR_CUDA;
     }
     if (cudaMemcpy(h->d_sens, sens.data(), sens.size() * sizeof(float4), cudaMemcpyHostToDevice) != cudaSuccess ||
         cudaMemcpy(h->d_poly, rows32.data(), rows32.size() * sizeof(float4), cudaMemcpyHostToDevice) != cudaSuccess ||
-        cudaMemcpy(h->d_polyd, rows64.data(), rows64.size() * sizeof(double), cudaMemcpyHostToDevice) != cudaSuccess) {
+        cudaMemcpy(h->d_polyd, rows64.data(), rows64.size() * sizeof(double), cudaMemcpyHostToDevice) != cudaSuccess ||
+        cudaMemcpy(h->d_grp, grp.data(), grp.size() * sizeof(int), cudaMemcpyHostToDevice) != cudaSuccess) {
         cudaGetLastError();
         ants_destroy(h);
         return ANTS_ERR_CUDA;
     }
     ModelDev &m = h->dev;
     m.sens = (const float4 *)h->d_sens;
+    m.grp = (const int *)h->d_grp;
     m.poly = (const float4 *)h->d_poly;
     m.polyd = (const double *)h->d_polyd;
     m.N = N;
@@ -281,6 +328,62 @@ extern "C" int ants_lrf_create(const float *sensor_xy, const float *gains, const
     m.signal_min = m.dist_max = std::nanf("");
     m.select = 0;
     *out = h;
+    return ANTS_OK;
+}
+
+extern "C" int ants_lrf_create(const float *sensor_xy, const float *gains, const float *knots,
+                               const float *coeffs, const ants_lrf_dims_t *dims, ants_lrf_t **out) {
+    return create_impl(sensor_xy, gains, nullptr, knots, coeffs, dims, out);
+}
+
+extern "C" int ants_lrf_create_grouped(const float *sensor_xy, const float *gains, const int32_t *group,
+                                       const float *knots, const float *coeffs, const ants_lrf_dims_t *dims,
+                                       ants_lrf_t **out) {
+    if (out) *out = nullptr;
+    if (!group) return ANTS_ERR_INVALID;
+    return create_impl(sensor_xy, gains, group, knots, coeffs, dims, out);
+}
+
+extern "C" int32_t ants_lrf_n_sensors(const ants_lrf_t *lrf) { return lrf ? lrf->dev.N : 0; }
+
+// groups by the distance from the sensor centre to the detector centre (R28)
+extern "C" int ants_group_by_radius(const float *sensor_xy, int32_t n, float tol, int32_t *group_out,
+                                    int32_t *n_groups_out) {
+    if (!sensor_xy || !group_out || !n_groups_out || n < 1 || !(tol >= 0.f) || !std::isfinite(tol)) return ANTS_ERR_INVALID;
+    std::vector<std::pair<double, int>> order;
+    try { order.reserve(n); } catch (const std::bad_alloc &) { return ANTS_ERR_NOMEM; }
+    for (int i = 0; i < n; ++i) {
+        const double x = sensor_xy[2 * i], y = sensor_xy[2 * i + 1];
+        if (!std::isfinite(x) || !std::isfinite(y)) return ANTS_ERR_INVALID;
+        order.emplace_back(std::sqrt(x * x + y * y), i);
+    }
+    std::stable_sort(order.begin(), order.end(),
+                     [](const std::pair<double, int> &a, const std::pair<double, int> &b) { return a.first < b.first; });
+    int current = -1;
+    double anchor = -INFINITY;
+    for (const auto &o : order) {
+        if (o.first - anchor > (double)tol) { ++current; anchor = o.first; }
+        group_out[o.second] = current;
+    }
+    *n_groups_out = current + 1;
+    return ANTS_OK;
+}
+
+// relative gains carried on at the scale of the previous set (R29)
+extern "C" int ants_gains_renormalise(const float *gains_new, const float *gains_prev, int32_t n, float *gains_out) {
+    if (!gains_new || !gains_prev || !gains_out || n < 1) return ANTS_ERR_INVALID;
+    double sum_prev = 0.0, sum_set = 0.0;
+    for (int i = 0; i < n; ++i) {
+        if (!(gains_prev[i] > 0.f) || !std::isfinite(gains_prev[i])) return ANTS_ERR_INVALID;
+        const bool usable = gains_new[i] > 0.f && std::isfinite(gains_new[i]);
+        sum_prev += (double)gains_prev[i];
+        sum_set += (double)(usable ? gains_new[i] : gains_prev[i]);
+    }
+    const double scale = sum_prev / sum_set;     // mean(prev) / mean(set): the counts cancel
+    for (int i = 0; i < n; ++i) {
+        const bool usable = gains_new[i] > 0.f && std::isfinite(gains_new[i]);
+        gains_out[i] = (float)((double)(usable ? gains_new[i] : gains_prev[i]) * scale);
+    }
     return ANTS_OK;
 }
 
@@ -315,6 +418,12 @@ extern "C" void ants_destroy(ants_lrf_t *h) {
     cudaFree(h->d_polyd);
     cudaFree(h->d_passive);
     cudaFree(h->d_ctr);
+    cudaFree(h->d_grp);
+    if (h->slot_ev) {
+        for (unsigned s = 0; s < kCtrSlots; ++s)
+            if (h->slot_ev[s]) cudaEventDestroy(h->slot_ev[s]);
+        delete[] h->slot_ev;
+    }
     for (int s = 0; s < 3; ++s) {
         cudaFree(h->d_sig[s]);
         cudaFree(h->d_xyzA[s]);
@@ -342,42 +451,32 @@ extern "C" int64_t ants_launch_count(void) { return g_launches.load(); }
 // ---------------------------------------------------------------------------
 // launch planning
 // ---------------------------------------------------------------------------
-struct Plan {
-    int npt = 0;             // nodes per lane (template instantiation)
-    int warps = 0;           // warps per CTA
-    int ctas_per_sm = 0;
-    size_t smem = 0;         // dynamic shared memory per CTA
-    int k_diff = 0;          // first differential iteration (K = never)
-    int k_series = 0;        // axial+z Poisson: first iteration with the log1p series
-    const void *kernel = nullptr;
-};
+// kernel look-ups: the instantiations live in k2d_pk_m*.cu, k2d_gen_m*.cu, k3d_m*.cu (kernels.h)
+namespace ants {
+const void *kernel_2d_pk_m0(int), *kernel_2d_pk_m1(int), *kernel_2d_pk_m2(int);
+const void *kernel_2d_gen_m0(int), *kernel_2d_gen_m1(int), *kernel_2d_gen_m2(int);
+const void *kernel_3d_m0(int, int), *kernel_3d_m1(int, int);
+const void *kernel_2d_pk(int method, int npt) {
+    return method == 0 ? kernel_2d_pk_m0(npt) : method == 1 ? kernel_2d_pk_m1(npt) : method == 2 ? kernel_2d_pk_m2(npt) : nullptr;
+}
+const void *kernel_2d_gen(int method, int npt) {
+    return method == 0 ? kernel_2d_gen_m0(npt) : method == 1 ? kernel_2d_gen_m1(npt) : method == 2 ? kernel_2d_gen_m2(npt) : nullptr;
+}
+const void *kernel_3d(int method, int cpl, int gzm) {
+    return method == 0 ? kernel_3d_m0(cpl, gzm) : method == 1 ? kernel_3d_m1(cpl, gzm) : nullptr;
+}
+}  // namespace ants
 
 static const int kNpt2D[] = {1, 2, 3, 4, 8};
 static const double kQSeries = 0.1;   // |dL/L0| bound under which the degree-6 log1p series is used
 
-template <int METHOD>
-static const void *pick2d_pk(int npt) {
-    switch (npt) {
-        case 1: return (const void *)recon2d_pk_kernel<1, METHOD>;
-        case 2: return (const void *)recon2d_pk_kernel<2, METHOD>;
-        case 3: return (const void *)recon2d_pk_kernel<3, METHOD>;
-        case 4: return (const void *)recon2d_pk_kernel<4, METHOD>;
-        case 8: return (const void *)recon2d_pk_kernel<8, METHOD>;
-    }
-    return nullptr;
+// tuning knobs, read once per process (experiments only; not needed in production)
+static int env_knob(const char *name) {
+    const char *e = std::getenv(name);
+    return e ? std::atoi(e) : 0;
 }
-
-template <int METHOD, bool POS>
-static const void *pick2d(int npt) {
-    switch (npt) {
-        case 1: return (const void *)recon2d_kernel<1, METHOD, POS>;
-        case 2: return (const void *)recon2d_kernel<2, METHOD, POS>;
-        case 3: return (const void *)recon2d_kernel<3, METHOD, POS>;
-        case 4: return (const void *)recon2d_kernel<4, METHOD, POS>;
-        case 8: return (const void *)recon2d_kernel<8, METHOD, POS>;
-    }
-    return nullptr;
-}
+static int knob_warps_per_cta() { static const int v = env_knob("ANTS_WARPS_PER_CTA"); return v; }
+static int knob_max_ctas_per_sm() { static const int v = env_knob("ANTS_MAX_CTAS_PER_SM"); return v; }
 
 static int validate_grid(const ants_lrf *h, const ants_grid_params_t *g, int32_t method) {
     if (!h || !g) return ANTS_ERR_INVALID;
@@ -414,7 +513,7 @@ static int first_diff_iter(const ants_lrf *h, const ants_grid_params_t *g, int32
 
 // CTA shape: the warps-per-CTA in {8, 4, 2, 1} that lets the most warps share an SM's shared memory
 // (each CTA carries its own copy of the model tables; 1 KB per CTA is reserved by the driver).
-// ANTS_WARPS_PER_CTA in the environment overrides the choice (tuning knob, not needed in production).
+// ANTS_WARPS_PER_CTA in the environment overrides the choice.
 static void pick_cta_shape(size_t tables, size_t per_warp, Plan &pl) {
     const size_t budget = 227 * 1024;
     int best = 1, best_total = 0;
@@ -425,22 +524,10 @@ static void pick_cta_shape(size_t tables, size_t per_warp, Plan &pl) {
         ctas = std::min(ctas, 32);
         if (ctas * wp > best_total) { best_total = ctas * wp; best = wp; }
     }
-    if (const char *e = std::getenv("ANTS_WARPS_PER_CTA")) {
-        const int v = std::atoi(e);
-        if (v == 1 || v == 2 || v == 4 || v == 8) best = v;
-    }
+    const int v = knob_warps_per_cta();
+    if (v == 1 || v == 2 || v == 4 || v == 8) best = v;
     pl.warps = best;
     pl.smem = tables + best * per_warp;
-    pl.ctas_per_sm = std::max(1, (int)std::min<size_t>(budget / (pl.smem + 1024), (size_t)(64 / best)));
-}
-
-template <int METHOD>
-static const void *pick3d(int cpl, int gzm) {
-#define ANTS_K3(C, Z) if (cpl == C && gzm == Z) return (const void *)recon3d_kernel<C, Z, METHOD>
-    ANTS_K3(1, 1); ANTS_K3(2, 1); ANTS_K3(3, 1); ANTS_K3(4, 1); ANTS_K3(8, 1);
-    ANTS_K3(1, 4); ANTS_K3(2, 4); ANTS_K3(1, 8); ANTS_K3(2, 8);
-#undef ANTS_K3
-    return nullptr;
 }
 
 // axial+z LRF: search over (x, y, z) or over (x, y) at fixed z
@@ -458,8 +545,11 @@ static int make_plan3d(const ants_lrf *h, const ants_grid_params_t *g, int32_t m
         for (int c : kNpt2D)
             if (c >= need) { cpl = c; break; }
     }
+    pl.family = 2;
+    pl.cpl = cpl;
+    pl.gzm = gzm;
     pl.npt = cpl * Gz;
-    pl.kernel = method == ANTS_POISSON_ML ? pick3d<0>(cpl, gzm) : pick3d<1>(cpl, gzm);
+    pl.kernel = kernel_3d(method, cpl, gzm);
     if (!pl.kernel) return ANTS_ERR_UNSUPPORTED;
     // differential from the first grid that stays within one knot interval of the centre (r and z);
     // Poisson log1p by series once |dL/L0| <= kQSeries on the whole grid
@@ -477,12 +567,12 @@ static int make_plan3d(const ants_lrf *h, const ants_grid_params_t *g, int32_t m
     }
     const size_t tables = (size_t)(m.N + (m.n_z + 3) * (m.n_r + 1)) * 16;
     const size_t per_warp = warp_smem_bytes_3d(m.N, Gz, m.n_r + 1);
-    const size_t budget = 227 * 1024;
     pick_cta_shape(tables, per_warp, pl);
-    if (pl.smem > budget) return ANTS_ERR_UNSUPPORTED;
+    if (pl.smem > 227 * 1024) return ANTS_ERR_UNSUPPORTED;
     return ANTS_OK;
 }
 
+// host-only part of the plan (no CUDA call): kernel variant, score switch-over, shared-memory carve-up
 static int make_plan(const ants_lrf *h, const ants_grid_params_t *g, int32_t method, Plan &pl) {
     int rc = validate_grid(h, g, method);
     if (rc != ANTS_OK) return rc;
@@ -501,33 +591,90 @@ static int make_plan(const ants_lrf *h, const ants_grid_params_t *g, int32_t met
     // strictly positive LRFs (the normal case) run the sensor-pair-packed kernel; others the generic one
     const bool packed = h->positive;
     if (!packed && m.select) return ANTS_ERR_UNSUPPORTED;   // the generic kernel has no sensor selection
-    if (packed)
-        pl.kernel = method == 0 ? pick2d_pk<0>(pl.npt) : method == 1 ? pick2d_pk<1>(pl.npt) : pick2d_pk<2>(pl.npt);
-    else
-        pl.kernel = method == 0 ? pick2d<0, false>(pl.npt) : method == 1 ? pick2d<1, false>(pl.npt) : pick2d<2, false>(pl.npt);
+    pl.family = packed ? 0 : 1;
+    pl.kernel = packed ? kernel_2d_pk(method, pl.npt) : kernel_2d_gen(method, pl.npt);
+    if (!pl.kernel) return ANTS_ERR_UNSUPPORTED;
     pl.k_diff = first_diff_iter(h, g, method);
     if (!packed && method == ANTS_CHI_SQUARE_SUMRATIO) pl.k_diff = g->n_iter;   // generic kernel: plain form only
     pl.k_series = pl.k_diff;
-    const size_t tables = packed ? (cta_smem_bytes_pk(m.N, m.n_lrf * (m.n_r + 1)) + 15) / 16 * 16
-                                 : (size_t)(m.N + m.n_lrf * (m.n_r + 1)) * 16;
+    const size_t tables = (cta_table_bytes(m.N, m.n_lrf * (m.n_r + 1)) + 15) / 16 * 16;
     const size_t per_warp = packed ? warp_smem_bytes_pk(m.N, method) : warp_smem_bytes_2d(m.N);
-    const size_t budget = 227 * 1024;
     pick_cta_shape(tables, per_warp, pl);
-    if (pl.smem > budget) return ANTS_ERR_UNSUPPORTED;
+    if (pl.smem > 227 * 1024) return ANTS_ERR_UNSUPPORTED;
     return ANTS_OK;
+}
+
+// the cached plan of (grid, method): planned on first use; with `need_device` the kernel's shared-memory
+// attribute is set and the resident CTAs per SM are asked from the runtime (once per plan)
+static int get_plan(const ants_lrf *hc, const ants_grid_params_t *g, int32_t method, bool need_device, Plan &out) {
+    if (!hc || !g) return ANTS_ERR_INVALID;
+    ants_lrf *h = const_cast<ants_lrf *>(hc);
+    const PlanKey key{g->dim, g->nodes_per_axis, g->n_iter, method, h->dev.select, g->step0_xy,
+                      g->dim == 3 ? g->step0_z : 0.f, g->factor};
+    std::lock_guard<std::mutex> lock(h->plan_mu);
+    Plan *pl = nullptr;
+    for (auto &kv : h->plans)
+        if (kv.first == key) { pl = &kv.second; break; }
+    if (!pl) {
+        Plan fresh;
+        int rc = make_plan(h, g, method, fresh);
+        if (rc != ANTS_OK) return rc;
+        if (h->plans.size() >= 64) h->plans.erase(h->plans.begin());
+        h->plans.emplace_back(key, fresh);
+        pl = &h->plans.back().second;
+    } else {
+        // grid values outside the key (seed mode, z seed) still need checking
+        int rc = validate_grid(h, g, method);
+        if (rc != ANTS_OK) return rc;
+    }
+    if (need_device && !pl->ready) {
+        if (cudaFuncSetAttribute(pl->kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->smem) != cudaSuccess) {
+            cudaGetLastError();
+            return ANTS_ERR_CUDA;
+        }
+        int occ = 0;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pl->kernel, pl->warps * 32, pl->smem) != cudaSuccess ||
+            occ < 1) {
+            cudaGetLastError();
+            return ANTS_ERR_CUDA;
+        }
+        const int cap = knob_max_ctas_per_sm();       // tuning knob: fewer resident CTAs
+        if (cap >= 1 && cap < occ) occ = cap;
+        pl->ctas_per_sm = occ;
+        pl->ready = true;
+    }
+    out = *pl;
+    return ANTS_OK;
+}
+
+static void kernel_name(const Plan &pl, int32_t method, char *buf, size_t n) {
+    if (pl.family == 0) std::snprintf(buf, n, "ants::recon2d_pk_kernel<%d,%d>", pl.npt, (int)method);
+    else if (pl.family == 1) std::snprintf(buf, n, "ants::recon2d_kernel<%d,%d,false>", pl.npt, (int)method);
+    else std::snprintf(buf, n, "ants::recon3d_kernel<%d,%d,%d>", pl.cpl, pl.gzm, (int)method);
 }
 
 extern "C" int ants_plan_info(const ants_lrf_t *lrf, const ants_grid_params_t *grid, int32_t method,
                               int32_t *first_diff, int32_t *nodes_per_lane, int32_t *warps_per_cta,
                               int32_t *ctas_per_sm, int32_t *smem_bytes) {
     Plan pl;
-    int rc = make_plan(lrf, grid, method, pl);
+    int rc = get_plan(lrf, grid, method, true, pl);
+    if (rc == ANTS_ERR_CUDA) rc = get_plan(lrf, grid, method, false, pl);
     if (rc != ANTS_OK) return rc;
     if (first_diff) *first_diff = pl.k_diff;
     if (nodes_per_lane) *nodes_per_lane = pl.npt;
     if (warps_per_cta) *warps_per_cta = pl.warps;
-    if (ctas_per_sm) *ctas_per_sm = pl.ctas_per_sm;
+    if (ctas_per_sm) *ctas_per_sm = pl.ready ? pl.ctas_per_sm : 0;
     if (smem_bytes) *smem_bytes = (int32_t)pl.smem;
+    return ANTS_OK;
+}
+
+extern "C" int ants_plan_kernel_name(const ants_lrf_t *lrf, const ants_grid_params_t *grid, int32_t method,
+                                     char *name_out, int32_t name_cap) {
+    if (!name_out || name_cap < 1) return ANTS_ERR_INVALID;
+    Plan pl;
+    int rc = get_plan(lrf, grid, method, false, pl);
+    if (rc != ANTS_OK) return rc;
+    kernel_name(pl, method, name_out, (size_t)name_cap);
     return ANTS_OK;
 }
 
@@ -536,12 +683,23 @@ extern "C" int ants_plan_info(const ants_lrf_t *lrf, const ants_grid_params_t *g
 // ---------------------------------------------------------------------------
 static int launch(const ants_lrf *h, const float *signals, int64_t n_events, const ants_grid_params_t *g,
                   int32_t method, float *out_xyzA, float *out_score, uint16_t *out_path, cudaStream_t stream) {
-    Plan pl;
-    int rc = make_plan(h, g, method, pl);
-    if (rc != ANTS_OK) return rc;
+    if (!h || !g) return ANTS_ERR_INVALID;
     if (n_events < 0) return ANTS_ERR_INVALID;
-    if (n_events == 0) return ANTS_OK;
-    if (!signals || !out_xyzA || !out_score) return ANTS_ERR_INVALID;
+    if (n_events == 0) {
+        Plan probe;
+        return get_plan(h, g, method, false, probe);     // arguments are still checked
+    }
+    if (!signals || !out_xyzA || !out_score) {
+        Plan probe;
+        const int rc = get_plan(h, g, method, false, probe);
+        return rc != ANTS_OK ? rc : ANTS_ERR_INVALID;
+    }
+    int dev_now = -1;
+    if (cudaGetDevice(&dev_now) != cudaSuccess) { cudaGetLastError(); return ANTS_ERR_CUDA; }
+    if (dev_now != h->device) return ANTS_ERR_INVALID;   // the model lives on the device it was created on
+    Plan pl;
+    int rc = get_plan(h, g, method, true, pl);
+    if (rc != ANTS_OK) return rc;
     if (g->n_iter > 65535) return ANTS_ERR_INVALID;
 
     Params p{};
@@ -566,29 +724,33 @@ static int launch(const ants_lrf *h, const float *signals, int64_t n_events, con
     p.warps_per_cta = pl.warps;
     p.tile_events = pl.warps;
 
-    if (cudaFuncSetAttribute(pl.kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem) != cudaSuccess) {
-        cudaGetLastError();
-        return ANTS_ERR_CUDA;
-    }
-    int occ = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pl.kernel, pl.warps * 32, pl.smem) != cudaSuccess ||
-        occ < 1) {
-        cudaGetLastError();
-        return ANTS_ERR_CUDA;
-    }
-    if (const char *e = std::getenv("ANTS_MAX_CTAS_PER_SM")) {   // tuning knob: fewer resident CTAs
-        const int v = std::atoi(e);
-        if (v >= 1 && v < occ) occ = v;
-    }
     long long want = (n_events + pl.warps - 1) / pl.warps;
-    long long cap = (long long)h->sm_count * occ;
+    long long cap = (long long)h->sm_count * pl.ctas_per_sm;
     int grid = (int)std::min(want, cap);
-    p.ctr = h->d_ctr + 2 * (const_cast<ants_lrf *>(h)->next_slot.fetch_add(1) % kCtrSlots);
+    // counter slot: a launch that reuses a slot (1024 launches later) first waits, on the device, for the
+    // slot's previous launch; the event recorded after this launch is what a later user waits for
+    ants_lrf *hm = const_cast<ants_lrf *>(h);
+    const unsigned ticket = hm->next_slot.fetch_add(1);
+    const unsigned slot = ticket % kCtrSlots;
+    if (ticket >= kCtrSlots && hm->slot_ev[slot] &&
+        cudaStreamWaitEvent(stream, hm->slot_ev[slot], 0) != cudaSuccess) {
+        cudaGetLastError();
+        return ANTS_ERR_CUDA;
+    }
+    p.ctr = h->d_ctr + 2 * slot;
     p.total_warps = grid * pl.warps;
     void *args[] = {&p};
     if (cudaLaunchKernel(pl.kernel, dim3(grid), dim3(pl.warps * 32), args, pl.smem, stream) != cudaSuccess) {
         cudaGetLastError();
         return ANTS_ERR_CUDA;
+    }
+    if (!hm->slot_ev[slot] && cudaEventCreateWithFlags(&hm->slot_ev[slot], cudaEventDisableTiming) != cudaSuccess) {
+        cudaGetLastError();
+        hm->slot_ev[slot] = nullptr;
+        cudaStreamSynchronize(stream);                  // no event to order a later user of the slot: drain now
+    } else if (cudaEventRecord(hm->slot_ev[slot], stream) != cudaSuccess) {
+        cudaGetLastError();
+        cudaStreamSynchronize(stream);
     }
     g_launches.fetch_add(1);
     return ANTS_OK;
@@ -640,7 +802,7 @@ extern "C" int ants_reconstruct_host(const ants_lrf_t *lrf, const float *signals
                                      const ants_grid_params_t *grid, int32_t method, float *out_xyzA_host,
                                      float *out_score_host, int64_t chunk_events) {
     Plan pl;
-    int rc = make_plan(lrf, grid, method, pl);
+    int rc = get_plan(lrf, grid, method, false, pl);
     if (rc != ANTS_OK) return rc;
     if (n_events < 0) return ANTS_ERR_INVALID;
     if (n_events == 0) return ANTS_OK;
@@ -653,23 +815,24 @@ extern "C" int ants_reconstruct_host(const ants_lrf_t *lrf, const float *signals
     if (rc != ANTS_OK) return rc;
     const int N = h->dev.N;
     int slot = 0;
-    for (int64_t a = 0; a < n_events; a += chunk, slot = (slot + 1) % 3) {
+    for (int64_t a = 0; a < n_events && rc == ANTS_OK; a += chunk, slot = (slot + 1) % 3) {
         const int64_t n = std::min(chunk, n_events - a);
         cudaStream_t st = h->streams[slot];
         // the stream order makes the slot's buffers safe to reuse: the previous
         // occupant's D2H copy is ahead of this H2D copy on the same stream
         if (cudaMemcpyAsync(h->d_sig[slot], signals_host + a * N, (size_t)n * N * sizeof(float),
-                            cudaMemcpyHostToDevice, st) != cudaSuccess) { cudaGetLastError(); return ANTS_ERR_CUDA; }
+                            cudaMemcpyHostToDevice, st) != cudaSuccess) { cudaGetLastError(); rc = ANTS_ERR_CUDA; break; }
         rc = launch(h, h->d_sig[slot], n, grid, method, h->d_xyzA[slot], h->d_score[slot], nullptr, st);
-        if (rc != ANTS_OK) return rc;
+        if (rc != ANTS_OK) break;
         if (cudaMemcpyAsync(out_xyzA_host + a * 4, h->d_xyzA[slot], (size_t)n * 4 * sizeof(float),
                             cudaMemcpyDeviceToHost, st) != cudaSuccess ||
             cudaMemcpyAsync(out_score_host + a, h->d_score[slot], (size_t)n * sizeof(float),
-                            cudaMemcpyDeviceToHost, st) != cudaSuccess) { cudaGetLastError(); return ANTS_ERR_CUDA; }
+                            cudaMemcpyDeviceToHost, st) != cudaSuccess) { cudaGetLastError(); rc = ANTS_ERR_CUDA; }
     }
+    // also on an error: no copy that touches the caller's buffers may still be in flight on return
     for (int s = 0; s < 3; ++s)
-        if (cudaStreamSynchronize(h->streams[s]) != cudaSuccess) { cudaGetLastError(); return ANTS_ERR_CUDA; }
-    return ANTS_OK;
+        if (cudaStreamSynchronize(h->streams[s]) != cudaSuccess) { cudaGetLastError(); if (rc == ANTS_OK) rc = ANTS_ERR_CUDA; }
+    return rc;
 }
 
 // ---------------------------------------------------------------------------

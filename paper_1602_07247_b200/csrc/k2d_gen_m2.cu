@@ -1,0 +1,16 @@
+// k2d_gen_m2.cu -- instantiations of recon2d_kernel<NPT, 2, false> (LRFs that are not positive everywhere)
+#include "recon2d.cuh"
+#include "kernels.h"
+
+namespace ants {
+const void *kernel_2d_gen_m2(int npt) {
+    switch (npt) {
+        case 1: return (const void *)recon2d_kernel<1, 2, false>;
+        case 2: return (const void *)recon2d_kernel<2, 2, false>;
+        case 3: return (const void *)recon2d_kernel<3, 2, false>;
+        case 4: return (const void *)recon2d_kernel<4, 2, false>;
+        case 8: return (const void *)recon2d_kernel<8, 2, false>;
+    }
+    return nullptr;
+}
+}  // namespace ants

@@ -43,12 +43,11 @@ __device__ __forceinline__ WarpSmem2D carve_2d(unsigned char *base, int N) {
 }
 
 // one plain spline evaluation s_m(i)(r) (no gain) from the shared-memory table
-__device__ __forceinline__ float eval_axial(const ModelDev &m, const float4 *poly_s, int i, float r) {
+__device__ __forceinline__ float eval_axial(const ModelDev &m, const float4 *row, float r) {
     float t = fminf(fmaxf(fmaf(r, m.sc, m.of), -0.5f), m.tmax);
     int k;
     float v;
     split_t(t, k, v);
-    const float4 *row = poly_s + (m.n_lrf > 1 ? i * (m.n_r + 1) : 0);
     return horner(row[k], v);
 }
 
@@ -69,7 +68,7 @@ __device__ __forceinline__ float centre_eval(const ModelDev &m, const float4 *ro
 // Follows the definitions directly: Poisson A = sumS/sumL, D = 2 sum[mu - S - S ln(mu/S)];
 // chi2 w = 1/max(S,1), A = sum wSL / sum wLL, chi2 = sum w (S - A L)^2.
 template <int METHOD>
-__device__ void final_score_2d(const ModelDev &m, const float4 *sens_s, const WarpSmem2D &w, int lane,
+__device__ void final_score_2d(const ModelDev &m, const float4 *sens_s, const int *grp_s, const WarpSmem2D &w, int lane,
                                float cx, float cy, float &A_out, float &score_out) {
     double *Ld = reinterpret_cast<double *>(w.A);
     const double r_lo = (double)m.r_lo, r_hi = (double)m.r_hi;
@@ -86,9 +85,9 @@ __device__ void final_score_2d(const ModelDev &m, const float4 *sens_s, const Wa
         double t = (rc - r_lo) / hstep;
         int k = min(max((int)floor(t), 0), m.n_r - 1);
         double u = t - (double)k;
-        const double *p = m.polyd + ((size_t)(m.n_lrf > 1 ? i : 0) * m.n_r + k) * 4;
+        const double *p = m.polyd + ((size_t)grp_s[i] * m.n_r + k) * 4;
         double s = p[0] + u * (p[1] + u * (p[2] + u * p[3]));
-        double L = (m.n_lrf > 1 ? 1.0 : (double)sn.z) * s;
+        double L = (double)sn.z * s;
         double S = (double)w.SC[i].x;
         Ld[i] = L;
         sumL += L;
@@ -144,17 +143,18 @@ template <int NPT, int METHOD, bool POS>
 __global__ void __launch_bounds__(256) recon2d_kernel(const Params p) {
     extern __shared__ __align__(16) unsigned char smem[];
     const ModelDev &m = p.m;
-    const int N = m.N;
+    const int N = m.N, nr1 = m.n_r + 1;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int rows = m.n_lrf * (m.n_r + 1);
+    const int rows = m.n_lrf * nr1;
 
-    // CTA-shared tables: sensor records and the spline rows
+    // CTA-shared tables: sensor records, the spline rows, the sensors' table indices
     float4 *sens_s = reinterpret_cast<float4 *>(smem);
     float4 *poly_s = sens_s + N;
-    for (int i = threadIdx.x; i < N; i += blockDim.x) sens_s[i] = m.sens[i];
+    int *grp_s = reinterpret_cast<int *>(poly_s + rows);
+    for (int i = threadIdx.x; i < N; i += blockDim.x) { sens_s[i] = m.sens[i]; grp_s[i] = m.grp[i]; }
     for (int i = threadIdx.x; i < rows; i += blockDim.x) poly_s[i] = m.poly[i];
     __syncthreads();
-    WarpSmem2D w = carve_2d(smem + (size_t)(N + rows) * 16 + (size_t)warp * warp_smem_bytes_2d(N), N);
+    WarpSmem2D w = carve_2d(smem + cta_table_bytes(N, rows) + (size_t)warp * warp_smem_bytes_2d(N), N);
 
     // this lane's nodes: offsets from the grid centre in units of the step (exact small numbers)
     const float half = 0.5f * (float)(p.G - 1);
@@ -217,8 +217,8 @@ __global__ void __launch_bounds__(256) recon2d_kernel(const Params p) {
             for (int i = lane; i < N; i += 32) {
                 float4 sn = sens_s[i];
                 float dx = cx - sn.x, dy = cy - sn.y;
-                float s = eval_axial(m, poly_s, i, sqrtf(fmaf(dx, dx, dy * dy)));
-                sl += (m.n_lrf > 1 ? 1.f : sn.z) * s;
+                float s = eval_axial(m, poly_s + grp_s[i] * nr1, sqrtf(fmaf(dx, dx, dy * dy)));
+                sl += sn.z * s;
             }
             sl = warp_sum(sl);
             A_ref = sl > 0.f ? sumS / sl : 1.f;
@@ -249,12 +249,11 @@ __global__ void __launch_bounds__(256) recon2d_kernel(const Params p) {
                     a1[j] = a2[j] = a3[j] = a4[j] = 0.f;
                     bad[j] = false;
                 }
-                const int row_stride = m.n_lrf > 1 ? m.n_r + 1 : 0;
-                const float4 *row = poly_s;
 #pragma unroll 2
-                for (int i = 0; i < N; ++i, row += row_stride) {
+                for (int i = 0; i < N; ++i) {
                     const float4 a = w.A[i];
-                    const float g = m.n_lrf > 1 ? 1.f : sens_s[i].z;
+                    const float4 *row = poly_s + grp_s[i] * nr1;
+                    const float g = sens_s[i].z;
 #pragma unroll
                     for (int j = 0; j < NPT; ++j) {
                         float dx = x[j] - a.x, dy = y[j] - a.y;
@@ -322,9 +321,9 @@ __global__ void __launch_bounds__(256) recon2d_kernel(const Params p) {
                         int k0;
                         float v0, r0c;
                         float4 q;
-                        float s0 = centre_eval(m, poly_s + (m.n_lrf > 1 ? i * (m.n_r + 1) : 0),
+                        float s0 = centre_eval(m, poly_s + grp_s[i] * nr1,
                                                sqrtf(fmaf(dx0, dx0, dy0 * dy0)), k0, v0, r0c, q);
-                        float L0 = (m.n_lrf > 1 ? 1.f : sn.z) * s0;
+                        float L0 = sn.z * s0;
                         float S = w.SC[i].x, wi = 1.f / fmaxf(S, 1.f);
                         P0 = fmaf(wi * S, L0, P0);
                         Q0 = fmaf(wi * L0, L0, Q0);
@@ -342,11 +341,11 @@ __global__ void __launch_bounds__(256) recon2d_kernel(const Params p) {
                     if (act) {
                         float4 sn = sens_s[i];
                         float S = w.SC[i].x;
-                        float g = m.n_lrf > 1 ? 1.f : sn.z;
+                        float g = sn.z;
                         float dx0 = cx - sn.x, dy0 = cy - sn.y;
                         float r0sq = fmaf(dx0, dx0, dy0 * dy0);
                         float r0 = sqrtf(r0sq);
-                        const float4 *row = poly_s + (m.n_lrf > 1 ? i * (m.n_r + 1) : 0);
+                        const float4 *row = poly_s + grp_s[i] * nr1;
                         int k0;
                         float v0, r0c;
                         float4 q;
@@ -487,7 +486,7 @@ __global__ void __launch_bounds__(256) recon2d_kernel(const Params p) {
 
         // ---- a6: FP64 energy and score at the final node, store --------------
         float A_fin, score_fin;
-        final_score_2d<METHOD>(m, sens_s, w, lane, cx, cy, A_fin, score_fin);
+        final_score_2d<METHOD>(m, sens_s, grp_s, w, lane, cx, cy, A_fin, score_fin);
         if (lane == 0) {
             reinterpret_cast<float4 *>(p.out_xyzA)[e] = make_float4(cx, cy, 0.f, A_fin);
             p.out_score[e] = score_fin;

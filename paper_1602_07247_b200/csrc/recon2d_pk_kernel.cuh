@@ -9,14 +9,14 @@ __global__ void __launch_bounds__(256, (NPT <= 3 ? 3 : 2)) recon2d_pk_kernel(con
     extern __shared__ __align__(16) unsigned char smem[];
     const ModelDev &m = p.m;
     const int N = m.N, nr1 = m.n_r + 1;
-    const bool indiv = m.n_lrf > 1;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int rows = m.n_lrf * nr1;
 
     // ---- CTA-shared tables ----
     float4 *sens_s = reinterpret_cast<float4 *>(smem);
     float4 *poly_s = sens_s + N;
-    for (int i = threadIdx.x; i < N; i += blockDim.x) sens_s[i] = m.sens[i];
+    int *grp_s = reinterpret_cast<int *>(poly_s + rows);
+    for (int i = threadIdx.x; i < N; i += blockDim.x) { sens_s[i] = m.sens[i]; grp_s[i] = m.grp[i]; }
     for (int i = threadIdx.x; i < rows; i += blockDim.x) poly_s[i] = m.poly[i];
     __syncthreads();
     WarpSmemPk w = carve_pk(smem + (cta_smem_bytes_pk(N, rows) + 15) / 16 * 16 +
@@ -134,8 +134,8 @@ __global__ void __launch_bounds__(256, (NPT <= 3 ? 3 : 2)) recon2d_pk_kernel(con
             for (int i = lane; i < N; i += 32) {
                 float4 sn = sens_s[i];
                 float dx = cx - sn.x, dy = cy - sn.y;
-                float s = eval_axial(m, poly_s, i, sqrt_approx(fmaf(dx, dx, dy * dy)));
-                if (w.SC[i].y == w.SC[i].y) sl += (indiv ? 1.f : sn.z) * s;
+                float s = eval_axial(m, poly_s + grp_s[i] * nr1, sqrt_approx(fmaf(dx, dx, dy * dy)));
+                if (w.SC[i].y == w.SC[i].y) sl += sn.z * s;
             }
             sl = warp_sum(sl);
             A_ref = sl > 0.f ? sumS * rcp_approx(sl) : 1.f;   // only conditions the plain score
@@ -186,7 +186,7 @@ __global__ void __launch_bounds__(256, (NPT <= 3 ? 3 : 2)) recon2d_pk_kernel(con
         WarpSmem2D w2;               // final_score_2d needs N doubles of scratch (D[0..1]) and SC
         w2.A = w.D[0];
         w2.SC = w.SC;
-        final_score_2d<METHOD>(m, sens_s, w2, lane, cx, cy, A_fin, score_fin);
+        final_score_2d<METHOD>(m, sens_s, grp_s, w2, lane, cx, cy, A_fin, score_fin);
         if (lane == 0) {
             reinterpret_cast<float4 *>(p.out_xyzA)[e] = make_float4(cx, cy, 0.f, A_fin);
             p.out_score[e] = score_fin;

@@ -14,7 +14,10 @@ constexpr int kMagicBits = 0x4B400000;    // bit pattern of kMagic; low bits of 
 
 // LRF model as the kernels see it (device pointers; built once in ants_lrf_create, step a0).
 struct ModelDev {
-    const float4 *sens;     // [N] {X, Y, g, 1/g}
+    const float4 *sens;     // [N] {X, Y, gL, 1/g}: gL scales the table into L_i (the relative gain for a shared or
+                            //   group profile, 1 for per-sensor tables); 1/g weights the centroid
+    const int *grp;         // [N] table index of every sensor (0 for one shared profile, i for per-sensor tables,
+                            //   the group index for a grouped model)
     const float4 *poly;     // axial: [n_lrf][n_r + 1] rows {q0,q1,q2,q3}: s = q0 + v(q1 + v(q2 + v q3)),
                             //   v = t - round(t - 0.5) - 0.5 in [-0.5, 0.5], t = (r - r_lo) * sc;
                             //   row n_r is the constant extension s(r_hi).
@@ -194,6 +197,11 @@ __device__ __forceinline__ float4 lds128(unsigned addr) {
     float4 v;
     asm("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
     return v;
+}
+
+// CTA-shared model tables of the axial kernels: sens_s [N] float4, poly_s [rows] float4, grp_s [N] int (padded)
+__host__ __device__ inline size_t cta_table_bytes(int N, int rows) {
+    return (size_t)(N + rows) * 16 + ((size_t)N * 4 + 15) / 16 * 16;
 }
 
 __device__ __forceinline__ float horner(const float4 p, float v) {

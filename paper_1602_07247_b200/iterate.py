@@ -34,7 +34,6 @@ def iterate_response(cfg, signals, n_cycles: int, score_max: float = float("nan"
             nxt.coeffs = c[:, None, :].astype(np.float32)
             if refit_gains and cur.n_lrf == 1:
                 g, _ = recon.ants_lrf_fit_gains(cur.sensor_xy, cur.knots, c[0], signals, xyzA)
-                g = np.where(np.isfinite(g) & (g > 0), g, cur.gains)
-                nxt.gains = (g / g.mean() * np.asarray(cur.gains).mean()).astype(np.float32)   # gains are relative
+                nxt.gains = recon.ants_gains_renormalise(g, cur.gains)     # gains are relative (R29)
         cur = nxt
         yield cycle, cur, n_pass

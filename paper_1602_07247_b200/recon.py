@@ -54,6 +54,18 @@ def load():
     vp, i32p = C.c_void_p, C.POINTER(C.c_int32)
     lib.ants_lrf_create.restype = C.c_int
     lib.ants_lrf_create.argtypes = [vp, vp, vp, vp, C.POINTER(LrfDims), C.POINTER(vp)]
+    lib.ants_lrf_create_grouped.restype = C.c_int
+    lib.ants_lrf_create_grouped.argtypes = [vp, vp, vp, vp, vp, C.POINTER(LrfDims), C.POINTER(vp)]
+    lib.ants_group_by_radius.restype = C.c_int
+    lib.ants_group_by_radius.argtypes = [vp, C.c_int32, C.c_float, vp, i32p]
+    lib.ants_gains_renormalise.restype = C.c_int
+    lib.ants_gains_renormalise.argtypes = [vp, vp, C.c_int32, vp]
+    lib.ants_lrf_n_sensors.restype = C.c_int32
+    lib.ants_lrf_n_sensors.argtypes = [vp]
+    lib.ants_plan_kernel_name.restype = C.c_int
+    lib.ants_plan_kernel_name.argtypes = [vp, C.POINTER(GridParams), C.c_int32, C.c_char_p, C.c_int32]
+    lib.ants_probe_throughput.restype = C.c_int
+    lib.ants_probe_throughput.argtypes = [C.c_int32, C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_double)]
     lib.ants_reconstruct.restype = C.c_int
     lib.ants_reconstruct.argtypes = [vp, vp, C.c_int64, C.POINTER(GridParams), C.c_int32, vp, vp, vp]
     lib.ants_reconstruct_trace.restype = C.c_int
@@ -106,6 +118,43 @@ def ants_lrf_create(sensor_xy, gains, knots, coeffs, dims: LrfDims) -> int:
     if rc != 0:
         raise AntsError(rc, "ants_lrf_create")
     return out.value
+
+
+def ants_lrf_create_grouped(sensor_xy, gains, group, knots, coeffs, dims: LrfDims) -> int:
+    """Grouped model (include/ants_recon.h): dims.n_lrf = number of groups, group int32 [N],
+    coeffs [n_groups][n_int_r + 3].  -> opaque handle (int)."""
+    xy, kn, co = _f32(sensor_xy), _f32(knots), _f32(coeffs)
+    g = None if gains is None else _f32(gains)
+    gr = np.ascontiguousarray(np.asarray(group, dtype=np.int32))
+    out = C.c_void_p()
+    rc = load().ants_lrf_create_grouped(xy.ctypes.data, None if g is None else g.ctypes.data, gr.ctypes.data,
+                                        kn.ctypes.data, co.ctypes.data, C.byref(dims), C.byref(out))
+    if rc != 0:
+        raise AntsError(rc, "ants_lrf_create_grouped")
+    return out.value
+
+
+def ants_group_by_radius(sensor_xy, tol: float = 1e-3):
+    """Distance-from-centre sensor groups (include/ants_recon.h).  -> (group int32 [N], n_groups)."""
+    xy = _f32(sensor_xy).reshape(-1, 2)
+    group = np.zeros(xy.shape[0], np.int32)
+    n = C.c_int32(0)
+    rc = load().ants_group_by_radius(xy.ctypes.data, xy.shape[0], float(tol), group.ctypes.data, C.byref(n))
+    if rc != 0:
+        raise AntsError(rc, "ants_group_by_radius")
+    return group, int(n.value)
+
+
+def ants_gains_renormalise(gains_new, gains_prev):
+    """Relative gains carried on at the scale of the previous set (include/ants_recon.h).  -> float32 [N]."""
+    gn, gp = _f32(gains_new).reshape(-1), _f32(gains_prev).reshape(-1)
+    if gn.size != gp.size:
+        raise ValueError("ants_gains_renormalise: size mismatch")
+    out = np.zeros(gn.size, np.float32)
+    rc = load().ants_gains_renormalise(gn.ctypes.data, gp.ctypes.data, gn.size, out.ctypes.data)
+    if rc != 0:
+        raise AntsError(rc, "ants_gains_renormalise")
+    return out
 
 
 def ants_lrf_set_selection(handle, passive=None, signal_min=float("nan"), dist_max=float("nan")) -> None:
@@ -208,41 +257,30 @@ def ants_lrf_fit_gains(sensor_xy, knots, coeffs, signals, xyzA, stream=None):
     return gains, used
 
 
-def group_by_radius(sensor_xy, tol: float = 1e-3):
-    """Sensor groups "according to the distance from the sensor center to the detector center":
-    sensors are sorted by their distance from the origin and a new group starts wherever the distance exceeds
-    the group's first one by more than tol (mm).  -> (group int32 [N], n_groups), for ants_lrf_fit_axial(group=)."""
-    xy = _f32(sensor_xy).reshape(-1, 2).astype(np.float64)
-    dist = np.sqrt((xy * xy).sum(axis=1))
-    order = np.argsort(dist, kind="stable")
-    group = np.empty(len(dist), np.int32)
-    current, anchor = -1, -np.inf
-    for i in order:
-        if dist[i] - anchor > tol:
-            current, anchor = current + 1, dist[i]
-        group[i] = current
-    return group, current + 1
-
-
-def expand_groups(coeffs, group, gains):
-    """A grouped response as one table per sensor (what ants_lrf_create takes with n_lrf = N): the table of
-    sensor i is its group's profile times its relative gain.  -> float32 [N][1][n_int_r + 3]."""
-    c = np.asarray(coeffs, np.float64)[np.asarray(group)] * np.asarray(gains, np.float64)[:, None]
-    return c.astype(np.float32)[:, None, :]
-
-
 def ants_destroy(handle) -> None:
     load().ants_destroy(handle)
 
 
 def ants_reconstruct(handle, signals, grid: GridParams, method: int, out_xyzA, out_score,
                      stream=None, out_path=None) -> None:
-    """signals/out_*: CUDA torch tensors (float32, contiguous; out_path int16/uint16 [E][K])."""
+    """signals [E][N], out_xyzA [E][4], out_score [E]: contiguous float32 CUDA tensors;
+    out_path (optional) [E][K] int16/uint16.  Shapes and dtypes are checked here: the C side only sees pointers."""
     import torch
-    E = int(signals.shape[0]) if signals.dim() == 2 else 0
-    for t in (signals, out_xyzA, out_score) + (() if out_path is None else (out_path,)):
-        if not (t.is_cuda and t.is_contiguous()):
-            raise ValueError("ants_reconstruct needs contiguous CUDA tensors")
+    N = int(load().ants_lrf_n_sensors(handle))
+    if signals.dim() != 2 or int(signals.shape[1]) != N:
+        raise ValueError(f"ants_reconstruct: signals must be [E][{N}]")
+    E = int(signals.shape[0])
+    for t in (signals, out_xyzA, out_score):
+        if not (t.is_cuda and t.is_contiguous() and t.dtype == torch.float32):
+            raise ValueError("ants_reconstruct needs contiguous float32 CUDA tensors")
+    if tuple(out_xyzA.shape) != (E, 4) or tuple(out_score.shape) != (E,):
+        raise ValueError("ants_reconstruct: out_xyzA must be [E][4] and out_score [E]")
+    if out_path is not None:
+        if not (out_path.is_cuda and out_path.is_contiguous() and out_path.element_size() == 2 and
+                not out_path.dtype.is_floating_point and tuple(out_path.shape) == (E, int(grid.n_iter))):
+            raise ValueError("ants_reconstruct: out_path must be a contiguous 16-bit integer CUDA tensor [E][K]")
+    if len({t.device for t in (signals, out_xyzA, out_score)}) != 1:
+        raise ValueError("ants_reconstruct: tensors on different devices")
     st = torch.cuda.current_stream().cuda_stream if stream is None else int(stream)
     if out_path is None:
         rc = load().ants_reconstruct(handle, signals.data_ptr(), E, C.byref(grid), int(method),
@@ -254,15 +292,41 @@ def ants_reconstruct(handle, signals, grid: GridParams, method: int, out_xyzA, o
         raise AntsError(rc, "ants_reconstruct")
 
 
+def _host_f32(a, shape, what):
+    """pointer of a C-contiguous float32 host buffer (numpy array or CPU torch tensor) of the given shape"""
+    if hasattr(a, "data_ptr"):
+        import torch
+        ok = (not a.is_cuda) and a.is_contiguous() and a.dtype == torch.float32 and tuple(a.shape) == shape
+        ptr = a.data_ptr()
+    else:
+        ok = isinstance(a, np.ndarray) and a.flags["C_CONTIGUOUS"] and a.dtype == np.float32 and a.shape == shape
+        ptr = a.ctypes.data if ok else 0
+    if not ok:
+        raise ValueError(f"ants_reconstruct_host: {what} must be a C-contiguous float32 host buffer of shape {shape}")
+    return ptr
+
+
 def ants_reconstruct_host(handle, signals, grid: GridParams, method: int, out_xyzA, out_score,
                           chunk_events: int = 0) -> None:
-    """signals/out_*: host buffers (numpy arrays or CPU torch tensors, pinned for async copies)."""
-    def ptr(a):
-        return a.data_ptr() if hasattr(a, "data_ptr") else a.ctypes.data
-    rc = load().ants_reconstruct_host(handle, ptr(signals), int(signals.shape[0]), C.byref(grid), int(method),
-                                      ptr(out_xyzA), ptr(out_score), int(chunk_events))
+    """signals [E][N], out_xyzA [E][4], out_score [E]: host buffers (numpy arrays or CPU torch tensors,
+    pinned for asynchronous copies)."""
+    N = int(load().ants_lrf_n_sensors(handle))
+    E = int(signals.shape[0])
+    ps = _host_f32(signals, (E, N), "signals")
+    px = _host_f32(out_xyzA, (E, 4), "out_xyzA")
+    pc = _host_f32(out_score, (E,), "out_score")
+    rc = load().ants_reconstruct_host(handle, ps, E, C.byref(grid), int(method), px, pc, int(chunk_events))
     if rc != 0:
         raise AntsError(rc, "ants_reconstruct_host")
+
+
+def ants_probe_throughput(kind: int, iters: int = 4096):
+    """Throughput micro-benchmark (include/ants_recon.h).  -> (scalar results per second, milliseconds)."""
+    ops, ms = C.c_double(0.0), C.c_double(0.0)
+    rc = load().ants_probe_throughput(int(kind), int(iters), C.byref(ops), C.byref(ms))
+    if rc != 0:
+        raise AntsError(rc, "ants_probe_throughput")
+    return ops.value, ms.value
 
 
 def plan_info(handle, grid: GridParams, method: int) -> dict:
@@ -271,7 +335,11 @@ def plan_info(handle, grid: GridParams, method: int) -> dict:
     if rc != 0:
         raise AntsError(rc, "ants_plan_info")
     keys = ("first_diff_iter", "nodes_per_lane", "warps_per_cta", "ctas_per_sm", "smem_bytes")
-    return dict(zip(keys, (x.value for x in v)))
+    out = dict(zip(keys, (x.value for x in v)))
+    name = C.create_string_buffer(96)
+    if load().ants_plan_kernel_name(handle, C.byref(grid), int(method), name, 96) == 0:
+        out["kernel"] = name.value.decode()
+    return out
 
 
 class Reconstructor:
@@ -283,7 +351,11 @@ class Reconstructor:
         self.grid = GridParams(cfg.dim, cfg.nodes_per_axis, cfg.step0_xy, cfg.step0_z, cfg.factor,
                                cfg.n_iter, int(getattr(cfg, "seed_mode", 0)), cfg.z_seed)
         self.method = int(cfg.method)
-        self.handle = ants_lrf_create(cfg.sensor_xy, cfg.gains, cfg.knots, cfg.coeffs, self.dims)
+        group = getattr(cfg, "group", None)
+        if group is None:
+            self.handle = ants_lrf_create(cfg.sensor_xy, cfg.gains, cfg.knots, cfg.coeffs, self.dims)
+        else:
+            self.handle = ants_lrf_create_grouped(cfg.sensor_xy, cfg.gains, group, cfg.knots, cfg.coeffs, self.dims)
         passive = getattr(cfg, "passive", None)
         smin, dmax = getattr(cfg, "signal_min", float("nan")), getattr(cfg, "dist_max", float("nan"))
         if passive is not None or smin == smin or dmax == dmax:

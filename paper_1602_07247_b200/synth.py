@@ -139,6 +139,8 @@ class Config:
     signal_min: float = float("nan")         # NaN = off
     dist_max: float = float("nan")           # NaN = off
     seed_mode: int = 0                       # 0 centroid, 1 strongest sensor
+    # photosensor grouping: table index of every sensor, n_lrf = number of groups; None = off
+    group: Optional[np.ndarray] = None
 
     @property
     def n_sensors(self) -> int:
@@ -294,7 +296,9 @@ def generate_events(cfg: Config, n_events: Optional[int] = None, device="cpu",
             else:
                 i0 = t.floor().clamp(max=_TABLE_R - 2).long()
                 w = t - i0
-                rows = torch.arange(N, device=dev)[None, :].expand(m, N)
+                tables = (torch.arange(N, device=dev) if cfg.group is None
+                          else torch.from_numpy(np.asarray(cfg.group, np.int64)).to(dev))
+                rows = tables[None, :].expand(m, N)
                 prof = tab[rows, i0] * (1 - w) + tab[rows, i0 + 1] * w
         else:
             z_lo, z_hi = float(cfg.knots[2]), float(cfg.knots[3])

@@ -81,12 +81,29 @@ def test_invalid_model_arguments_are_rejected_before_any_gpu_work():
         assert ei.value.status == -1, kw
 
 
-def test_distance_grouping_helper_agrees_with_the_oracle():
+def test_distance_grouping_in_the_library_agrees_with_the_oracle():
+    """ants_group_by_radius is host-only: it runs without a GPU.  The oracle's grouping (oracle/fit.py, pinned by
+    hex ring counts in tests/test_oracle_fit.py) is the reference."""
     from oracle import fit as ofit
     for xy in (synth.hex_array(1, 30.0), synth.hex_array(3, 30.0), synth.hex_array(6, 25.0), synth.square_array(8, 6.0)):
-        g, n = recon.group_by_radius(xy)
+        g, n = recon.ants_group_by_radius(xy)
         g0, n0 = ofit.group_by_radius(xy)
         assert n == n0 and np.array_equal(g, g0)
-    c = np.arange(8, dtype=np.float64).reshape(2, 4)
-    out = recon.expand_groups(c, [0, 1, 1], [1.0, 2.0, 0.5])
-    assert out.shape == (3, 1, 4) and np.array_equal(out[1, 0], 2.0 * c[1]) and np.array_equal(out[2, 0], 0.5 * c[1])
+    with pytest.raises(recon.AntsError):
+        recon.ants_group_by_radius(synth.hex_array(1, 30.0), tol=-1.0)
+
+
+def test_gain_renormalisation_in_the_library_agrees_with_the_oracle():
+    from oracle import fit as ofit
+    rng = np.random.default_rng(5)
+    prev = rng.uniform(0.5, 1.5, 37).astype(np.float32)
+    new = (prev * rng.uniform(0.9, 1.1, 37) * 3.7).astype(np.float32)
+    new[[3, 11]] = np.nan
+    new[20] = -0.25
+    out = recon.ants_gains_renormalise(new, prev)
+    ref = ofit.renormalise_gains(new, prev)
+    assert np.array_equal(out, ref)
+    bad = prev.copy()
+    bad[0] = 0.0
+    with pytest.raises(recon.AntsError):
+        recon.ants_gains_renormalise(new, bad)

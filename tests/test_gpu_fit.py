@@ -176,10 +176,11 @@ def test_event_filter_is_bit_exact_and_feeds_the_fit():
 
 
 def test_grouped_fit_parity_and_use_in_reconstruction():
-    """ants_lrf_fit_axial_grouped vs the oracle (R28) with the distance groups of the 19-PMT array, then the
-    grouped response expanded to one table per sensor drives a reconstruction that agrees with the oracle's."""
+    """ants_lrf_fit_axial_grouped vs the oracle (R28) with the distance groups of the 19-PMT array; the grouped
+    response then goes straight into ants_lrf_create_grouped (one table per group in shared memory) and drives a
+    reconstruction in parity with the oracle's grouped model."""
     cfg, ev, xyzA = _reconstructed(2, 60_011)
-    group, n_groups = recon.group_by_radius(cfg.sensor_xy)
+    group, n_groups = recon.ants_group_by_radius(cfg.sensor_xy)
     assert n_groups == 4 and np.array_equal(group, ofit.group_by_radius(cfg.sensor_xy)[0])
     knots = np.array([0.0, 55.0], np.float32)        # the range the central PMT sees with events inside 60 mm
     c, used = recon.ants_lrf_fit_axial(cfg.sensor_xy, cfg.gains, knots, n_groups, cfg.n_int_r, ev["signals"], xyzA,
@@ -191,17 +192,44 @@ def test_grouped_fit_parity_and_use_in_reconstruction():
     with pytest.raises(recon.AntsError):
         recon.ants_lrf_fit_axial(cfg.sensor_xy, cfg.gains, knots, n_groups, cfg.n_int_r, ev["signals"], xyzA,
                                  group=np.full(cfg.n_sensors, 7))
-    # expand: table of sensor i = its group's profile times its gain
     import parity_rules
-    exp = synth.make_config(2)
-    exp.n_lrf = cfg.n_sensors
-    exp.knots = knots
-    exp.coeffs = recon.expand_groups(c, group, cfg.gains)
-    exp.gains = np.ones(cfg.n_sensors, np.float32)
+    grp = synth.make_config(2)
+    grp.n_lrf = n_groups
+    grp.group = group
+    grp.knots = knots
+    grp.coeffs = c[:, None, :].astype(np.float32)
     sub = ev["signals"][:8001].contiguous()
-    r = recon.Reconstructor(exp)
+    r = recon.Reconstructor(grp)
     try:
+        assert "recon2d_pk_kernel" in r.plan()["kernel"]
         out = [t.cpu().numpy() for t in r(sub, trace=True)]
     finally:
         r.close()
-    parity_rules.assert_parity(parity_rules.compare(exp, sub.cpu().numpy(), *out), "grouped response expanded")
+    parity_rules.assert_parity(parity_rules.compare(grp, sub.cpu().numpy(), *out), "grouped response")
+    with pytest.raises(recon.AntsError) as ei:           # a group index outside 0 .. n_groups-1
+        recon.ants_lrf_create_grouped(grp.sensor_xy, grp.gains, np.full(cfg.n_sensors, n_groups), grp.knots, grp.coeffs,
+                                      recon.LrfDims(cfg.n_sensors, n_groups, 1, cfg.n_int_r, 0))
+    assert ei.value.status == -1
+
+
+@pytest.mark.parametrize("method,seed", [(0, 1), (1, 2), (2, 3)])
+def test_grouped_model_on_random_groups(method, seed):
+    """Random groups, gains and group profiles (chi-square variants included): a grouped handle reconstructs in
+    parity with the oracle's grouped model."""
+    import parity_rules
+    rng = np.random.default_rng(seed)
+    cfg = synth.make_config(5)
+    n_groups = 5
+    cfg.group = rng.integers(0, n_groups, cfg.n_sensors).astype(np.int32)
+    cfg.n_lrf = n_groups
+    base = cfg.coeffs[0, 0].astype(np.float64)
+    cfg.coeffs = (base[None, :] * rng.uniform(0.7, 1.3, (n_groups, 1))).astype(np.float32)[:, None, :]
+    cfg.method = method
+    cfg.n_iter = 10
+    ev = synth.generate_events(cfg, 3001, device="cuda:0")
+    r = recon.Reconstructor(cfg)
+    try:
+        out = [t.cpu().numpy() for t in r(ev["signals"], trace=True)]
+    finally:
+        r.close()
+    parity_rules.assert_parity(parity_rules.compare(cfg, ev["signals"].cpu().numpy(), *out), f"random groups m{method}")

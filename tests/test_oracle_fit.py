@@ -211,3 +211,59 @@ def test_grouped_fit_is_the_lstsq_of_each_group():
     one, _ = fit.fit_axial(cfg.sensor_xy, cfg.gains, cfg.knots, 1, cfg.n_int_r, sig, pos)
     one_g, _ = fit.fit_axial(cfg.sensor_xy, cfg.gains, cfg.knots, 1, cfg.n_int_r, sig, pos, group=np.zeros(cfg.n_sensors, np.int32))
     assert np.array_equal(one, one_g)
+
+
+def test_grouped_model_is_the_expanded_model():
+    """R28: L_i = g_i s_group(i)(r).  Pin: the oracle's grouped LRF equals the library-evaluated (scipy) group
+    profile times the gain, and a grouped model reconstructs exactly like the same response written out as one
+    table per sensor (coefficients of the group times the gain, computed here in float32-exact numbers)."""
+    from oracle import oracle
+    rng = np.random.default_rng(11)
+    cfg = synth.make_config(2)
+    n_groups = 3
+    group = rng.integers(0, n_groups, cfg.n_sensors).astype(np.int32)
+    gains = (2.0 ** rng.integers(-1, 2, cfg.n_sensors)).astype(np.float32)       # powers of two: exact products
+    coeffs = (cfg.coeffs[0, 0][None, :] * np.array([1.0, 0.75, 1.25], np.float32)[:, None]).astype(np.float32)
+    grouped = oracle.Model(cfg.sensor_xy, gains, cfg.knots, coeffs, n_groups, 1, cfg.n_int_r, 0, group=group)
+    expanded = oracle.Model(cfg.sensor_xy, np.ones(cfg.n_sensors, np.float32), cfg.knots,
+                            (coeffs[group] * gains[:, None]).astype(np.float32), cfg.n_sensors, 1, cfg.n_int_r, 0)
+    for i in range(cfg.n_sensors):
+        for x, y in ((3.0, -7.0), (40.0, 22.0), (-81.0, 5.5)):
+            r = np.hypot(x - float(cfg.sensor_xy[i, 0]), y - float(cfg.sensor_xy[i, 1]))
+            lib = float(gains[i]) * float(synth.eval_axial(coeffs[group[i]], 0.0, 90.0, np.array([r]))[0])
+            assert abs(grouped.lrf(i, x, y) - lib) <= 1e-12 * abs(lib)
+            assert grouped.lrf(i, x, y) == expanded.lrf(i, x, y)
+    sig = synth.generate_events(cfg, 300)["signals"].numpy()
+    grid = oracle.grid_from_config(cfg)
+    for method in (0, 1):
+        a = oracle.reconstruct(grouped, sig, grid, method, trace=True)
+        b = oracle.reconstruct(expanded, sig, grid, method, trace=True)
+        # the centroid weighs by 1/g in the grouped model and by 1 in the expanded one: compare from the same start
+        assert np.array_equal(a["idx"][:, 1:] >= 0, b["idx"][:, 1:] >= 0)
+    ones = oracle.Model(cfg.sensor_xy, np.ones(cfg.n_sensors, np.float32), cfg.knots, coeffs, n_groups, 1, cfg.n_int_r, 0, group=group)
+    exp1 = oracle.Model(cfg.sensor_xy, np.ones(cfg.n_sensors, np.float32), cfg.knots, coeffs[group].astype(np.float32),
+                        cfg.n_sensors, 1, cfg.n_int_r, 0)
+    for method in (0, 1, 2):
+        a = oracle.reconstruct(ones, sig, grid, method, trace=True)
+        b = oracle.reconstruct(exp1, sig, grid, method, trace=True)
+        assert np.array_equal(a["xyzA"], b["xyzA"]) and np.array_equal(a["score"], b["score"]) and np.array_equal(a["idx"], b["idx"])
+
+
+def test_gain_renormalisation_keeps_the_mean_and_the_ratios():
+    """R29 pins: the mean of the result equals the mean of the previous set; ratios between re-evaluated sensors
+    are those of the new estimates; a sensor without an estimate keeps its previous gain (before the common
+    scaling); an all-usable set that already has the right mean comes back unchanged."""
+    rng = np.random.default_rng(3)
+    prev = rng.uniform(0.6, 1.4, 19).astype(np.float32)
+    new = (prev.astype(np.float64) * rng.uniform(0.8, 1.2, 19) * 5.0).astype(np.float32)
+    new[4] = np.nan
+    new[9] = 0.0
+    out = fit.renormalise_gains(new, prev).astype(np.float64)
+    assert abs(out.mean() - prev.astype(np.float64).mean()) <= 1e-6
+    ok = np.ones(19, bool)
+    ok[[4, 9]] = False
+    ratio = out[ok] / new[ok].astype(np.float64)
+    assert np.ptp(ratio) <= 2e-7 * ratio.mean()
+    assert abs(out[4] / prev[4] - ratio.mean()) <= 2e-7 * ratio.mean() and abs(out[9] / prev[9] - ratio.mean()) <= 2e-7 * ratio.mean()
+    same = fit.renormalise_gains(prev, prev)
+    assert np.abs(same.astype(np.float64) - prev).max() <= 1.2e-7 * prev.max()

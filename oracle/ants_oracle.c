@@ -32,6 +32,10 @@
  * CUDA library, widened; sums run left to right in sensor order; no blocking,
  * no fusion, no reordering.  OpenMP only splits the independent events.
  *
+ * XY, Composite and Sliced parameterisations (R30-R33) are pinned in
+ * tests/test_oracle_xy.py against scipy design matrices, plane/midplane values and
+ * a numpy argmin.
+ *
  * Pins (tests/test_oracle_pins.py): partition of unity, polynomial
  * reproduction by blossoming, scipy BSpline agreement, separable tensor
  * product, centroid special cases, energy vs 1-D minimisation, D >= 0 and
@@ -53,7 +57,8 @@
 typedef struct {
     int32_t n_sensors;       /* N */
     int32_t n_lrf;           /* 1: shared profile scaled by gains[i]; N: individual */
-    int32_t lrf_dim;         /* 1: L(r); 2: L(r,z) tensor product */
+    int32_t lrf_dim;         /* LRF parameterisation (section 6.1): 1 Axial L(r); 2 Axial+Z L(r,z)
+                                tensor product; 3 XY; 4 Composite = Axial + XY; 5 Sliced = XY LRFs on z planes */
     int32_t n_int_r;         /* uniform intervals in r, n_int_r+3 coefficients */
     int32_t n_int_z;         /* uniform intervals in z (0 if lrf_dim==1) */
     const float *sensor_xy;  /* [N][2] */
@@ -70,6 +75,15 @@ typedef struct {
      * the same LRF for all photosensors within it ... a scaling parameter (relative gain) has to be assigned
      * to each of them"); reading R28.  NULL = no explicit grouping (n_lrf == 1 or n_lrf == N as above) */
     const int32_t *group;    /* [N] table index 0..n_lrf-1 of every sensor, or NULL */
+    /* XY-type parameterisations (lrf_dim 3, 4, 5; "XY LRF", "Composite LRF",
+     * PAPER.md:396 "Sliced LRF"); readings R30-R33 */
+    int32_t n_int_x, n_int_y;  /* uniform intervals of the XY spline in the sensor-local coordinates (u, v) */
+    int32_t n_planes;          /* Sliced: number of z planes (>= 2), uniformly spaced from z_lo to z_hi; else 0 */
+    const float *knots_xy;     /* {u_lo, u_hi, v_lo, v_hi} and, for Sliced, {z_lo, z_hi} after them */
+    const float *coeffs_xy;    /* [n_lrf][n_planes or 1][n_int_y+3][n_int_x+3], u fastest */
+    const float *xform;        /* [N][4] or NULL: T_i row-major, (u, v) = T_i (p_xy - P_i) (R33: a sensor that a
+                                  rotation/reflection of the array maps onto its group's reference sensor sees the
+                                  reference LRF in a frame turned with it); NULL = identity */
 } oracle_model_t;
 
 typedef struct {
@@ -128,21 +142,67 @@ double oracle_spline2(const float *c, int nr, int nz, double r_lo, double r_hi,
 
 /* ---- LRF of sensor i at (x,y,z): L_i = g*_i s_m(i)(|p_xy - P_i|[, z])
  * (PAPER.md:388 axial; PAPER.md:394 axial+z; PAPER.md:400 shared profile +
- * relative gain; PAPER.md:402-406 sensor groups) ----------------------------- */
+ * relative gain; PAPER.md:402-406 sensor groups; PAPER.md:388-396 XY, Composite
+ * and Sliced parameterisations) ---------------------------------------------- */
 double oracle_lrf(const oracle_model_t *m, int i, double x, double y, double z)
 {
     double dx = x - (double)m->sensor_xy[2 * i], dy = y - (double)m->sensor_xy[2 * i + 1];
     double r = sqrt(dx * dx + dy * dy);
-    int per = (m->n_int_r + 3) * (m->lrf_dim == 2 ? m->n_int_z + 3 : 1);
     /* table and scale of sensor i: a group's profile times the sensor's relative gain;
      * one shared profile is the one-group case; a table of the sensor's own is not scaled */
-    const float *c = m->coeffs + (size_t)(m->group ? m->group[i] : (m->n_lrf == 1 ? 0 : i)) * per;
+    size_t tab = (size_t)(m->group ? m->group[i] : (m->n_lrf == 1 ? 0 : i));
     double g = (m->group || m->n_lrf == 1) ? (double)m->gains[i] : 1.0;
-    double s = m->lrf_dim == 1
-        ? oracle_spline1(c, m->n_int_r, m->knots[0], m->knots[1], r)
-        : oracle_spline2(c, m->n_int_r, m->n_int_z, m->knots[0], m->knots[1],
-                         m->knots[2], m->knots[3], r, z);
+    double s = 0.0;
+    if (m->lrf_dim == 1 || m->lrf_dim == 4) {           /* Axial, or the axial component of Composite */
+        const float *c = m->coeffs + tab * (size_t)(m->n_int_r + 3);
+        s += oracle_spline1(c, m->n_int_r, m->knots[0], m->knots[1], r);
+    }
+    if (m->lrf_dim == 2) {                              /* Axial+Z */
+        const float *c = m->coeffs + tab * (size_t)((m->n_int_r + 3) * (m->n_int_z + 3));
+        s += oracle_spline2(c, m->n_int_r, m->n_int_z, m->knots[0], m->knots[1], m->knots[2], m->knots[3], r, z);
+    }
+    if (m->lrf_dim >= 3) {
+        /* R30: "LRF is a function of X and Y and no other type of symmetry can be assumed":
+         * a tensor-product cubic B-spline of the position relative to the sensor, (u, v) = T_i (p_xy - P_i),
+         * each coordinate clamped into the tabulated range like r (R5).
+         * R31: "a sum of two components: an Axial LRF and an XY LRF".
+         * R32: "a set of several XY LRFs, each defined on a specific Z plane.  The LRF values for the points
+         * between the planes are calculated using linear interpolation of the LRF values at two closest
+         * points from two closest planes": planes z_p = z_lo + p dz, p = 0 .. n_planes-1. */
+        double u = dx, v = dy;
+        if (m->xform) {
+            const float *T = m->xform + 4 * i;
+            u = (double)T[0] * dx + (double)T[1] * dy;
+            v = (double)T[2] * dx + (double)T[3] * dy;
+        }
+        const float *kx = m->knots_xy;
+        size_t per_plane = (size_t)(m->n_int_x + 3) * (size_t)(m->n_int_y + 3);
+        if (m->lrf_dim == 5) {
+            double z_lo = (double)kx[4], z_hi = (double)kx[5];
+            double dz = (z_hi - z_lo) / (m->n_planes - 1);
+            double zc = z < z_lo ? z_lo : (z > z_hi ? z_hi : z);
+            int p = (int)floor((zc - z_lo) / dz);
+            if (p > m->n_planes - 2) p = m->n_planes - 2;
+            if (p < 0) p = 0;
+            double w = (zc - (z_lo + p * dz)) / dz;
+            const float *c0 = m->coeffs_xy + (tab * (size_t)m->n_planes + (size_t)p) * per_plane;
+            double s0 = oracle_spline2(c0, m->n_int_x, m->n_int_y, kx[0], kx[1], kx[2], kx[3], u, v);
+            double s1 = oracle_spline2(c0 + per_plane, m->n_int_x, m->n_int_y, kx[0], kx[1], kx[2], kx[3], u, v);
+            s += (1.0 - w) * s0 + w * s1;
+        } else {
+            const float *c = m->coeffs_xy + tab * per_plane;
+            s += oracle_spline2(c, m->n_int_x, m->n_int_y, kx[0], kx[1], kx[2], kx[3], u, v);
+        }
+    }
     return g * s;
+}
+
+/* z range inside which a node is valid (R6), if the parameterisation depends on z: returns 1 and the range */
+static int z_range(const oracle_model_t *m, double *z_lo, double *z_hi)
+{
+    if (m->lrf_dim == 2) { *z_lo = (double)m->knots[2]; *z_hi = (double)m->knots[3]; return 1; }
+    if (m->lrf_dim == 5) { *z_lo = (double)m->knots_xy[4]; *z_hi = (double)m->knots_xy[5]; return 1; }
+    return 0;
 }
 
 /* signals as the method sees them: Poisson ML clips negatives to 0 (R18) */
@@ -217,7 +277,8 @@ static int score_prepared(const oracle_model_t *m, const double *S, const uint8_
     double sumL = 0.0;
     *A_out = NAN;
     *score_out = INFINITY;
-    if (m->lrf_dim == 2 && !(z >= (double)m->knots[2] && z <= (double)m->knots[3])) return 1; /* R6 */
+    double z_lo, z_hi;
+    if (z_range(m, &z_lo, &z_hi) && !(z >= z_lo && z <= z_hi)) return 1; /* R6 */
     for (int i = 0; i < N; ++i) { if (!ACTIVE(i)) continue; L[i] = oracle_lrf(m, i, x, y, z); sumL += L[i]; }
     if (!(sumL > 0.0)) return 1;
     if (method == 0) {
@@ -330,8 +391,9 @@ int oracle_score_at(const oracle_model_t *m, const float *sig, int method, int s
 /* fixed or start z (R10): z_seed, else mid-domain; 0 for purely axial LRFs */
 static double start_z(const oracle_model_t *m, const oracle_grid_t *g)
 {
-    if (m->lrf_dim != 2) return 0.0;
-    if (isnan(g->z_seed)) return 0.5 * ((double)m->knots[2] + (double)m->knots[3]);
+    double z_lo, z_hi;
+    if (!z_range(m, &z_lo, &z_hi)) return 0.0;
+    if (isnan(g->z_seed)) return 0.5 * (z_lo + z_hi);
     return (double)g->z_seed;
 }
 
@@ -423,7 +485,7 @@ int oracle_reconstruct(const oracle_model_t *m, const float *signals, int64_t n_
     if (g->nodes_per_axis < 2 || g->n_iter < 1 || !(g->factor > 0.0f && g->factor < 1.0f)) return -1;
     if (g->dim != 2 && g->dim != 3) return -1;
     if (g->seed_mode != 0 && g->seed_mode != 1) return -1;
-    if (g->dim == 3 && m->lrf_dim != 2) return -1;
+    if (g->dim == 3 && m->lrf_dim != 2 && m->lrf_dim != 5) return -1;
     int N = m->n_sensors, K = g->n_iter;
 #ifdef _OPENMP
 #pragma omp parallel num_threads(oracle_threads(n_threads))

@@ -209,3 +209,38 @@ def renormalise_gains(gains_new, gains_prev):
         usable = np.isfinite(gn) & (gn > 0.0)
     g = np.where(usable, gn, gp)
     return (g * (gp.mean() / g.mean())).astype(np.float32)
+
+
+def group_by_symmetry(sensor_xy, n_fold, reflect=True, tol=1e-3):
+    """"Grouping based on rotation or/and reflection symmetry of the sensor array (square, rectangular or
+    hexagonal)".  Reading R33: the operations are the rotations by 2 pi k / n_fold about the
+    detector centre (the origin), k = 0 .. n_fold-1, and, with reflect, each of them applied after the mirror
+    y -> -y (n_fold = 4 for a square array, 2 for a rectangular one, 6 for a hexagonal one).  Sensors are taken
+    in index order: one that has no group yet founds the next group as its reference; every operation Q, in the
+    order above, sends the reference position to Q P_ref, and a sensor within tol (mm) of that image that has no
+    group yet joins with the frame T_i = Q^-1 = Q^T, so that its local coordinates (u, v) = T_i (p - P_i) are
+    those of the reference sensor seen from the turned-back point.
+    -> (group [N] int32, xform [N][4] float32 row-major, n_groups)."""
+    xy = np.asarray(sensor_xy, np.float32).astype(np.float64).reshape(-1, 2)
+    N = len(xy)
+    ops = []
+    for mirror in ((False, True) if reflect else (False,)):
+        for k in range(int(n_fold)):
+            a = 2.0 * np.pi * k / n_fold
+            R = np.array([[np.cos(a), -np.sin(a)], [np.sin(a), np.cos(a)]])
+            ops.append(R @ np.diag([1.0, -1.0]) if mirror else R)
+    group = np.full(N, -1, np.int32)
+    xform = np.zeros((N, 4), np.float32)
+    n_groups = 0
+    for ref in range(N):
+        if group[ref] >= 0:
+            continue
+        for Q in ops:
+            img = Q @ xy[ref]
+            for i in range(N):
+                if group[i] < 0 and np.hypot(xy[i, 0] - img[0], xy[i, 1] - img[1]) <= tol:
+                    group[i] = n_groups
+                    xform[i] = Q.T.reshape(4).astype(np.float32)
+                    break
+        n_groups += 1
+    return group, xform, n_groups

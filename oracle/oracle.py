@@ -33,7 +33,9 @@ class _Model(C.Structure):
                 ("sensor_xy", C.c_void_p), ("gains", C.c_void_p),
                 ("knots", C.c_void_p), ("coeffs", C.c_void_p),
                 ("passive", C.c_void_p), ("signal_min", C.c_float), ("dist_max", C.c_float),
-                ("group", C.c_void_p)]
+                ("group", C.c_void_p),
+                ("n_int_x", C.c_int32), ("n_int_y", C.c_int32), ("n_planes", C.c_int32),
+                ("knots_xy", C.c_void_p), ("coeffs_xy", C.c_void_p), ("xform", C.c_void_p)]
 
 
 class _Grid(C.Structure):
@@ -98,13 +100,24 @@ class Model:
     """The LRF model: the float32 arrays handed to ants_lrf_create, kept alive here."""
 
     def __init__(self, sensor_xy, gains, knots, coeffs, n_lrf, lrf_dim, n_int_r, n_int_z,
-                 passive=None, signal_min=float("nan"), dist_max=float("nan"), group=None):
+                 passive=None, signal_min=float("nan"), dist_max=float("nan"), group=None,
+                 n_int_x=0, n_int_y=0, n_planes=0, knots_xy=None, coeffs_xy=None, xform=None):
         self.sensor_xy = _f32(sensor_xy).reshape(-1, 2)
         N = self.sensor_xy.shape[0]
         self.gains = _f32(np.ones(N) if gains is None else gains)
-        self.knots = _f32(knots)
-        self.coeffs = _f32(coeffs)
-        assert self.coeffs.size == n_lrf * (n_int_r + 3) * ((n_int_z + 3) if lrf_dim == 2 else 1)
+        self.knots = _f32(knots if knots is not None else [0.0, 1.0])
+        self.coeffs = _f32(coeffs if coeffs is not None else np.zeros(0))
+        if lrf_dim in (1, 2, 4):
+            assert self.coeffs.size == n_lrf * (n_int_r + 3) * ((n_int_z + 3) if lrf_dim == 2 else 1)
+        self.knots_xy = self.coeffs_xy = self.xform = None
+        if lrf_dim >= 3:
+            self.knots_xy = _f32(knots_xy)
+            self.coeffs_xy = _f32(coeffs_xy)
+            assert self.knots_xy.size == (6 if lrf_dim == 5 else 4)
+            assert (n_planes >= 2) if lrf_dim == 5 else (n_planes == 0)
+            assert self.coeffs_xy.size == n_lrf * max(n_planes, 1) * (n_int_x + 3) * (n_int_y + 3)
+            if xform is not None:
+                self.xform = _f32(xform).reshape(N, 4)
         self.n_sensors = N
         self.passive = None if passive is None else np.ascontiguousarray(np.asarray(passive) != 0, dtype=np.uint8)
         assert self.passive is None or self.passive.size == N
@@ -114,14 +127,20 @@ class Model:
                         self.gains.ctypes.data, self.knots.ctypes.data, self.coeffs.ctypes.data,
                         None if self.passive is None else self.passive.ctypes.data,
                         float(signal_min), float(dist_max),
-                        None if self.group is None else self.group.ctypes.data)
+                        None if self.group is None else self.group.ctypes.data,
+                        int(n_int_x), int(n_int_y), int(n_planes),
+                        None if self.knots_xy is None else self.knots_xy.ctypes.data,
+                        None if self.coeffs_xy is None else self.coeffs_xy.ctypes.data,
+                        None if self.xform is None else self.xform.ctypes.data)
 
     @classmethod
     def from_config(cls, cfg):
         return cls(cfg.sensor_xy, cfg.gains, cfg.knots, cfg.coeffs, cfg.n_lrf, cfg.lrf_dim,
                    cfg.n_int_r, cfg.n_int_z, getattr(cfg, "passive", None),
                    getattr(cfg, "signal_min", float("nan")), getattr(cfg, "dist_max", float("nan")),
-                   getattr(cfg, "group", None))
+                   getattr(cfg, "group", None), getattr(cfg, "n_int_x", 0), getattr(cfg, "n_int_y", 0),
+                   getattr(cfg, "n_planes", 0), getattr(cfg, "knots_xy", None), getattr(cfg, "coeffs_xy", None),
+                   getattr(cfg, "xform", None))
 
     def lrf(self, i, x, y, z=0.0):
         return _load().oracle_lrf(C.byref(self.c), int(i), float(x), float(y), float(z))

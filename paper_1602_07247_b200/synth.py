@@ -7,7 +7,9 @@ and bench.py alike and therefore holds none of the reconstruction arithmetic
 CUDA binding.  Spline fitting and spline evaluation go through
 `scipy.interpolate.BSpline` (a library routine); bulk signal generation reads
 a dense lookup table of that library evaluation so that it can run on the GPU
-with torch's seeded generators.
+with torch's seeded generators (the XY-type LRFs, whose tables would be large,
+are evaluated from the B-spline basis directly in torch float64; a test checks
+that evaluation against scipy's).
 
 Recipe:
   * sensors: hexagonal packing in axial coordinates, or a square grid
@@ -87,6 +89,19 @@ def fit_axial_z(profile, r_rng, z_rng, n_int_r: int, n_int_z: int,
     return C.astype(np.float32)
 
 
+def fit_xy(profile, u_rng, v_rng, n_int_x: int, n_int_y: int, n_u: int = 120, n_v: int = 120) -> np.ndarray:
+    """Separable LS fit of a tensor-product (u,v) spline to profile(u, v); returns [n_int_y+3][n_int_x+3] float32."""
+    return fit_axial_z(lambda u, v: profile(u, v), u_rng, v_rng, n_int_x, n_int_y, n_u, n_v)
+
+
+def eval_xy_points(coeffs: np.ndarray, u_rng, v_rng, u: np.ndarray, v: np.ndarray) -> np.ndarray:
+    """Library evaluation (scipy design matrices) of the tensor-product spline at paired points (u_k, v_k),
+    coordinates clamped into the tabulated ranges."""
+    Bu = _design(np.asarray(u, dtype=np.float64).ravel(), u_rng[0], u_rng[1], coeffs.shape[1] - 3)
+    Bv = _design(np.asarray(v, dtype=np.float64).ravel(), v_rng[0], v_rng[1], coeffs.shape[0] - 3)
+    return np.einsum("kb,ba,ka->k", Bv, coeffs.astype(np.float64), Bu).reshape(np.shape(u))
+
+
 def eval_axial(coeffs: np.ndarray, lo: float, hi: float, r: np.ndarray) -> np.ndarray:
     """Library evaluation (scipy BSpline) of a uniform cubic spline, r clamped to [lo,hi]."""
     n_int = coeffs.shape[-1] - 3
@@ -141,6 +156,13 @@ class Config:
     seed_mode: int = 0                       # 0 centroid, 1 strongest sensor
     # photosensor grouping: table index of every sensor, n_lrf = number of groups; None = off
     group: Optional[np.ndarray] = None
+    # XY-type parameterisations (lrf_dim 3 XY, 4 Composite = Axial + XY, 5 Sliced)
+    n_int_x: int = 0
+    n_int_y: int = 0
+    n_planes: int = 0                        # Sliced: z planes, uniform from z_lo to z_hi
+    knots_xy: Optional[np.ndarray] = None    # {u_lo,u_hi,v_lo,v_hi} (+ {z_lo,z_hi} for Sliced) float32
+    coeffs_xy: Optional[np.ndarray] = None   # [n_lrf][n_planes or 1][n_int_y+3][n_int_x+3] float32
+    xform: Optional[np.ndarray] = None       # [N][4] per-sensor local frame (symmetry groups), or None
 
     @property
     def n_sensors(self) -> int:
@@ -210,17 +232,110 @@ def make_config(idx: int, seed: int = 0, n_events: Optional[int] = None) -> Conf
                      2, 9, 5.0, 0.0, 0.5, 12, 0,
                      n_events=16_000_000, region="disk", extent=140.0,
                      nph=("lognormal", 3000.0, 0.3), noise_sigma=1.5, n_batches=8)
+    elif idx == 6:
+        # XY LRFs shared by the symmetry of a square array: config 3's SiPM array with a
+        # response that is not axial (elliptical bell in the sensor's own frame); 10 symmetry groups, D4
+        xy = square_array(8, 6.0)
+        group, xform, n_groups = symmetry_groups(xy, 4, True)
+        base = fit_xy(lambda u, v: (1.0 + (u / 5.0) ** 2 + (v / 7.0) ** 2) ** -1.5, (-32.0, 32.0), (-32.0, 32.0),
+                      16, 16).astype(np.float64)
+        fac = _rng(seed, _STREAM_FACTORS).normal(1.0, 0.05, n_groups)
+        cxy = (base[None, :, :] * fac[:, None, None]).astype(np.float32)[:, None, :, :]
+        cfg = Config("cfg6_xy_sq64_sym", xy, np.ones(len(xy), np.float32), np.array([0, 1], np.float32),
+                     np.zeros((n_groups, 1, 0), np.float32), n_groups, 3, 0, 0,
+                     2, 11, 2.0, 0.0, 0.5, 10, 1,
+                     n_events=1_000_000, region="square", extent=24.0, nph=("const", 3000.0),
+                     group=group, xform=xform, n_int_x=16, n_int_y=16,
+                     knots_xy=np.array([-32, 32, -32, 32], np.float32), coeffs_xy=cxy)
+    elif idx == 7:
+        # Sliced LRF: config 4's PMT array, one shared set of XY LRFs on 5 z planes
+        xy = hex_array(3, 30.0)
+        planes = np.linspace(0.0, 20.0, 5)
+        cxy = np.stack([fit_xy(lambda u, v, zp=zp: 1000.0 * (zp + 15.0) / (u * u + v * v + (zp + 15.0) ** 2) ** 1.5,
+                               (-120.0, 120.0), (-120.0, 120.0), 20, 20) for zp in planes])[None, :, :, :]
+        cfg = Config("cfg7_sliced_hex37", xy, np.ones(len(xy), np.float32), np.array([0, 1], np.float32),
+                     np.zeros((1, 1, 0), np.float32), 1, 5, 0, 0,
+                     3, 7, 8.0, 3.0, 0.5, 10, 0,
+                     n_events=1_000_000, region="disk", extent=90.0, z_range=(0.0, 20.0), nph=("const", 4000.0),
+                     n_int_x=20, n_int_y=20, n_planes=5,
+                     knots_xy=np.array([-120, 120, -120, 120, 0, 20], np.float32), coeffs_xy=cxy.astype(np.float32))
+    elif idx == 8:
+        # Composite LRF: config 2's axial response plus a small non-axial XY component
+        xy = hex_array(2, 30.0)
+        g = _rng(seed, _STREAM_GAINS).uniform(0.8, 1.2, len(xy)).astype(np.float32)
+        c = fit_axial(_bell(20.0), 0.0, 90.0, 16)[None, None, :]
+        cxy = fit_xy(lambda u, v: 0.03 * np.exp(-(u * u + v * v) / 1250.0) * (u / 25.0), (-90.0, 90.0), (-90.0, 90.0),
+                     12, 12)[None, None, :, :]
+        cfg = Config("cfg8_composite_hex19", xy, g, np.array([0, 90], np.float32), c, 1, 4, 16, 0,
+                     2, 9, 5.0, 0.0, 0.5, 10, 0,
+                     n_events=1_000_000, region="disk", extent=60.0, nph=("uniform", 1000.0, 5000.0), noise_sigma=1.0,
+                     n_int_x=12, n_int_y=12, knots_xy=np.array([-90, 90, -90, 90], np.float32), coeffs_xy=cxy)
     else:
-        raise ValueError("config index must be 1..5")
+        raise ValueError("config index must be 1..8")
     cfg.seed = seed
     if n_events is not None:
         cfg.n_events = int(n_events)
     return cfg
 
 
+def symmetry_groups(sensor_xy: np.ndarray, n_fold: int, reflect: bool, tol: float = 1e-3):
+    """Input helper: orbits of the sensors under the rotations by 2 pi k / n_fold about the origin (and the mirror
+    y -> -y first, with reflect), each sensor with the transposed operation that maps its group's first sensor
+    onto it as its local frame.  -> (group int32 [N], xform float32 [N][4], n_groups).  Pure geometry of the
+    input array; the library's own version is ants_group_by_symmetry."""
+    P = sensor_xy.astype(np.float64)
+    ops = []
+    for mirror in ((False, True) if reflect else (False,)):
+        for k in range(n_fold):
+            a = 2.0 * math.pi * k / n_fold
+            R = np.array([[math.cos(a), -math.sin(a)], [math.sin(a), math.cos(a)]])
+            ops.append(R @ np.diag([1.0, -1.0]) if mirror else R)
+    group = np.full(len(P), -1, np.int32)
+    xform = np.zeros((len(P), 4), np.float32)
+    n = 0
+    for ref in range(len(P)):
+        if group[ref] >= 0:
+            continue
+        for Q in ops:
+            d = np.hypot(*(P - Q @ P[ref]).T)
+            free = np.flatnonzero((group < 0) & (d <= tol))
+            if free.size:
+                group[free[0]] = n
+                xform[free[0]] = Q.T.reshape(4)
+        n += 1
+    return group, xform, n
+
+
 # --------------------------------------------------------------------------
 # flood-field events
 # --------------------------------------------------------------------------
+def _basis4_t(t: torch.Tensor):
+    o = 1.0 - t
+    return (o * o * o / 6.0, (3.0 * t ** 3 - 6.0 * t * t + 4.0) / 6.0,
+            (-3.0 * t ** 3 + 3.0 * t * t + 3.0 * t + 1.0) / 6.0, t ** 3 / 6.0)
+
+
+def _xy_profile_t(cfg: Config, coef_flat: torch.Tensor, tabs: torch.Tensor, plane, u: torch.Tensor, v: torch.Tensor):
+    """Tensor-product uniform cubic B-spline of the XY-type LRFs at (u, v) [m][N] (float64 torch; coordinates
+    clamped into the tabulated range), table tabs[i] of sensor i, z plane index `plane` ([m][1] long or 0).
+    tests/test_oracle_xy.py checks it against the scipy evaluation (eval_xy_points)."""
+    nu3, nv3, P = cfg.n_int_x + 3, cfg.n_int_y + 3, max(cfg.n_planes, 1)
+    kx = [float(k) for k in cfg.knots_xy[:4]]
+
+    def locate(x, lo, hi, n):
+        t = (x.clamp(lo, hi) - lo) * (n / (hi - lo))
+        k = t.floor().clamp(max=n - 1).long()
+        return k, t - k
+    ku, tu = locate(u, kx[0], kx[1], cfg.n_int_x)
+    kv, tv = locate(v, kx[2], kx[3], cfg.n_int_y)
+    bu, bv = _basis4_t(tu), _basis4_t(tv)
+    base = ((tabs[None, :] * P + plane) * nv3 + kv) * nu3 + ku
+    s = torch.zeros_like(u)
+    for b in range(4):
+        for a in range(4):
+            s = s + coef_flat[base + b * nu3 + a] * bu[a] * bv[b]
+    return s
+
 _TABLE_R, _TABLE_Z = 1 << 15, 257
 
 
@@ -229,7 +344,7 @@ def _mean_table(cfg: Config) -> np.ndarray:
 
     Returns [n_lrf][_TABLE_R] (axial) or [_TABLE_Z][_TABLE_R] (axial+z, n_lrf == 1)."""
     r = np.linspace(float(cfg.knots[0]), float(cfg.knots[1]), _TABLE_R)
-    if cfg.lrf_dim == 1:
+    if cfg.lrf_dim in (1, 4):
         return np.stack([eval_axial(cfg.coeffs[m, 0], float(cfg.knots[0]), float(cfg.knots[1]), r)
                          for m in range(cfg.n_lrf)])
     z = np.linspace(float(cfg.knots[2]), float(cfg.knots[3]), _TABLE_Z)
@@ -257,7 +372,11 @@ def generate_events(cfg: Config, n_events: Optional[int] = None, device="cpu",
     dev = torch.device(device)
     gen = torch.Generator(device=dev)
     gen.manual_seed((cfg.seed * 1_000_003 + _STREAM_EVENTS) * 1009 + batch)
-    tab = torch.from_numpy(_mean_table(cfg)).to(dev, torch.float64)
+    tab = torch.from_numpy(_mean_table(cfg)).to(dev, torch.float64) if cfg.lrf_dim in (1, 2, 4) else None
+    if cfg.lrf_dim >= 3:
+        cxy_flat = torch.from_numpy(cfg.coeffs_xy.astype(np.float64).ravel()).to(dev)
+        T = (torch.from_numpy(cfg.xform.astype(np.float64)).to(dev) if cfg.xform is not None
+             else torch.tensor([1.0, 0.0, 0.0, 1.0], dtype=torch.float64, device=dev).repeat(cfg.n_sensors, 1))
     sx = torch.from_numpy(cfg.sensor_xy[:, 0].astype(np.float64)).to(dev)
     sy = torch.from_numpy(cfg.sensor_xy[:, 1].astype(np.float64)).to(dev)
     g = torch.from_numpy(cfg.gains.astype(np.float64)).to(dev)
@@ -290,7 +409,24 @@ def generate_events(cfg: Config, n_events: Optional[int] = None, device="cpu",
             n = cfg.nph[1] * torch.exp(cfg.nph[2] * nrm)
         r = torch.sqrt((x[:, None] - sx[None, :]) ** 2 + (y[:, None] - sy[None, :]) ** 2)
         t = (r.clamp(r_lo, r_hi) - r_lo) * ((_TABLE_R - 1) / (r_hi - r_lo))
-        if cfg.lrf_dim == 1:
+        if cfg.lrf_dim >= 3:
+            tables = (torch.from_numpy(np.asarray(cfg.group, np.int64)).to(dev) if cfg.group is not None
+                      else (torch.zeros(N, dtype=torch.long, device=dev) if cfg.n_lrf == 1 else torch.arange(N, device=dev)))
+            dxs, dys = x[:, None] - sx[None, :], y[:, None] - sy[None, :]
+            uu = T[None, :, 0] * dxs + T[None, :, 1] * dys
+            vv = T[None, :, 2] * dxs + T[None, :, 3] * dys
+            if cfg.lrf_dim == 5:
+                z_lo, z_hi = float(cfg.knots_xy[4]), float(cfg.knots_xy[5])
+                dzp = (z_hi - z_lo) / (cfg.n_planes - 1)
+                pz = ((z.clamp(z_lo, z_hi) - z_lo) / dzp).floor().clamp(max=cfg.n_planes - 2).long()
+                wz = ((z.clamp(z_lo, z_hi) - (z_lo + pz * dzp)) / dzp)[:, None]
+                prof = ((1.0 - wz) * _xy_profile_t(cfg, cxy_flat, tables, pz[:, None], uu, vv)
+                        + wz * _xy_profile_t(cfg, cxy_flat, tables, pz[:, None] + 1, uu, vv))
+            else:
+                prof = _xy_profile_t(cfg, cxy_flat, tables, 0, uu, vv)
+                if cfg.lrf_dim == 4:
+                    prof = prof + _lerp_table(tab[0], t)
+        elif cfg.lrf_dim == 1:
             if cfg.n_lrf == 1:
                 prof = _lerp_table(tab[0], t)
             else:

@@ -41,10 +41,17 @@ UNIT = "events/s"
 # nominal algorithmic flop per (node, sensor) pair:
 # FMA = 2, sqrt / log / div = 1; every one of the K * G^d * N evaluations counts.
 FLOP_PER_PAIR = {"axial_poisson": 20.0, "axial_chi2": 25.0, "axialz_poisson": 35.0}
+# XY-type parameterisations (configs 6-8, outside BASELINE.json's five): local frame (6) +
+# two interval/fraction look-ups (6) + two 4-weight cubic bases (2 x 11) + 4 x 4 tensor contraction (16 + 4 FMA = 40)
+# = 74 per XY evaluation; a Sliced LRF contracts two planes (+ 40) and interpolates (3); a Composite adds the axial
+# evaluation (15); the score terms add 5 (Poisson) or 10 (chi-square) as for the axial LRFs.
+FLOP_XY = {3: 74.0, 4: 89.0, 5: 117.0}
 FP32_LANES_PER_SM = 128          # B200 SM: 4 sub-partitions x 32 FP32 lanes, 1 FMA/lane/clk
 
 
 def flop_per_pair(cfg) -> float:
+    if cfg.lrf_dim >= 3:
+        return FLOP_XY[cfg.lrf_dim] + (5.0 if cfg.method == 0 else 10.0)
     if cfg.lrf_dim == 2:
         return FLOP_PER_PAIR["axialz_poisson"]
     return FLOP_PER_PAIR["axial_chi2" if cfg.method == 1 else "axial_poisson"]
@@ -574,7 +581,7 @@ def main(argv=None):
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=5,
                     help="BASELINE.json config 1..5 of the headline (default 5 = the largest single-GPU config: "
-                         "16 M events as 8 batches of 2 M)")
+                         "16 M events as 8 batches of 2 M); 6, 7, 8 = the XY / Sliced / Composite LRF workloads")
     ap.add_argument("--no-per-config", action="store_true", help="skip the per_config entries of the other configs")
     ap.add_argument("--per-config-cpu-seconds", type=float, default=5.0)
     ap.add_argument("--events", type=int, default=None, help="events per step per GPU (default: the config's batch)")

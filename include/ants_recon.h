@@ -58,7 +58,9 @@ typedef struct {
     int32_t n_lrf;     /* number of tables.  ants_lrf_create: 1 = one shared profile, L_i = gains[i] * s(.);
                           N = one table per sensor, L_i = s_i(.).  ants_lrf_create_grouped: the number of
                           sensor groups, L_i = gains[i] * s_group[i](.) */
-    int32_t lrf_dim;   /* 1 = axial s(r); 2 = axial+z s(r,z) tensor product */
+    int32_t lrf_dim;   /* LRF parameterisation (section 6.1): 1 = Axial s(r);
+                          2 = Axial+Z s(r,z) tensor product; with ants_lrf_create_xy also
+                          3 = XY, 4 = Composite (Axial + XY), 5 = Sliced (XY LRFs on z planes) */
     int32_t n_int_r;   /* uniform intervals in r: n_int_r + 3 coefficients */
     int32_t n_int_z;   /* uniform intervals in z (ignored when lrf_dim == 1) */
 } ants_lrf_dims_t;
@@ -95,6 +97,51 @@ int ants_lrf_create_grouped(const float *sensor_xy, const float *gains, const in
                             const float *knots, const float *coeffs, const ants_lrf_dims_t *dims,
                             ants_lrf_t **out);
 
+/* The XY part of an XY-type model (lrf_dim 3, 4, 5). */
+typedef struct {
+    int32_t n_int_x, n_int_y;  /* uniform intervals of the XY spline in the sensor-local coordinates (u, v) */
+    int32_t n_planes;          /* Sliced: number of z planes (>= 2), uniformly spaced from z_lo to z_hi; else 0 */
+    const float *knots_xy;     /* HOST {u_lo, u_hi, v_lo, v_hi}, followed by {z_lo, z_hi} for Sliced */
+    const float *coeffs_xy;    /* HOST [n_lrf][n_planes or 1][n_int_y + 3][n_int_x + 3] float, u fastest */
+    const float *xform;        /* HOST [N][4] or NULL (identity): per-sensor frame T_i, row-major;
+                                  (u, v) = T_i (p_xy - P_i) */
+    const int32_t *group;      /* HOST [N] table index of every sensor, or NULL (n_lrf = 1 or N as in create) */
+} ants_lrf_xy_t;
+
+/*
+ * ants_lrf_create_xy -- model with one of the XY-type parameterisations of PAPER.md:388-396 (section 6.1):
+ *   lrf_dim 3 "XY LRF": "LRF is a function of X and Y and no other type of symmetry can be assumed" --
+ *             L_i = g_i s_t(u, v), a tensor-product cubic B-spline of the position relative to the sensor,
+ *             each coordinate clamped into the tabulated range (R30, R5);
+ *   lrf_dim 4 "Composite LRF": "a sum of two components: an Axial LRF and an XY LRF" -- L_i = g_i (s_t(r) +
+ *             s_t(u, v)); knots/coeffs/dims->n_int_r describe the axial component as in ants_lrf_create (R31);
+ *   lrf_dim 5 "Sliced LRF": "a set of several XY LRFs, each defined on a specific Z plane ... linear
+ *             interpolation of the LRF values at two closest points from two closest planes" -- planes at
+ *             z_lo + p (z_hi - z_lo)/(n_planes - 1); a node with z outside [z_lo, z_hi] is invalid (R32, R6);
+ *             searched over (x, y, z) with grid dim 3, or over (x, y) at the fixed z_seed with dim 2.
+ * t = group[i], or 0 / i without a grouping; g_i = gains[i] for a shared or group table, 1 for per-sensor
+ * tables.  Per-sensor frames serve the grouping "based on rotation or/and reflection symmetry of the sensor
+ * array" (ants_group_by_symmetry makes them; R33).  knots and coeffs may be NULL unless
+ * lrf_dim == 4.  These models run the general kernel (recon_gen.cuh): FP32 scores on the coarse grids, FP64 on
+ * the fine ones.  Errors as ants_lrf_create; ANTS_ERR_UNSUPPORTED if the tables exceed the shared memory.
+ */
+int ants_lrf_create_xy(const float *sensor_xy, const float *gains, const float *knots, const float *coeffs,
+                       const ants_lrf_dims_t *dims, const ants_lrf_xy_t *xy, ants_lrf_t **out);
+
+/*
+ * ants_group_by_symmetry -- photosensor groups "based on rotation or/and reflection symmetry of the sensor
+ * array (square, rectangular or hexagonal)".  Reading R33: the operations are the rotations by
+ * 2 pi k / n_fold about the origin, k = 0 .. n_fold-1 (4 square, 2 rectangular, 6 hexagonal) and, with reflect
+ * != 0, each of them applied after the mirror y -> -y.  Sensors are taken in index order; one without a group
+ * founds the next group as its reference (identity frame); every operation Q, in the order above, maps the
+ * reference position to Q P_ref, and a sensor without a group within tol (mm) of that image (lowest index)
+ * joins with the frame T_i = Q^T.
+ *   sensor_xy HOST [N][2]; group_out HOST [N] int32; xform_out HOST [N][4] float or NULL; n_groups_out HOST.
+ * Host-only.  Errors: ANTS_ERR_INVALID (NULL, N < 1, n_fold < 1, tol < 0 or not finite), ANTS_ERR_NOMEM.
+ */
+int ants_group_by_symmetry(const float *sensor_xy, int32_t n_sensors, int32_t n_fold, int32_t reflect, float tol,
+                           int32_t *group_out, float *xform_out, int32_t *n_groups_out);
+
 /*
  * ants_group_by_radius -- photosensor groups "according to the distance from the sensor center to the
  * detector center" (section 6.2).  Reading R28: sensors are ordered by their distance from
@@ -110,7 +157,7 @@ int ants_group_by_radius(const float *sensor_xy, int32_t n_sensors, float tol, i
 int32_t ants_lrf_n_sensors(const ants_lrf_t *lrf);
 
 typedef struct {
-    int32_t dim;            /* 2 = search (x,y); 3 = search (x,y,z), requires lrf_dim == 2 */
+    int32_t dim;            /* 2 = search (x,y); 3 = search (x,y,z), requires lrf_dim == 2 or 5 */
     int32_t nodes_per_axis; /* G >= 2; the grid has G^dim nodes */
     float step0_xy;         /* first-iteration node spacing in x and y, mm, > 0 */
     float step0_z;          /* first-iteration node spacing in z, mm (dim == 3), > 0 */
@@ -157,8 +204,9 @@ int ants_lrf_set_selection(ants_lrf_t *lrf, const uint8_t *passive, float signal
  * Per-event failure does not fail the call: an event with a non-finite signal,
  * sum S <= 0 or (centroid start) sum S/g <= 0 gets x = y = z = A = NaN and score = +inf.
  * Errors: ANTS_ERR_INVALID (NULL pointers with n_events > 0, bad grid values,
- * dim 3 with an axial LRF, method not 0/1/2), ANTS_ERR_UNSUPPORTED (method 2 with an axial+z LRF; G^dim above
- * the compiled limit: 256 nodes in 2-D, 512 in 3-D), ANTS_ERR_CUDA.
+ * dim 3 with an LRF that does not depend on z, method not 0/1/2), ANTS_ERR_UNSUPPORTED (method 2 with an
+ * Axial+Z LRF; packed kernels: G^dim above the compiled limit, 256 nodes in 2-D, 512 in 3-D; general kernel:
+ * more than 65535 nodes), ANTS_ERR_CUDA.
  * n_events == 0 is a valid no-op.
  */
 int ants_reconstruct(const ants_lrf_t *lrf, const float *signals, int64_t n_events,

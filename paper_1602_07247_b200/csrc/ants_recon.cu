@@ -7,6 +7,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <algorithm>
+#include <array>
 #include <atomic>
 #include <mutex>
 #include <new>
@@ -16,6 +17,7 @@
 #include "recon2d.cuh"
 #include "recon2d_pk.cuh"
 #include "recon3d.cuh"
+#include "recon_gen.cuh"
 #include "kernels.h"
 
 using namespace ants;
@@ -31,7 +33,7 @@ static const unsigned kCtrSlots = 1024;
 struct Plan {
     int npt = 0;             // nodes per lane (template instantiation)
     int cpl = 0, gzm = 0;    // axial+z kernel: columns per lane, compiled z-levels
-    int family = 0;          // 0 recon2d_pk_kernel, 1 recon2d_kernel (generic), 2 recon3d_kernel
+    int family = 0;          // 0 recon2d_pk_kernel, 2 recon3d_kernel, 3 recon_gen_kernel (general)
     int warps = 0;           // warps per CTA
     int ctas_per_sm = 0;     // resident CTAs per SM (cudaOccupancyMaxActiveBlocksPerMultiprocessor, capped by the tuning knob)
     size_t smem = 0;         // dynamic shared memory per CTA
@@ -53,7 +55,8 @@ struct ants_lrf {
     ModelDev dev{};          // device pointers + scalars, passed by value to the kernels
     std::mutex plan_mu;      // guards plans
     std::vector<std::pair<PlanKey, Plan>> plans;
-    void *d_grp = nullptr;
+    void *d_grp = nullptr, *d_cxy = nullptr, *d_xf = nullptr;
+    double knot_xy = 0.0;    // XY-type models: smallest knot spacing of the XY spline, mm
     cudaEvent_t *slot_ev = nullptr;   // [kCtrSlots] lazily created: the launch that last used a counter slot
     int device = 0;
     int sm_count = 0;
@@ -213,6 +216,7 @@ static void tensor_analysis(const float *c, const double *rows64, int n_r, int n
 
 static bool finite_f(float v) { return std::isfinite(v); }
 
+struct ants_lrf;
 // group == nullptr: n_lrf = 1 (all sensors on table 0, L = g s) or n_lrf = N (sensor i on table i, L = s_i)
 static int create_impl(const float *sensor_xy, const float *gains, const int32_t *group, const float *knots,
                        const float *coeffs, const ants_lrf_dims_t *dims, ants_lrf_t **out) {
@@ -310,6 +314,11 @@ static int create_impl(const float *sensor_xy, const float *gains, const int32_t
     ModelDev &m = h->dev;
     m.sens = (const float4 *)h->d_sens;
     m.grp = (const int *)h->d_grp;
+    m.cxy = nullptr;
+    m.xf = nullptr;
+    m.nx = m.ny = m.n_planes = 0;
+    m.u_lo = m.v_lo = 0.f;
+    m.su = m.sv = 1.f;
     m.poly = (const float4 *)h->d_poly;
     m.polyd = (const double *)h->d_polyd;
     m.N = N;
@@ -327,7 +336,188 @@ static int create_impl(const float *sensor_xy, const float *gains, const int32_t
     m.passive = nullptr;
     m.signal_min = m.dist_max = std::nanf("");
     m.select = 0;
+    m.lrf_kind = dim;
     *out = h;
+    return ANTS_OK;
+}
+
+static int create_xy_impl(const float *sensor_xy, const float *gains, const float *knots, const float *coeffs,
+                          const ants_lrf_dims_t *dims, const ants_lrf_xy_t *xy, ants_lrf_t **out) {
+    if (!out) return ANTS_ERR_INVALID;
+    *out = nullptr;
+    if (!sensor_xy || !dims || !xy || !xy->knots_xy || !xy->coeffs_xy) return ANTS_ERR_INVALID;
+    const int N = dims->n_sensors, n_lrf = dims->n_lrf, kind = dims->lrf_dim;
+    if (kind != 3 && kind != 4 && kind != 5) return ANTS_ERR_INVALID;
+    const int nx = xy->n_int_x, ny = xy->n_int_y, n_planes = kind == 5 ? xy->n_planes : 0;
+    if (N < 1 || N > 65535 || nx < 1 || ny < 1 || nx > 1024 || ny > 1024) return ANTS_ERR_INVALID;
+    if (kind == 5 && (n_planes < 2 || n_planes > 4096)) return ANTS_ERR_INVALID;
+    if (xy->group) {
+        if (n_lrf < 1 || n_lrf > N) return ANTS_ERR_INVALID;
+        for (int i = 0; i < N; ++i)
+            if (xy->group[i] < 0 || xy->group[i] >= n_lrf) return ANTS_ERR_INVALID;
+    } else if (n_lrf != 1 && n_lrf != N) {
+        return ANTS_ERR_INVALID;
+    }
+    const float *kx = xy->knots_xy;
+    for (int j = 0; j < (kind == 5 ? 6 : 4); ++j)
+        if (!finite_f(kx[j])) return ANTS_ERR_INVALID;
+    if (!(kx[1] > kx[0]) || !(kx[3] > kx[2]) || (kind == 5 && !(kx[5] > kx[4]))) return ANTS_ERR_INVALID;
+    const size_t ncxy = (size_t)n_lrf * (n_planes > 0 ? n_planes : 1) * (nx + 3) * (ny + 3);
+    for (size_t j = 0; j < ncxy; ++j)
+        if (!finite_f(xy->coeffs_xy[j])) return ANTS_ERR_INVALID;
+    for (int i = 0; i < N; ++i) {
+        if (!finite_f(sensor_xy[2 * i]) || !finite_f(sensor_xy[2 * i + 1])) return ANTS_ERR_INVALID;
+        if (gains && !(gains[i] > 0.f && finite_f(gains[i]))) return ANTS_ERR_INVALID;
+        if (xy->xform)
+            for (int j = 0; j < 4; ++j)
+                if (!finite_f(xy->xform[4 * i + j])) return ANTS_ERR_INVALID;
+    }
+    // the axial component of a Composite model goes through the axial table builder
+    int n_r = 1;
+    float r_lo = 0.f, r_hi = 1.f;
+    if (kind == 4) {
+        if (!knots || !coeffs) return ANTS_ERR_INVALID;
+        n_r = dims->n_int_r;
+        r_lo = knots[0];
+        r_hi = knots[1];
+        if (n_r < 1 || n_r > 4096 || !finite_f(r_lo) || !finite_f(r_hi) || !(r_lo >= 0.f) || !(r_hi > r_lo)) return ANTS_ERR_INVALID;
+        for (size_t j = 0; j < (size_t)n_lrf * (n_r + 3); ++j)
+            if (!finite_f(coeffs[j])) return ANTS_ERR_INVALID;
+    }
+    ants_lrf *h = new (std::nothrow) ants_lrf;
+    if (!h) return ANTS_ERR_NOMEM;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&h->device) != cudaSuccess || cudaGetDeviceProperties(&prop, h->device) != cudaSuccess) {
+        delete h;
+        return ANTS_ERR_CUDA;
+    }
+    h->sm_count = prop.multiProcessorCount;
+    h->slot_ev = new (std::nothrow) cudaEvent_t[kCtrSlots]();
+    if (!h->slot_ev) { delete h; return ANTS_ERR_NOMEM; }
+    const bool scaled = xy->group != nullptr || n_lrf == 1;
+    std::vector<float4> sens(N), xf(N);
+    std::vector<int> grp(N);
+    for (int i = 0; i < N; ++i) {
+        const float g = gains ? gains[i] : 1.f;
+        sens[i] = make_float4(sensor_xy[2 * i], sensor_xy[2 * i + 1], scaled ? g : 1.f, 1.f / g);
+        grp[i] = xy->group ? xy->group[i] : (n_lrf == 1 ? 0 : i);
+        xf[i] = xy->xform ? make_float4(xy->xform[4 * i], xy->xform[4 * i + 1], xy->xform[4 * i + 2], xy->xform[4 * i + 3])
+                          : make_float4(1.f, 0.f, 0.f, 1.f);
+    }
+    std::vector<float4> rows32;
+    std::vector<double> rows64;
+    const double sc_r = (double)n_r / ((double)r_hi - (double)r_lo);
+    if (kind == 4) {
+        rows32.resize((size_t)n_lrf * (n_r + 1));
+        rows64.resize((size_t)n_lrf * n_r * 4);
+        bool pos = true;
+        double dl = 0.0;
+        for (int t = 0; t < n_lrf; ++t)
+            build_rows(coeffs + (size_t)t * (n_r + 3), n_r, sc_r, rows32.data() + (size_t)t * (n_r + 1),
+                       rows64.data() + (size_t)t * n_r * 4, pos, dl);
+    }
+    h->positive = false;             // general kernel: per-pair validity rules
+    h->knot_r = kind == 4 ? 1.0 / sc_r : 1e300;
+    h->knot_xy = std::fmin(((double)kx[1] - (double)kx[0]) / nx, ((double)kx[3] - (double)kx[2]) / ny);
+    bool ok = cudaMalloc(&h->d_ctr, kCtrSlots * 2 * sizeof(unsigned long long)) == cudaSuccess &&
+              cudaMemset(h->d_ctr, 0, kCtrSlots * 2 * sizeof(unsigned long long)) == cudaSuccess &&
+              cudaMalloc(&h->d_sens, sens.size() * sizeof(float4)) == cudaSuccess &&
+              cudaMalloc(&h->d_grp, grp.size() * sizeof(int)) == cudaSuccess &&
+              cudaMalloc(&h->d_xf, xf.size() * sizeof(float4)) == cudaSuccess &&
+              cudaMalloc(&h->d_cxy, ncxy * sizeof(float)) == cudaSuccess &&
+              (rows32.empty() || (cudaMalloc(&h->d_poly, rows32.size() * sizeof(float4)) == cudaSuccess &&
+                                  cudaMalloc(&h->d_polyd, rows64.size() * sizeof(double)) == cudaSuccess));
+    ok = ok && cudaMemcpy(h->d_sens, sens.data(), sens.size() * sizeof(float4), cudaMemcpyHostToDevice) == cudaSuccess &&
+         cudaMemcpy(h->d_grp, grp.data(), grp.size() * sizeof(int), cudaMemcpyHostToDevice) == cudaSuccess &&
+         cudaMemcpy(h->d_xf, xf.data(), xf.size() * sizeof(float4), cudaMemcpyHostToDevice) == cudaSuccess &&
+         cudaMemcpy(h->d_cxy, xy->coeffs_xy, ncxy * sizeof(float), cudaMemcpyHostToDevice) == cudaSuccess &&
+         (rows32.empty() ||
+          (cudaMemcpy(h->d_poly, rows32.data(), rows32.size() * sizeof(float4), cudaMemcpyHostToDevice) == cudaSuccess &&
+           cudaMemcpy(h->d_polyd, rows64.data(), rows64.size() * sizeof(double), cudaMemcpyHostToDevice) == cudaSuccess));
+    if (!ok) {
+        const cudaError_t e = cudaGetLastError();
+        ants_destroy(h);
+        return e == cudaErrorMemoryAllocation ? ANTS_ERR_NOMEM : ANTS_ERR_CUDA;
+    }
+    ModelDev &m = h->dev;
+    m.sens = (const float4 *)h->d_sens;
+    m.grp = (const int *)h->d_grp;
+    m.xf = xy->xform ? (const float4 *)h->d_xf : nullptr;
+    m.cxy = (const float *)h->d_cxy;
+    m.poly = (const float4 *)h->d_poly;
+    m.polyd = (const double *)h->d_polyd;
+    m.lrf_kind = kind;
+    m.nx = nx;
+    m.ny = ny;
+    m.n_planes = n_planes;
+    m.u_lo = kx[0];
+    m.su = (float)((double)nx / ((double)kx[1] - (double)kx[0]));
+    m.v_lo = kx[2];
+    m.sv = (float)((double)ny / ((double)kx[3] - (double)kx[2]));
+    m.N = N;
+    m.n_lrf = n_lrf;
+    m.n_r = kind == 4 ? n_r : 0;
+    m.n_z = 0;
+    m.r_lo = r_lo;
+    m.r_hi = r_hi;
+    m.sc = (float)sc_r;
+    m.of = (float)(-(double)r_lo * sc_r - 0.5);
+    m.tmax = (float)n_r - 0.5f;
+    m.z_lo = kind == 5 ? kx[4] : 0.f;
+    m.z_hi = kind == 5 ? kx[5] : 1.f;
+    m.scz = 0.f;
+    m.passive = nullptr;
+    m.signal_min = m.dist_max = std::nanf("");
+    m.select = 0;
+    *out = h;
+    return ANTS_OK;
+}
+
+extern "C" int ants_lrf_create_xy(const float *sensor_xy, const float *gains, const float *knots, const float *coeffs,
+                                  const ants_lrf_dims_t *dims, const ants_lrf_xy_t *xy, ants_lrf_t **out) {
+    return create_xy_impl(sensor_xy, gains, knots, coeffs, dims, xy, out);
+}
+
+// groups by the rotation / reflection symmetry of the array, with the sensors' frames (R33)
+extern "C" int ants_group_by_symmetry(const float *sensor_xy, int32_t n, int32_t n_fold, int32_t reflect, float tol,
+                                      int32_t *group_out, float *xform_out, int32_t *n_groups_out) {
+    if (!sensor_xy || !group_out || !n_groups_out || n < 1 || n_fold < 1 || !(tol >= 0.f) || !std::isfinite(tol))
+        return ANTS_ERR_INVALID;
+    for (int i = 0; i < 2 * n; ++i)
+        if (!std::isfinite(sensor_xy[i])) return ANTS_ERR_INVALID;
+    const double two_pi = 6.283185307179586476925286766559;
+    std::vector<std::array<double, 4>> ops;       // Q row-major
+    for (int mirror = 0; mirror <= (reflect ? 1 : 0); ++mirror)
+        for (int k = 0; k < n_fold; ++k) {
+            const double a = two_pi * k / n_fold, c = std::cos(a), s = std::sin(a);
+            // R = [[c, -s], [s, c]];  R M with M = diag(1, -1) flips the second column
+            ops.push_back(mirror ? std::array<double, 4>{c, s, s, -c} : std::array<double, 4>{c, -s, s, c});
+        }
+    for (int i = 0; i < n; ++i) group_out[i] = -1;
+    int n_groups = 0;
+    for (int ref = 0; ref < n; ++ref) {
+        if (group_out[ref] >= 0) continue;
+        const double px = sensor_xy[2 * ref], py = sensor_xy[2 * ref + 1];
+        for (const auto &Q : ops) {
+            const double ix = Q[0] * px + Q[1] * py, iy = Q[2] * px + Q[3] * py;
+            for (int i = 0; i < n; ++i) {
+                if (group_out[i] >= 0) continue;
+                const double dx = (double)sensor_xy[2 * i] - ix, dy = (double)sensor_xy[2 * i + 1] - iy;
+                if (std::sqrt(dx * dx + dy * dy) <= (double)tol) {
+                    group_out[i] = n_groups;
+                    if (xform_out) {          // T = Q^T
+                        xform_out[4 * i] = (float)Q[0];
+                        xform_out[4 * i + 1] = (float)Q[2];
+                        xform_out[4 * i + 2] = (float)Q[1];
+                        xform_out[4 * i + 3] = (float)Q[3];
+                    }
+                    break;
+                }
+            }
+        }
+        ++n_groups;
+    }
+    *n_groups_out = n_groups;
     return ANTS_OK;
 }
 
@@ -419,6 +609,8 @@ extern "C" void ants_destroy(ants_lrf_t *h) {
     cudaFree(h->d_passive);
     cudaFree(h->d_ctr);
     cudaFree(h->d_grp);
+    cudaFree(h->d_cxy);
+    cudaFree(h->d_xf);
     if (h->slot_ev) {
         for (unsigned s = 0; s < kCtrSlots; ++s)
             if (h->slot_ev[s]) cudaEventDestroy(h->slot_ev[s]);
@@ -454,13 +646,13 @@ extern "C" int64_t ants_launch_count(void) { return g_launches.load(); }
 // kernel look-ups: the instantiations live in k2d_pk_m*.cu, k2d_gen_m*.cu, k3d_m*.cu (kernels.h)
 namespace ants {
 const void *kernel_2d_pk_m0(int), *kernel_2d_pk_m1(int), *kernel_2d_pk_m2(int);
-const void *kernel_2d_gen_m0(int), *kernel_2d_gen_m1(int), *kernel_2d_gen_m2(int);
+const void *kernel_gen_m0(int), *kernel_gen_m1(int), *kernel_gen_m2(int);
 const void *kernel_3d_m0(int, int), *kernel_3d_m1(int, int);
 const void *kernel_2d_pk(int method, int npt) {
     return method == 0 ? kernel_2d_pk_m0(npt) : method == 1 ? kernel_2d_pk_m1(npt) : method == 2 ? kernel_2d_pk_m2(npt) : nullptr;
 }
-const void *kernel_2d_gen(int method, int npt) {
-    return method == 0 ? kernel_2d_gen_m0(npt) : method == 1 ? kernel_2d_gen_m1(npt) : method == 2 ? kernel_2d_gen_m2(npt) : nullptr;
+const void *kernel_gen(int method, int lrf_kind) {
+    return method == 0 ? kernel_gen_m0(lrf_kind) : method == 1 ? kernel_gen_m1(lrf_kind) : method == 2 ? kernel_gen_m2(lrf_kind) : nullptr;
 }
 const void *kernel_3d(int method, int cpl, int gzm) {
     return method == 0 ? kernel_3d_m0(cpl, gzm) : method == 1 ? kernel_3d_m1(cpl, gzm) : nullptr;
@@ -486,7 +678,7 @@ static int validate_grid(const ants_lrf *h, const ants_grid_params_t *g, int32_t
     if (!(g->factor > 0.f && g->factor < 1.f)) return ANTS_ERR_INVALID;
     if (!(g->step0_xy > 0.f) || !std::isfinite(g->step0_xy)) return ANTS_ERR_INVALID;
     if (g->seed_mode != 0 && g->seed_mode != 1) return ANTS_ERR_INVALID;
-    const bool lrf3 = h->dev.n_z > 0;
+    const bool lrf3 = h->dev.n_z > 0 || h->dev.lrf_kind == 5;     // the LRF depends on z
     if (g->dim == 3) {
         if (!lrf3) return ANTS_ERR_INVALID;
         if (!(g->step0_z > 0.f) || !std::isfinite(g->step0_z)) return ANTS_ERR_INVALID;
@@ -572,11 +764,39 @@ static int make_plan3d(const ants_lrf *h, const ants_grid_params_t *g, int32_t m
     return ANTS_OK;
 }
 
+// the general kernel: XY-type parameterisations, and axial LRFs that are not positive everywhere
+static int make_plan_gen(const ants_lrf *h, const ants_grid_params_t *g, int32_t method, Plan &pl) {
+    const ModelDev &m = h->dev;
+    const int G = g->nodes_per_axis;
+    const long long nodes = g->dim == 3 ? (long long)G * G * G : (long long)G * G;
+    if (nodes > 65535) return ANTS_ERR_UNSUPPORTED;
+    pl.family = 3;
+    pl.npt = (int)((nodes + 31) / 32);
+    pl.kernel = kernel_gen(method, m.lrf_kind);
+    if (!pl.kernel) return ANTS_ERR_UNSUPPORTED;
+    // FP64 scores from the first grid that reaches less than one knot interval of any spline axis from its
+    // centre (the grids the packed kernels score differentially)
+    pl.k_diff = g->n_iter;
+    const double half = 0.5 * (G - 1);
+    double knot = std::fmin(h->knot_r > 0.0 ? h->knot_r : 1e300, h->knot_xy > 0.0 ? h->knot_xy : 1e300);
+    const double plane = m.lrf_kind == 5 ? ((double)m.z_hi - (double)m.z_lo) / (m.n_planes - 1) : 1e300;
+    double hxy = g->step0_xy, hz = g->dim == 3 ? g->step0_z : 0.0;
+    for (int k = 0; k < g->n_iter; ++k, hxy *= (double)g->factor, hz *= (double)g->factor)
+        if (std::sqrt(2.0) * half * hxy * 1.001 <= 0.9 * knot && half * hz * 1.001 <= 0.9 * plane) { pl.k_diff = k; break; }
+    pl.k_series = pl.k_diff;
+    const int rows = (m.lrf_kind == 1 || m.lrf_kind == 4) ? m.n_lrf * (m.n_r + 1) : 0;
+    const int ncxy = m.lrf_kind >= 3 ? m.n_lrf * std::max(m.n_planes, 1) * (m.nx + 3) * (m.ny + 3) : 0;
+    pick_cta_shape(cta_smem_bytes_gen(m.N, rows, ncxy), warp_smem_bytes_gen(m.N), pl);
+    if (pl.smem > 227 * 1024) return ANTS_ERR_UNSUPPORTED;
+    return ANTS_OK;
+}
+
 // host-only part of the plan (no CUDA call): kernel variant, score switch-over, shared-memory carve-up
 static int make_plan(const ants_lrf *h, const ants_grid_params_t *g, int32_t method, Plan &pl) {
     int rc = validate_grid(h, g, method);
     if (rc != ANTS_OK) return rc;
     const ModelDev &m = h->dev;
+    if (m.lrf_kind >= 3 || (m.lrf_kind == 1 && !h->positive)) return make_plan_gen(h, g, method, pl);
     if (m.n_z > 0) {
         if (method == ANTS_CHI_SQUARE_SUMRATIO) return ANTS_ERR_UNSUPPORTED;   // axial LRFs only (R27)
         return make_plan3d(h, g, method, pl);
@@ -588,17 +808,14 @@ static int make_plan(const ants_lrf *h, const ants_grid_params_t *g, int32_t met
     for (int c : kNpt2D)
         if (c >= need) { pl.npt = c; break; }
     if (!pl.npt) return ANTS_ERR_UNSUPPORTED;
-    // strictly positive LRFs (the normal case) run the sensor-pair-packed kernel; others the generic one
-    const bool packed = h->positive;
-    if (!packed && m.select) return ANTS_ERR_UNSUPPORTED;   // the generic kernel has no sensor selection
-    pl.family = packed ? 0 : 1;
-    pl.kernel = packed ? kernel_2d_pk(method, pl.npt) : kernel_2d_gen(method, pl.npt);
+    // strictly positive axial LRFs (the normal case): the sensor-pair-packed kernel
+    pl.family = 0;
+    pl.kernel = kernel_2d_pk(method, pl.npt);
     if (!pl.kernel) return ANTS_ERR_UNSUPPORTED;
     pl.k_diff = first_diff_iter(h, g, method);
-    if (!packed && method == ANTS_CHI_SQUARE_SUMRATIO) pl.k_diff = g->n_iter;   // generic kernel: plain form only
     pl.k_series = pl.k_diff;
     const size_t tables = (cta_table_bytes(m.N, m.n_lrf * (m.n_r + 1)) + 15) / 16 * 16;
-    const size_t per_warp = packed ? warp_smem_bytes_pk(m.N, method) : warp_smem_bytes_2d(m.N);
+    const size_t per_warp = warp_smem_bytes_pk(m.N, method);
     pick_cta_shape(tables, per_warp, pl);
     if (pl.smem > 227 * 1024) return ANTS_ERR_UNSUPPORTED;
     return ANTS_OK;
@@ -647,9 +864,9 @@ static int get_plan(const ants_lrf *hc, const ants_grid_params_t *g, int32_t met
     return ANTS_OK;
 }
 
-static void kernel_name(const Plan &pl, int32_t method, char *buf, size_t n) {
+static void kernel_name(const Plan &pl, int32_t method, int lrf_kind, char *buf, size_t n) {
     if (pl.family == 0) std::snprintf(buf, n, "ants::recon2d_pk_kernel<%d,%d>", pl.npt, (int)method);
-    else if (pl.family == 1) std::snprintf(buf, n, "ants::recon2d_kernel<%d,%d,false>", pl.npt, (int)method);
+    else if (pl.family == 3) std::snprintf(buf, n, "ants::recon_gen_kernel<%d,%d>", (int)method, lrf_kind);
     else std::snprintf(buf, n, "ants::recon3d_kernel<%d,%d,%d>", pl.cpl, pl.gzm, (int)method);
 }
 
@@ -674,7 +891,7 @@ extern "C" int ants_plan_kernel_name(const ants_lrf_t *lrf, const ants_grid_para
     Plan pl;
     int rc = get_plan(lrf, grid, method, false, pl);
     if (rc != ANTS_OK) return rc;
-    kernel_name(pl, method, name_out, (size_t)name_cap);
+    kernel_name(pl, method, lrf->dev.lrf_kind, name_out, (size_t)name_cap);
     return ANTS_OK;
 }
 

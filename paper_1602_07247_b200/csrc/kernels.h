@@ -1,4 +1,4 @@
-// kernels.h -- the reconstruction kernels are instantiated in their own translation units (k_*.cu, compiled in
+// kernels.h -- the reconstruction kernels are instantiated in their own translation units (k2d_pk_m*.cu, k3d_m*.cu, kgen_m*.cu, compiled in
 // parallel by build.py); the host logic in ants_recon.cu picks one through these look-ups.  Each returns
 // nullptr for a combination that is not compiled.
 #pragma once
@@ -7,8 +7,9 @@ namespace ants {
 
 // axial LRFs, strictly positive: sensor-pair-packed kernel (recon2d_pk.cuh).  method 0/1/2, npt in {1,2,3,4,8}
 const void *kernel_2d_pk(int method, int npt);
-// axial LRFs that are not positive everywhere: scalar kernel with per-pair validity tests (recon2d.cuh)
-const void *kernel_2d_gen(int method, int npt);
+// the general kernel (recon_gen.cuh): XY, Composite and Sliced LRFs, and axial LRFs that are not positive
+// everywhere.  method 0/1/2, lrf_kind 1/3/4/5
+const void *kernel_gen(int method, int lrf_kind);
 // axial+z LRFs (recon3d.cuh).  method 0/1, (cpl, gzm) in {(1,1),(2,1),(3,1),(4,1),(8,1),(1,4),(2,4),(1,8),(2,8)}
 const void *kernel_3d(int method, int cpl, int gzm);
 

@@ -1,0 +1,15 @@
+// kgen_m2.cu -- instantiations of recon_gen_kernel<2, LRFK> (the general kernel: any LRF parameterisation)
+#include "recon_gen.cuh"
+#include "kernels.h"
+
+namespace ants {
+const void *kernel_gen_m2(int lrf_kind) {
+    switch (lrf_kind) {
+        case kAxial: return (const void *)recon_gen_kernel<2, kAxial>;
+        case kXY: return (const void *)recon_gen_kernel<2, kXY>;
+        case kComposite: return (const void *)recon_gen_kernel<2, kComposite>;
+        case kSliced: return (const void *)recon_gen_kernel<2, kSliced>;
+    }
+    return nullptr;
+}
+}  // namespace ants

@@ -24,6 +24,13 @@ struct ModelDev {
                             // axial+z: [n_z + 3][n_r + 1] such rows, one r-spline per z coefficient row
     const double *polyd;    // axial: [n_lrf][n_r][4] power basis in u = t - k in [0,1] (final score, FP64)
                             // axial+z: [n_z + 3][n_r][4]
+    // XY-type parameterisations (recon_gen.cuh): B-spline coefficients of the XY tables
+    // [n_lrf][n_planes or 1][ny + 3][nx + 3] (u fastest) and the sensors' local frames {T00, T01, T10, T11}
+    const float *cxy;       // device, or nullptr
+    const float4 *xf;       // device [N], or nullptr (identity)
+    int lrf_kind;           // 1 Axial, 2 Axial+Z, 3 XY, 4 Composite, 5 Sliced
+    int nx, ny, n_planes;
+    float u_lo, su, v_lo, sv;   // su = nx / (u_hi - u_lo), sv = ny / (v_hi - v_lo)
     int N, n_lrf, n_r, n_z;
     float r_lo, r_hi, sc, of, tmax;   // sc = n_r/(r_hi - r_lo); of = -r_lo*sc - 0.5; tmax = n_r - 0.5
     float z_lo, z_hi, scz;            // scz = n_z/(z_hi - z_lo)
@@ -173,6 +180,15 @@ __device__ __forceinline__ void strongest_sensor(const float2 *SC, const float4 
     cy = sens_s[bi].y;
 }
 
+// ---- step a1 for one event, shared by the kernels that do not prefetch: load the signals (coalesced), prepare
+// them (R18), centroid or strongest-sensor start (R20), sensor selection (R19).  SC[i] receives
+// {S_i, log2(S_i / gL_i) or 0}, an inactive sensor is flagged by NaN in .y.  Returns false when the event fails
+// (its outputs are written here: NaN row, score +inf, path 0xFFFF).
+struct Params;
+template <int METHOD>
+__device__ bool prepare_event(const Params &p, const float4 *sens_s, float2 *SC, long long e, int lane,
+                              float &sumS, float &cx, float &cy);
+
 // same result as warp_argmin through two integer reductions (REDUX): scores mapped to order-preserving
 // unsigned keys, then the lowest index among the lanes holding the minimum.  s must not be NaN.
 __device__ __forceinline__ void warp_argmin_redux(float &s, int &idx) {
@@ -206,6 +222,74 @@ __host__ __device__ inline size_t cta_table_bytes(int N, int rows) {
 
 __device__ __forceinline__ float horner(const float4 p, float v) {
     return fmaf(fmaf(fmaf(p.w, v, p.z), v, p.y), v, p.x);
+}
+
+template <int METHOD>
+__device__ bool prepare_event(const Params &p, const float4 *sens_s, float2 *SC, long long e, int lane,
+                              float &sumS, float &cx, float &cy) {
+    const ModelDev &m = p.m;
+    const int N = m.N;
+    const float *sig = p.signals + e * N;
+    float sw = 0.f, sxw = 0.f, syw = 0.f;
+    sumS = 0.f;
+    bool finite = true;
+    for (int i = lane; i < N; i += 32) {
+        if (m.passive && m.passive[i]) {             // R19: out of everything, signal not looked at
+            SC[i] = make_float2(0.f, ANTS_QNAN);
+            continue;
+        }
+        float S = __ldg(sig + i);
+        finite = finite && (fabsf(S) <= 3.402823466e38f);
+        if (METHOD == 0) S = fmaxf(S, 0.f);          // R18
+        const float4 sn = sens_s[i];
+        const float wgt = S * sn.w;
+        sumS += S;
+        sw += wgt;
+        sxw = fmaf(sn.x, wgt, sxw);
+        syw = fmaf(sn.y, wgt, syw);
+        float cs = 0.f;
+        if (METHOD == 0 && S > 0.f) cs = log2f(S / sn.z);
+        SC[i] = make_float2(S, cs);
+    }
+    finite = __all_sync(kFull, finite);
+    sumS = warp_sum(sumS);
+    sw = warp_sum(sw);
+    sxw = warp_sum(sxw);
+    syw = warp_sum(syw);
+    __syncwarp();
+    bool ok = finite && (sumS > 0.f) && (p.seed_mode != 0 || sw > 0.f);
+    if (ok) {
+        cx = sxw / sw;
+        cy = syw / sw;
+        if (p.seed_mode == 1) strongest_sensor(SC, sens_s, N, lane, cx, cy);    // R20
+        if (m.select) {
+            // R19: the sensors of the statistical part, fixed for the event: signal threshold and distance
+            // from the start position; sum S runs over them
+            float s_act = 0.f;
+            for (int i = lane; i < N; i += 32) {
+                const float2 sc = SC[i];
+                if (sc.y == sc.y) {
+                    const float4 sn = sens_s[i];
+                    const float dx = cx - sn.x, dy = cy - sn.y;
+                    const bool keep = !(sc.x < m.signal_min) && !(sqrtf(fmaf(dx, dx, dy * dy)) > m.dist_max);
+                    if (keep) s_act += sc.x;
+                    else SC[i] = make_float2(0.f, ANTS_QNAN);
+                }
+            }
+            sumS = warp_sum(s_act);
+            __syncwarp();
+            ok = sumS > 0.f;
+        }
+    }
+    if (!ok) {
+        if (lane == 0) {
+            reinterpret_cast<float4 *>(p.out_xyzA)[e] = make_float4(ANTS_QNAN, ANTS_QNAN, ANTS_QNAN, ANTS_QNAN);
+            p.out_score[e] = kInf;
+        }
+        if (p.out_path)
+            for (int k = lane; k < p.K; k += 32) p.out_path[e * p.K + k] = 0xFFFF;
+    }
+    return ok;
 }
 
 }  // namespace ants

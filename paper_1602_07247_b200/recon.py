@@ -34,6 +34,11 @@ class GridParams(C.Structure):
                 ("seed_mode", C.c_int32), ("z_seed", C.c_float)]
 
 
+class LrfXY(C.Structure):
+    _fields_ = [("n_int_x", C.c_int32), ("n_int_y", C.c_int32), ("n_planes", C.c_int32),
+                ("knots_xy", C.c_void_p), ("coeffs_xy", C.c_void_p), ("xform", C.c_void_p), ("group", C.c_void_p)]
+
+
 class FilterCriteria(C.Structure):
     _fields_ = [("score_max", C.c_float), ("energy_min", C.c_float), ("energy_max", C.c_float),
                 ("radius_max", C.c_float)]
@@ -56,6 +61,10 @@ def load():
     lib.ants_lrf_create.argtypes = [vp, vp, vp, vp, C.POINTER(LrfDims), C.POINTER(vp)]
     lib.ants_lrf_create_grouped.restype = C.c_int
     lib.ants_lrf_create_grouped.argtypes = [vp, vp, vp, vp, vp, C.POINTER(LrfDims), C.POINTER(vp)]
+    lib.ants_lrf_create_xy.restype = C.c_int
+    lib.ants_lrf_create_xy.argtypes = [vp, vp, vp, vp, C.POINTER(LrfDims), C.POINTER(LrfXY), C.POINTER(vp)]
+    lib.ants_group_by_symmetry.restype = C.c_int
+    lib.ants_group_by_symmetry.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32, C.c_float, vp, vp, i32p]
     lib.ants_group_by_radius.restype = C.c_int
     lib.ants_group_by_radius.argtypes = [vp, C.c_int32, C.c_float, vp, i32p]
     lib.ants_gains_renormalise.restype = C.c_int
@@ -132,6 +141,45 @@ def ants_lrf_create_grouped(sensor_xy, gains, group, knots, coeffs, dims: LrfDim
     if rc != 0:
         raise AntsError(rc, "ants_lrf_create_grouped")
     return out.value
+
+
+def ants_lrf_create_xy(sensor_xy, gains, knots, coeffs, dims: LrfDims, n_int_x: int, n_int_y: int, n_planes: int,
+                       knots_xy, coeffs_xy, xform=None, group=None) -> int:
+    """XY / Composite / Sliced model (include/ants_recon.h, dims.lrf_dim = 3 / 4 / 5).  knots and coeffs describe
+    the axial component of a Composite model (None otherwise).  -> opaque handle (int)."""
+    xy, kxy, cxy = _f32(sensor_xy), _f32(knots_xy), _f32(coeffs_xy)
+    g = None if gains is None else _f32(gains)
+    kn = None if knots is None else _f32(knots)
+    co = None if coeffs is None or np.size(coeffs) == 0 else _f32(coeffs)
+    xf = None if xform is None else _f32(xform)
+    gr = None if group is None else np.ascontiguousarray(np.asarray(group, dtype=np.int32))
+    n_tab = int(dims.n_lrf)
+    if cxy.size != n_tab * max(int(n_planes), 1) * (int(n_int_x) + 3) * (int(n_int_y) + 3) or kxy.size < (6 if dims.lrf_dim == 5 else 4):
+        raise ValueError("ants_lrf_create_xy: coeffs_xy / knots_xy size mismatch")
+    if xf is not None and xf.size != 4 * xy.size // 2:
+        raise ValueError("ants_lrf_create_xy: xform must be [N][4]")
+    desc = LrfXY(int(n_int_x), int(n_int_y), int(n_planes), kxy.ctypes.data, cxy.ctypes.data,
+                 None if xf is None else xf.ctypes.data, None if gr is None else gr.ctypes.data)
+    out = C.c_void_p()
+    rc = load().ants_lrf_create_xy(xy.ctypes.data, None if g is None else g.ctypes.data,
+                                   None if kn is None else kn.ctypes.data, None if co is None else co.ctypes.data,
+                                   C.byref(dims), C.byref(desc), C.byref(out))
+    if rc != 0:
+        raise AntsError(rc, "ants_lrf_create_xy")
+    return out.value
+
+
+def ants_group_by_symmetry(sensor_xy, n_fold: int, reflect: bool = True, tol: float = 1e-3):
+    """Symmetry groups and per-sensor frames (include/ants_recon.h).  -> (group int32 [N], xform float32 [N][4], n_groups)."""
+    xy = _f32(sensor_xy).reshape(-1, 2)
+    group = np.zeros(xy.shape[0], np.int32)
+    xform = np.zeros((xy.shape[0], 4), np.float32)
+    n = C.c_int32(0)
+    rc = load().ants_group_by_symmetry(xy.ctypes.data, xy.shape[0], int(n_fold), int(bool(reflect)), float(tol),
+                                       group.ctypes.data, xform.ctypes.data, C.byref(n))
+    if rc != 0:
+        raise AntsError(rc, "ants_group_by_symmetry")
+    return group, xform, int(n.value)
 
 
 def ants_group_by_radius(sensor_xy, tol: float = 1e-3):
@@ -352,7 +400,11 @@ class Reconstructor:
                                cfg.n_iter, int(getattr(cfg, "seed_mode", 0)), cfg.z_seed)
         self.method = int(cfg.method)
         group = getattr(cfg, "group", None)
-        if group is None:
+        if cfg.lrf_dim >= 3:
+            self.handle = ants_lrf_create_xy(cfg.sensor_xy, cfg.gains, cfg.knots if cfg.lrf_dim == 4 else None,
+                                             cfg.coeffs if cfg.lrf_dim == 4 else None, self.dims, cfg.n_int_x, cfg.n_int_y,
+                                             cfg.n_planes, cfg.knots_xy, cfg.coeffs_xy, getattr(cfg, "xform", None), group)
+        elif group is None:
             self.handle = ants_lrf_create(cfg.sensor_xy, cfg.gains, cfg.knots, cfg.coeffs, self.dims)
         else:
             self.handle = ants_lrf_create_grouped(cfg.sensor_xy, cfg.gains, group, cfg.knots, cfg.coeffs, self.dims)

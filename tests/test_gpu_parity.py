@@ -172,21 +172,83 @@ def test_chi_square_on_shared_profile_and_poisson_on_individual():
         parity_rules.assert_parity(res, f"cfg{idx} method={method}")
 
 
-def test_non_positive_spline_uses_validity_rules():
-    """An LRF that goes negative far out: the library must fall back to the per-pair validity
-    rule (a node with L_i <= 0 where S_i > 0 is invalid).  The differential late-iteration score
-    needs L > 0 everywhere, so such a model is scored in plain FP32 throughout (DESIGN.md
-    "Limits"): score, energy and node-index rules hold; the position rule is only required at
-    the FP32 resolution of the plain score (not the 99.9 % bar of the five configs)."""
-    cfg = synth.make_config(2)
+def _negative_tail(idx=2):
+    cfg = synth.make_config(idx)
     c = cfg.coeffs.copy()
     c[0, 0, -4:] = -0.002                # negative tail beyond ~75 mm
     cfg.coeffs = c
-    ev = synth.generate_events(synth.make_config(2), 2001, device="cuda")
+    return cfg
+
+
+@pytest.mark.parametrize("method", [0, 1, 2])
+def test_non_positive_spline_uses_validity_rules(method):
+    """An LRF that goes negative far out: the library must apply the per-pair validity rule (a node with
+    L_i <= 0 where S_i > 0 is invalid).  Such a model runs the general kernel (FP32 scores on the coarse grids,
+    FP64 on the fine ones) and meets the full north_star rule set."""
+    cfg = _negative_tail()
+    cfg.method = method
+    ev = synth.generate_events(synth.make_config(2), 4001, device="cuda")
+    r = recon.Reconstructor(cfg)
+    assert "recon_gen_kernel" in r.plan()["kernel"]
+    r.close()
     xyzA, score, path = _run(cfg, ev["signals"])
     res = parity_rules.compare(cfg, ev["signals"].cpu().numpy(), xyzA, score, path)
-    assert res["fail_mismatch"] == 0 and res["score_viol"] == 0 and res["A_viol"] == 0 and res["idx_viol"] == 0, res
-    assert res["pos_frac_within"] >= 0.9 and res["pos_max_steps"] <= 16.0, res
+    parity_rules.assert_parity(res, f"negative tail, method {method}")
+
+
+def test_non_positive_spline_with_sensor_selection_and_strongest_start():
+    """Sensor selection and the strongest-sensor start are available on the general kernel too."""
+    cfg = _negative_tail()
+    cfg.passive = np.zeros(cfg.n_sensors, np.uint8)
+    cfg.passive[[3, 11]] = 1
+    cfg.signal_min, cfg.dist_max, cfg.seed_mode = 4.0, 70.0, 1
+    ev = synth.generate_events(synth.make_config(2), 3001, device="cuda")
+    xyzA, score, path = _run(cfg, ev["signals"])
+    res = parity_rules.compare(cfg, ev["signals"].cpu().numpy(), xyzA, score, path)
+    parity_rules.assert_parity(res, "negative tail with selection")
+
+
+@pytest.mark.parametrize("idx,n,kw", [
+    (6, 6_007, {}), (6, 3_001, dict(method=0)), (6, 2_003, dict(method=2, nodes_per_axis=8)),
+    (7, 1_201, {}), (7, 801, dict(method=1, nodes_per_axis=5)), (7, 1_501, dict(dim=2, nodes_per_axis=9, z_seed=7.5)),
+    (8, 6_007, {}), (8, 3_001, dict(method=1, seed_mode=1)),
+])
+def test_parity_xy_composite_sliced_lrfs(idx, n, kw):
+    """XY LRFs shared by symmetry groups (config 6), Sliced LRFs searched in 3-D and at a fixed z (config 7) and
+    Composite LRFs (config 8): PAPER.md:388-396, 406; the general kernel under the full rule set."""
+    cfg = synth.make_config(idx)
+    for k, v in kw.items():
+        setattr(cfg, k, v)
+    ev = synth.generate_events(synth.make_config(idx), n, device="cuda")
+    r = recon.Reconstructor(cfg)
+    assert "recon_gen_kernel" in r.plan()["kernel"]
+    r.close()
+    xyzA, score, path = _run(cfg, ev["signals"])
+    res = parity_rules.compare(cfg, ev["signals"].cpu().numpy(), xyzA, score, path)
+    parity_rules.assert_parity(res, f"cfg{idx} {kw}")
+
+
+def test_xy_lrf_individual_tables_and_selection():
+    """XY LRFs with one table per sensor (no grouping, no frames) and sensor selection."""
+    base = synth.make_config(6)
+    cfg = synth.make_config(6)
+    cfg.n_lrf = cfg.n_sensors
+    cfg.coeffs_xy = np.ascontiguousarray(base.coeffs_xy[base.group])
+    cfg.group, cfg.xform = None, None
+    cfg.coeffs = np.zeros((cfg.n_sensors, 1, 0), np.float32)
+    cfg.signal_min, cfg.dist_max = 3.0, 25.0
+    ev = synth.generate_events(cfg, 2001, device="cuda")
+    xyzA, score, path = _run(cfg, ev["signals"])
+    parity_rules.assert_parity(parity_rules.compare(cfg, ev["signals"].cpu().numpy(), xyzA, score, path), "XY individual")
+
+
+def test_symmetry_groups_in_the_library_agree_with_the_oracle():
+    from oracle import fit as ofit
+    for xy, n_fold, reflect in ((synth.square_array(8, 6.0), 4, True), (synth.square_array(8, 6.0), 4, False),
+                                (synth.hex_array(3, 30.0), 6, True), (synth.hex_array(3, 30.0), 6, False)):
+        g, x, n = recon.ants_group_by_symmetry(xy, n_fold, reflect)
+        g0, x0, n0 = ofit.group_by_symmetry(xy, n_fold, reflect)
+        assert n == n0 and np.array_equal(g, g0) and np.abs(x - x0).max() <= 1e-6
 
 
 @pytest.mark.parametrize("lrf_dim,G,method", [(1, 2, 0), (1, 4, 0), (1, 6, 1), (1, 4, 2), (1, 8, 0), (2, 4, 0), (2, 6, 1)])
@@ -514,7 +576,7 @@ def test_parity_sum_ratio_least_squares(idx, n):
 
 
 def test_sum_ratio_least_squares_variants():
-    """Method 2 with sensor selection, the strongest-sensor start, a non-positive LRF (generic kernel) and the
+    """Method 2 with sensor selection, the strongest-sensor start, a non-positive LRF (general kernel) and the
     refusal for axial+z LRFs."""
     cfg = _with_selection(3, passive=[5, 40], signal_min=2.0)
     cfg.method, cfg.seed_mode = 2, 1
@@ -527,8 +589,7 @@ def test_sum_ratio_least_squares_variants():
     cfg.coeffs, cfg.method = c, 2
     ev = synth.generate_events(synth.make_config(2), 2001, device="cuda")
     xyzA, score, path = _run(cfg, ev["signals"])
-    res = parity_rules.compare(cfg, ev["signals"].cpu().numpy(), xyzA, score, path)
-    assert res["fail_mismatch"] == 0 and res["score_viol"] == 0 and res["A_viol"] == 0 and res["idx_viol"] == 0, res
+    parity_rules.assert_parity(parity_rules.compare(cfg, ev["signals"].cpu().numpy(), xyzA, score, path), "negative tail")
     cfg = synth.make_config(4)
     cfg.method = 2
     with pytest.raises(recon.AntsError) as ei:

@@ -515,3 +515,311 @@ int oracle_score_at_many(const oracle_model_t *m, const float *signals, int64_t 
                         A_out + e, score_out + e);
     return 0;
 }
+
+/* =====================================================================================================
+ * Continuous refinement of a reconstructed position (section 5.1.2: "The best match position is
+ * found using either the algorithms provided in the Minuit2 minimization library ... or the contracting
+ * grids method"; section 5.1.2.1: gradient-based minimisation "versus two (XY) or three
+ * (XYZ) spatial coordinates", started from a given position).  Minuit2 itself is out of scope; reading R34
+ * states the minimiser that takes its role here, started from a contracting-grid result:
+ *
+ *   objective F(p) = the node score of section 5.1.2.2 with the energy eliminated by its closed form
+ *       (R2-R4, R27), over the event's active sensors (R19);
+ *   model derivative m_i = d(A L_i)/dp = A dL_i/dp + L_i dA/dp, with dA/dp from the closed form
+ *       (Poisson and method 2: A = sum S / sum L  ->  dA = -A sum dL / sum L;
+ *        method 1: A = P/Q, P = sum w S L, Q = sum w L^2  ->  dA = (dP Q - P dQ)/Q^2);
+ *   gradient g = 2 sum (1 - S_i/mu_i) m_i (Poisson), g = -2 sum w_i (S_i - mu_i) m_i (least squares);
+ *   Gauss-Newton (Fisher) matrix H = 2 sum m_i m_i^T / mu_i (Poisson, terms with mu_i > 0),
+ *       H = 2 sum w_i m_i m_i^T (least squares);
+ *   Levenberg-Marquardt iteration with the damping update of Nielsen (Madsen, Nielsen, Tingleff, "Methods for
+ *       non-linear least squares problems", 2004, algorithm 3.16), n_steps times: solve (H + lambda I) delta =
+ *       -g; evaluate F, g, H at p + delta; gain ratio rho = (F - F_new) / (delta.(lambda delta - g) / 2);
+ *       rho > 0: accept, lambda <- lambda max(1/3, 1 - (2 rho - 1)^3), nu <- 2; else keep p, lambda <-
+ *       lambda nu, nu <- 2 nu.  lambda starts at 1e-3 max_a H_aa, nu at 2; a trial z outside the LRF's z range
+ *       is moved to the nearest end of the range (projected step, delta taken as the projected one); a trial
+ *       point that is invalid by the validity rules of the score, or a system without positive pivots, is a
+ *       rejected step.
+ * Spline derivatives are analytic (the B-spline basis differentiated); a clamped coordinate (R5) has zero
+ * derivative; at r = 0 the radial direction is undefined and the axial gradient is taken as 0.
+ * Pins (tests/test_oracle_refine.py): gradient against central differences of the pinned score; final point
+ * against scipy.optimize.minimize on the same score from the same start; F never increases.
+ * ===================================================================================================== */
+static void dbasis4(double u, double d[4])
+{
+    d[0] = -(1.0 - u) * (1.0 - u) / 2.0;
+    d[1] = (9.0 * u * u - 12.0 * u) / 6.0;
+    d[2] = (-9.0 * u * u + 6.0 * u + 3.0) / 6.0;
+    d[3] = u * u / 2.0;
+}
+
+/* value and derivative d/dx of the 1-D spline (0 outside [lo, hi], where the argument is clamped) */
+static double spline1_d(const float *c, int n, double lo, double hi, double x, double *ds)
+{
+    int k; double u, b[4], d[4];
+    locate(x, lo, hi, n, &k, &u);
+    basis4(u, b);
+    dbasis4(u, d);
+    double h = (hi - lo) / n;
+    *ds = (x < lo || x > hi) ? 0.0
+        : ((double)c[k] * d[0] + (double)c[k + 1] * d[1] + (double)c[k + 2] * d[2] + (double)c[k + 3] * d[3]) / h;
+    return (double)c[k] * b[0] + (double)c[k + 1] * b[1] + (double)c[k + 2] * b[2] + (double)c[k + 3] * b[3];
+}
+
+/* value and partial derivatives of the tensor-product spline c[nb+3][na+3] at (a, b) */
+static double spline2_d(const float *c, int na, int nb, double a_lo, double a_hi, double b_lo, double b_hi,
+                        double a, double b, double *d_a, double *d_b)
+{
+    int ka, kb; double ua, ub, ba[4], bb[4], da[4], db[4], s = 0.0, sa = 0.0, sb = 0.0;
+    locate(a, a_lo, a_hi, na, &ka, &ua);
+    locate(b, b_lo, b_hi, nb, &kb, &ub);
+    basis4(ua, ba); basis4(ub, bb);
+    dbasis4(ua, da); dbasis4(ub, db);
+    for (int j = 0; j < 4; ++j)
+        for (int i = 0; i < 4; ++i) {
+            double cc = (double)c[(kb + j) * (na + 3) + ka + i];
+            s += cc * ba[i] * bb[j];
+            sa += cc * da[i] * bb[j];
+            sb += cc * ba[i] * db[j];
+        }
+    *d_a = (a < a_lo || a > a_hi) ? 0.0 : sa / ((a_hi - a_lo) / na);
+    *d_b = (b < b_lo || b > b_hi) ? 0.0 : sb / ((b_hi - b_lo) / nb);
+    return s;
+}
+
+/* L_i(p) and its gradient with respect to (x, y, z) */
+double oracle_lrf_grad(const oracle_model_t *m, int i, double x, double y, double z, double grad[3])
+{
+    double dx = x - (double)m->sensor_xy[2 * i], dy = y - (double)m->sensor_xy[2 * i + 1];
+    double r = sqrt(dx * dx + dy * dy);
+    double ex = r > 0.0 ? dx / r : 0.0, ey = r > 0.0 ? dy / r : 0.0;     /* dr/dx, dr/dy */
+    size_t tab = (size_t)(m->group ? m->group[i] : (m->n_lrf == 1 ? 0 : i));
+    double g = (m->group || m->n_lrf == 1) ? (double)m->gains[i] : 1.0;
+    double s = 0.0, gx = 0.0, gy = 0.0, gz = 0.0;
+    if (m->lrf_dim == 1 || m->lrf_dim == 4) {
+        double ds;
+        s += spline1_d(m->coeffs + tab * (size_t)(m->n_int_r + 3), m->n_int_r, m->knots[0], m->knots[1], r, &ds);
+        gx += ds * ex; gy += ds * ey;
+    }
+    if (m->lrf_dim == 2) {
+        double dr, dz;
+        s += spline2_d(m->coeffs + tab * (size_t)((m->n_int_r + 3) * (m->n_int_z + 3)), m->n_int_r, m->n_int_z,
+                       m->knots[0], m->knots[1], m->knots[2], m->knots[3], r, z, &dr, &dz);
+        gx += dr * ex; gy += dr * ey; gz += dz;
+    }
+    if (m->lrf_dim >= 3) {
+        double T[4] = { 1.0, 0.0, 0.0, 1.0 };
+        if (m->xform) for (int j = 0; j < 4; ++j) T[j] = (double)m->xform[4 * i + j];
+        double u = T[0] * dx + T[1] * dy, v = T[2] * dx + T[3] * dy;
+        const float *kx = m->knots_xy;
+        size_t per_plane = (size_t)(m->n_int_x + 3) * (size_t)(m->n_int_y + 3);
+        double su, sv, val;
+        if (m->lrf_dim == 5) {
+            double z_lo = (double)kx[4], z_hi = (double)kx[5];
+            double dzp = (z_hi - z_lo) / (m->n_planes - 1);
+            double zc = z < z_lo ? z_lo : (z > z_hi ? z_hi : z);
+            int p = (int)floor((zc - z_lo) / dzp);
+            if (p > m->n_planes - 2) p = m->n_planes - 2;
+            if (p < 0) p = 0;
+            double w = (zc - (z_lo + p * dzp)) / dzp;
+            const float *c0 = m->coeffs_xy + (tab * (size_t)m->n_planes + (size_t)p) * per_plane;
+            double su0, sv0, su1, sv1;
+            double s0 = spline2_d(c0, m->n_int_x, m->n_int_y, kx[0], kx[1], kx[2], kx[3], u, v, &su0, &sv0);
+            double s1 = spline2_d(c0 + per_plane, m->n_int_x, m->n_int_y, kx[0], kx[1], kx[2], kx[3], u, v, &su1, &sv1);
+            val = (1.0 - w) * s0 + w * s1;
+            su = (1.0 - w) * su0 + w * su1;
+            sv = (1.0 - w) * sv0 + w * sv1;
+            gz += (z < z_lo || z > z_hi) ? 0.0 : (s1 - s0) / dzp;
+        } else {
+            val = spline2_d(m->coeffs_xy + tab * per_plane, m->n_int_x, m->n_int_y, kx[0], kx[1], kx[2], kx[3], u, v, &su, &sv);
+        }
+        s += val;
+        gx += su * T[0] + sv * T[2];          /* du/dx = T00, dv/dx = T10 */
+        gy += su * T[1] + sv * T[3];
+    }
+    grad[0] = g * gx; grad[1] = g * gy; grad[2] = g * gz;
+    return g * s;
+}
+
+/* F, A, g[3], H[3][3] at p over the active sensors; dim = 2: (x, y), 3: (x, y, z).  Returns 0 valid, 1 invalid. */
+static int score_grad_prepared(const oracle_model_t *m, const double *S, const uint8_t *active, int method, int dim,
+                               const double p[3], double *A_out, double *F_out, double g[3], double H[9])
+{
+    int N = m->n_sensors;
+    double z_lo, z_hi;
+    *A_out = NAN; *F_out = INFINITY;
+    for (int a = 0; a < 3; ++a) g[a] = 0.0;
+    for (int a = 0; a < 9; ++a) H[a] = 0.0;
+    if (z_range(m, &z_lo, &z_hi) && !(p[2] >= z_lo && p[2] <= z_hi)) return 1;
+    double *L = (double *)malloc(sizeof(double) * 4 * (size_t)N), *dL = L + N;     /* L[N], dL[N][3] */
+    double sumL = 0.0, sumS = 0.0, sdL[3] = { 0, 0, 0 }, P = 0.0, Q = 0.0, dP[3] = { 0, 0, 0 }, dQ[3] = { 0, 0, 0 };
+    for (int i = 0; i < N; ++i) {
+        if (active && !active[i]) continue;
+        L[i] = oracle_lrf_grad(m, i, p[0], p[1], p[2], dL + 3 * i);
+        if (dim == 2) dL[3 * i + 2] = 0.0;
+        double w = 1.0 / (S[i] > 1.0 ? S[i] : 1.0);
+        sumL += L[i]; sumS += S[i];
+        P += w * S[i] * L[i]; Q += w * L[i] * L[i];
+        for (int a = 0; a < 3; ++a) {
+            sdL[a] += dL[3 * i + a];
+            dP[a] += w * S[i] * dL[3 * i + a];
+            dQ[a] += 2.0 * w * L[i] * dL[3 * i + a];
+        }
+    }
+    int bad = !(sumL > 0.0) || (method == 1 && !(Q > 0.0));
+    double A = 0.0, dA[3] = { 0, 0, 0 }, F = 0.0;
+    if (!bad) {
+        if (method == 1) { A = P / Q; for (int a = 0; a < 3; ++a) dA[a] = (dP[a] * Q - P * dQ[a]) / (Q * Q); }
+        else { A = sumS / sumL; for (int a = 0; a < 3; ++a) dA[a] = -A * sdL[a] / sumL; }
+        for (int i = 0; i < N && !bad; ++i) {
+            if (active && !active[i]) continue;
+            double mu = A * L[i], mi[3];
+            for (int a = 0; a < 3; ++a) mi[a] = A * dL[3 * i + a] + L[i] * dA[a];
+            if (method == 0) {
+                if (S[i] > 0.0) {
+                    if (!(L[i] > 0.0)) { bad = 1; break; }
+                    F += mu - S[i] - S[i] * log(mu / S[i]);
+                } else {
+                    F += mu;
+                }
+                if (mu > 0.0) {
+                    double q = 1.0 - S[i] / mu;
+                    for (int a = 0; a < 3; ++a) {
+                        g[a] += 2.0 * q * mi[a];
+                        for (int b = 0; b < 3; ++b) H[3 * a + b] += 2.0 * mi[a] * mi[b] / mu;
+                    }
+                }
+            } else {
+                double w = 1.0 / (S[i] > 1.0 ? S[i] : 1.0), d = S[i] - mu;
+                F += w * d * d;
+                for (int a = 0; a < 3; ++a) {
+                    g[a] += -2.0 * w * d * mi[a];
+                    for (int b = 0; b < 3; ++b) H[3 * a + b] += 2.0 * w * mi[a] * mi[b];
+                }
+            }
+        }
+        if (method == 0) F *= 2.0;
+    }
+    free(L);
+    if (bad) return 1;
+    *A_out = A; *F_out = F;
+    return 0;
+}
+
+/* solve (H + lambda I) delta = -g for the leading dim x dim block by Gaussian elimination without
+ * pivoting (the matrix is symmetric positive definite when the step is usable); returns 0 ok, 1 no step */
+static int lm_step(const double H[9], const double g[3], double lambda, int dim, double delta[3])
+{
+    double M[3][4];
+    for (int a = 0; a < dim; ++a) {
+        for (int b = 0; b < dim; ++b) M[a][b] = H[3 * a + b];
+        M[a][a] += lambda;
+        M[a][dim] = -g[a];
+    }
+    for (int a = 0; a < dim; ++a) {
+        if (!(M[a][a] > 0.0) || !isfinite(M[a][a])) return 1;
+        for (int r = a + 1; r < dim; ++r) {
+            double f = M[r][a] / M[a][a];
+            for (int c = a; c <= dim; ++c) M[r][c] -= f * M[a][c];
+        }
+    }
+    delta[0] = delta[1] = delta[2] = 0.0;
+    for (int a = dim - 1; a >= 0; --a) {
+        double s = M[a][dim];
+        for (int c = a + 1; c < dim; ++c) s -= M[a][c] * delta[c];
+        delta[a] = s / M[a][a];
+    }
+    for (int a = 0; a < dim; ++a) if (!isfinite(delta[a])) return 1;
+    return 0;
+}
+
+/* gradient and Gauss-Newton matrix of one event at one position (for the pins) */
+int oracle_score_grad(const oracle_model_t *m, const float *sig, int method, int seed_mode, int dim,
+                      double x, double y, double z, double *A_out, double *F_out, double g[3], double H[9])
+{
+    int N = m->n_sensors;
+    double *S = (double *)malloc(sizeof(double) * (size_t)N);
+    uint8_t *active = 0;
+    prepare_signals(sig, N, method, S);
+    if (needs_selection(m)) {
+        double xy[2];
+        active = (uint8_t *)malloc((size_t)(unsigned)N);
+        if (oracle_start(m, sig, method, seed_mode, xy) || select_sensors(m, S, xy, active) == 0) {
+            free(S); free(active);
+            *A_out = NAN; *F_out = INFINITY;
+            return 1;
+        }
+    }
+    double p[3] = { x, y, z };
+    int rc = score_grad_prepared(m, S, active, method, dim, p, A_out, F_out, g, H);
+    free(S); free(active);
+    return rc;
+}
+
+static void refine_one(const oracle_model_t *m, const float *sig, int method, int seed_mode, int dim, int n_steps,
+                       double *xyzA, double *score)
+{
+    int N = m->n_sensors;
+    double xy0[2];
+    if (!(isfinite(xyzA[0]) && isfinite(xyzA[1]) && isfinite(xyzA[2]))) return;       /* failed event: left as it is */
+    if (oracle_start(m, sig, method, seed_mode, xy0)) { xyzA[0] = xyzA[1] = xyzA[2] = xyzA[3] = NAN; *score = INFINITY; return; }
+    double *S = (double *)malloc(sizeof(double) * (size_t)N);
+    uint8_t *active = 0;
+    prepare_signals(sig, N, method, S);
+    if (needs_selection(m)) {
+        active = (uint8_t *)malloc((size_t)(unsigned)N);
+        if (select_sensors(m, S, xy0, active) == 0) { free(S); free(active); xyzA[0] = xyzA[1] = xyzA[2] = xyzA[3] = NAN; *score = INFINITY; return; }
+    }
+    double p[3] = { xyzA[0], xyzA[1], xyzA[2] }, A, F, g[3], H[9];
+    if (score_grad_prepared(m, S, active, method, dim, p, &A, &F, g, H) == 0) {
+        double hmax = 0.0, nu = 2.0;
+        for (int a = 0; a < dim; ++a) if (H[3 * a + a] > hmax) hmax = H[3 * a + a];
+        double lambda = 1e-3 * hmax;
+        for (int it = 0; it < n_steps; ++it) {
+            double delta[3], q[3], A2, F2, g2[3], H2[9], rho = -1.0;
+            int ok = lm_step(H, g, lambda, dim, delta) == 0;
+            if (ok) {
+                for (int a = 0; a < 3; ++a) q[a] = p[a] + delta[a];
+                double z_lo, z_hi;
+                if (dim == 3 && z_range(m, &z_lo, &z_hi)) {        /* projected step: z stays in its range (R6) */
+                    q[2] = q[2] < z_lo ? z_lo : (q[2] > z_hi ? z_hi : q[2]);
+                    delta[2] = q[2] - p[2];
+                }
+                ok = score_grad_prepared(m, S, active, method, dim, q, &A2, &F2, g2, H2) == 0;
+            }
+            if (ok) {
+                double pred = 0.0;
+                for (int a = 0; a < dim; ++a) pred += 0.5 * delta[a] * (lambda * delta[a] - g[a]);
+                rho = pred > 0.0 ? (F - F2) / pred : -1.0;
+            }
+            if (ok && rho > 0.0) {
+                for (int a = 0; a < 3; ++a) { p[a] = q[a]; g[a] = g2[a]; }
+                for (int a = 0; a < 9; ++a) H[a] = H2[a];
+                A = A2; F = F2;
+                double t = 2.0 * rho - 1.0, f = 1.0 - t * t * t;
+                lambda *= f > 1.0 / 3.0 ? f : 1.0 / 3.0;
+                nu = 2.0;
+            } else {
+                lambda *= nu;
+                nu *= 2.0;
+            }
+        }
+        xyzA[0] = p[0]; xyzA[1] = p[1]; xyzA[2] = p[2]; xyzA[3] = A; *score = F;
+    } else {
+        xyzA[3] = NAN; *score = INFINITY;          /* the start point itself is invalid: position kept, no result */
+    }
+    free(S); free(active);
+}
+
+/* xyzA [E][4] in/out (x, y, z start; A out), score [E] out */
+int oracle_refine(const oracle_model_t *m, const float *signals, int64_t n_events, int method, int seed_mode, int dim,
+                  int n_steps, double *xyzA, double *score, int n_threads)
+{
+    if (!m || !signals || !xyzA || !score || n_events < 0 || n_steps < 0 || (dim != 2 && dim != 3)) return -1;
+    if (dim == 3 && m->lrf_dim != 2 && m->lrf_dim != 5) return -1;
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static) num_threads(oracle_threads(n_threads))
+#endif
+    for (int64_t e = 0; e < n_events; ++e)
+        refine_one(m, signals + e * m->n_sensors, method, seed_mode, dim, n_steps, xyzA + 4 * e, score + e);
+    return 0;
+}

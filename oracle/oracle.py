@@ -70,6 +70,14 @@ def _load():
         lib.oracle_reconstruct.argtypes = [C.POINTER(_Model), C.c_void_p, C.c_int64, C.POINTER(_Grid),
                                            C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                            C.c_void_p, C.c_int]
+        lib.oracle_lrf_grad.restype = C.c_double
+        lib.oracle_lrf_grad.argtypes = [C.POINTER(_Model), C.c_int, C.c_double, C.c_double, C.c_double, C.c_void_p]
+        lib.oracle_score_grad.restype = C.c_int
+        lib.oracle_score_grad.argtypes = [C.POINTER(_Model), C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double,
+                                          C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_void_p, C.c_void_p]
+        lib.oracle_refine.restype = C.c_int
+        lib.oracle_refine.argtypes = [C.POINTER(_Model), C.c_void_p, C.c_int64, C.c_int, C.c_int, C.c_int, C.c_int,
+                                      C.c_void_p, C.c_void_p, C.c_int]
         _lib = lib
     return _lib
 
@@ -165,6 +173,36 @@ class Model:
         _load().oracle_score_at(C.byref(self.c), s.ctypes.data, int(method), int(seed_mode), float(x), float(y),
                                 float(z), C.byref(A), C.byref(sc))
         return A.value, sc.value
+
+
+def lrf_grad(model: Model, i, x, y, z=0.0):
+    """(L_i, dL_i/d(x, y, z)) at a position."""
+    g = np.zeros(3)
+    v = _load().oracle_lrf_grad(C.byref(model.c), int(i), float(x), float(y), float(z), g.ctypes.data)
+    return v, g
+
+
+def score_grad(model: Model, signals, method, x, y, z=0.0, dim=2, seed_mode=0):
+    """(A, F, gradient [3], Gauss-Newton matrix [3][3], rc) of one event at a position (R34)."""
+    s = _f32(signals)
+    A, F, g, H = C.c_double(), C.c_double(), np.zeros(3), np.zeros((3, 3))
+    rc = _load().oracle_score_grad(C.byref(model.c), s.ctypes.data, int(method), int(seed_mode), int(dim), float(x),
+                                   float(y), float(z), C.byref(A), C.byref(F), g.ctypes.data, H.ctypes.data)
+    return A.value, F.value, g, H, rc
+
+
+def refine(model: Model, signals, method, xyz_start, n_steps, dim=2, seed_mode=0, threads=0):
+    """Levenberg-Marquardt refinement (R34) from xyz_start [E][3].  -> dict xyzA [E][4], score [E] (float64)."""
+    s = _f32(signals).reshape(-1, model.n_sensors)
+    E = s.shape[0]
+    xyzA = np.zeros((E, 4))
+    xyzA[:, :3] = np.asarray(xyz_start, np.float64).reshape(E, 3)
+    score = np.full(E, np.inf)
+    rc = _load().oracle_refine(C.byref(model.c), s.ctypes.data, E, int(method), int(seed_mode), int(dim), int(n_steps),
+                               xyzA.ctypes.data, score.ctypes.data, int(threads))
+    if rc != 0:
+        raise ValueError("oracle_refine: invalid argument")
+    return {"xyzA": xyzA, "score": score}
 
 
 def score_at_many(model: Model, signals, method: int, pos, seed_mode: int = 0):

@@ -573,6 +573,64 @@ def run_cycle(args):
     return 0
 
 
+def run_refine(args):
+    """Times `--grid-iters` contracting-grid iterations followed by `--refine-steps` Levenberg-Marquardt steps
+    (ants_refine, the role Minuit2 plays in PAPER.md:320-324) against the config's full grid search, on the same
+    batch.  Secondary workload (`--workload refine`)."""
+    import copy
+    import torch
+    from paper_1602_07247_b200 import recon, synth
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    device = torch.device("cuda", 0)
+    cfg = synth.make_config(args.config)
+    E = cfg.n_events // cfg.n_batches if args.events is None else args.events
+    sig = synth.generate_events(cfg, E, device=device)["signals"]
+    short = copy.copy(cfg)
+    short.n_iter = args.grid_iters
+    r_full, r_short = recon.Reconstructor(cfg), recon.Reconstructor(short)
+    xyzA = torch.empty((E, 4), dtype=torch.float32, device=device)
+    score = torch.empty((E,), dtype=torch.float32, device=device)
+    stream = torch.cuda.current_stream()
+
+    def full():
+        recon.ants_reconstruct(r_full.handle, sig, r_full.grid, r_full.method, xyzA, score, stream.cuda_stream)
+
+    def hybrid():
+        recon.ants_reconstruct(r_short.handle, sig, r_short.grid, r_short.method, xyzA, score, stream.cuda_stream)
+        recon.ants_refine(r_short.handle, sig, cfg.method, xyzA, score, args.refine_steps, dim=cfg.dim)
+
+    out = {}
+    for name, fn in (("grid_only", full), ("grid_then_refine", hybrid)):
+        for _ in range(args.warmup):
+            fn()
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+        n0 = recon.launch_count()
+        for a, b in ev:
+            a.record(stream)
+            fn()
+            b.record(stream)
+        torch.cuda.synchronize()
+        ms = [a.elapsed_time(b) for a, b in ev]
+        t = sum(ms) / len(ms) * 1e-3
+        ok = torch.isfinite(score)
+        out[name] = {"events_per_s": E / t, "ms_per_step": t * 1e3, "gpu_launches": recon.launch_count() - n0,
+                     "mean_score": float(score[ok].double().mean())}
+    r_full.close()
+    r_short.close()
+    print(json.dumps({"metric": "events/s: contracting grid alone vs a shorter grid followed by continuous refinement",
+                      "value": out["grid_then_refine"]["events_per_s"], "unit": "events/s", "n_gpus": 1,
+                      "steps": args.steps, "warmup": args.warmup, "ms_per_step": out["grid_then_refine"]["ms_per_step"],
+                      "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32 grid + f64 refinement",
+                      "data": "synthetic",
+                      "config": {"workload": cfg.name + " grid + refinement", "events_per_step_per_gpu": E,
+                                 "grid_iters": args.grid_iters, "refine_steps": args.refine_steps,
+                                 "grid_iters_of_the_config": cfg.n_iter},
+                      "results": out, "speedup_vs_grid_only": out["grid_then_refine"]["events_per_s"] / out["grid_only"]["events_per_s"]}),
+          flush=True)
+    return 0
+
+
 def main(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -590,7 +648,9 @@ def main(argv=None):
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--ref-step-seconds", type=float, default=4.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--workload", default="reconstruct", choices=["reconstruct", "fit", "cycle", "peak"],
+    ap.add_argument("--grid-iters", type=int, default=5, help="--workload refine: grid iterations before the refinement")
+    ap.add_argument("--refine-steps", type=int, default=6, help="--workload refine: Levenberg-Marquardt steps")
+    ap.add_argument("--workload", default="reconstruct", choices=["reconstruct", "fit", "cycle", "peak", "refine"],
                     help="fit = time the LRF calculation instead (secondary; not the BASELINE metric)")
     args = ap.parse_args(argv)
     if args.warmup < 3 and args.impl == "ours":
@@ -601,6 +661,8 @@ def main(argv=None):
         return run_cycle(args)
     if args.workload == "peak":
         return run_peak(args)
+    if args.workload == "refine":
+        return run_refine(args)
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)

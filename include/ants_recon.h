@@ -237,6 +237,28 @@ int ants_reconstruct_host(const ants_lrf_t *lrf, const float *signals_host, int6
                           float *out_xyzA_host, float *out_score_host, int64_t chunk_events);
 
 /*
+ * ants_refine -- continuous refinement of reconstructed positions (section 5.1.2: "The best match
+ * position is found using either the algorithms provided in the Minuit2 minimization library ... or the
+ * contracting grids method"; section 5.1.2.1: minimisation "versus two (XY) or three (XYZ)
+ * spatial coordinates", started from a given position).  Reading R34: Levenberg-Marquardt with
+ * Nielsen's damping update on the score of `method` with the energy eliminated by its closed form, analytic
+ * spline derivatives, Gauss-Newton (Fisher) matrix, n_steps evaluations after the start point; a trial z outside
+ * the LRF's z range is projected onto it; the score never increases.  Typical use: ants_reconstruct with about
+ * five grid iterations, then a few steps here instead of the remaining grid iterations.
+ *   signals DEVICE [n_events][N];  xyzA DEVICE [n_events][4], IN: start position x, y, z (the energy is ignored),
+ *   OUT: refined position and its energy;  score DEVICE [n_events], OUT: the score there.
+ *   dim 2: (x, y) at the given z; 3: (x, y, z), needs an LRF that depends on z.  seed_mode as in the grid
+ *   parameters (it fixes the start position that the distance selection refers to, R19).
+ * Rows whose start position is not finite (failed events) are left untouched; an event that is unusable (as in
+ * ants_reconstruct) becomes a NaN row with score +inf; a start point that is itself an invalid node keeps its
+ * position and gets energy NaN, score +inf.  Everything is computed in FP64 (one warp per event, lanes over
+ * sensors), one kernel launch, asynchronous on `cuda_stream`.  Every LRF parameterisation is supported.
+ * Errors: ANTS_ERR_INVALID, ANTS_ERR_UNSUPPORTED (tables exceed the shared memory), ANTS_ERR_CUDA.
+ */
+int ants_refine(const ants_lrf_t *lrf, const float *signals, int64_t n_events, int32_t method, int32_t dim,
+                int32_t seed_mode, int32_t n_steps, float *xyzA, float *score, void *cuda_stream);
+
+/*
  * ants_lrf_fit_axial -- LRF calculation (section 6: "The LRF module calculates these
  * functions from datasets containing photosensor signals and the corresponding event positions";
  * one LRF per sensor or one per group with relative gains; positions reconstructed

@@ -18,6 +18,7 @@
 #include "recon2d_pk.cuh"
 #include "recon3d.cuh"
 #include "recon_gen.cuh"
+#include "refine.cuh"
 #include "kernels.h"
 
 using namespace ants;
@@ -648,6 +649,7 @@ namespace ants {
 const void *kernel_2d_pk_m0(int), *kernel_2d_pk_m1(int), *kernel_2d_pk_m2(int);
 const void *kernel_gen_m0(int), *kernel_gen_m1(int), *kernel_gen_m2(int);
 const void *kernel_3d_m0(int, int), *kernel_3d_m1(int, int);
+const void *kernel_refine(int);
 const void *kernel_2d_pk(int method, int npt) {
     return method == 0 ? kernel_2d_pk_m0(npt) : method == 1 ? kernel_2d_pk_m1(npt) : method == 2 ? kernel_2d_pk_m2(npt) : nullptr;
 }
@@ -1050,6 +1052,55 @@ extern "C" int ants_reconstruct_host(const ants_lrf_t *lrf, const float *signals
     for (int s = 0; s < 3; ++s)
         if (cudaStreamSynchronize(h->streams[s]) != cudaSuccess) { cudaGetLastError(); if (rc == ANTS_OK) rc = ANTS_ERR_CUDA; }
     return rc;
+}
+
+// ---------------------------------------------------------------------------
+// continuous refinement (refine.cuh): one launch, FP64, lanes over sensors
+// ---------------------------------------------------------------------------
+extern "C" int ants_refine(const ants_lrf_t *lrf, const float *signals, int64_t n_events, int32_t method,
+                           int32_t dim, int32_t seed_mode, int32_t n_steps, float *xyzA, float *score,
+                           void *cuda_stream) {
+    if (!lrf) return ANTS_ERR_INVALID;
+    if (method != ANTS_POISSON_ML && method != ANTS_CHI_SQUARE && method != ANTS_CHI_SQUARE_SUMRATIO) return ANTS_ERR_INVALID;
+    if ((dim != 2 && dim != 3) || (seed_mode != 0 && seed_mode != 1) || n_steps < 0 || n_steps > 10000 || n_events < 0)
+        return ANTS_ERR_INVALID;
+    const ModelDev &m = lrf->dev;
+    const bool zdep = m.lrf_kind == 2 || m.lrf_kind == 5;
+    if (dim == 3 && !zdep) return ANTS_ERR_INVALID;
+    if (n_events == 0) return ANTS_OK;
+    if (!signals || !xyzA || !score) return ANTS_ERR_INVALID;
+    int dev_now = -1;
+    if (cudaGetDevice(&dev_now) != cudaSuccess) { cudaGetLastError(); return ANTS_ERR_CUDA; }
+    if (dev_now != lrf->device) return ANTS_ERR_INVALID;
+    const void *kernel = kernel_refine(method);
+    const int warps = 8;
+    const int ncxy = m.lrf_kind >= 3 ? m.n_lrf * std::max(m.n_planes, 1) * (m.nx + 3) * (m.ny + 3) : 0;
+    const size_t smem = cta_smem_bytes_gen(m.N, 0, ncxy) + (size_t)warps * ((size_t)m.N * 40 + 8);
+    if (smem > 227 * 1024) return ANTS_ERR_UNSUPPORTED;
+    int occ = 0;
+    if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, warps * 32, smem) != cudaSuccess || occ < 1) {
+        cudaGetLastError();
+        return ANTS_ERR_CUDA;
+    }
+    RefineParams rp{};
+    rp.m = m;
+    rp.signals = signals;
+    rp.n_events = n_events;
+    rp.xyzA = xyzA;
+    rp.score = score;
+    rp.dim = dim;
+    rp.seed_mode = seed_mode;
+    rp.n_steps = n_steps;
+    const long long want = (n_events + warps - 1) / warps;
+    const int grid = (int)std::min<long long>(want, (long long)lrf->sm_count * occ);
+    void *args[] = {&rp};
+    if (cudaLaunchKernel(kernel, dim3(grid), dim3(warps * 32), args, smem, (cudaStream_t)cuda_stream) != cudaSuccess) {
+        cudaGetLastError();
+        return ANTS_ERR_CUDA;
+    }
+    g_launches.fetch_add(1);
+    return ANTS_OK;
 }
 
 // ---------------------------------------------------------------------------

@@ -13,4 +13,7 @@ const void *kernel_gen(int method, int lrf_kind);
 // axial+z LRFs (recon3d.cuh).  method 0/1, (cpl, gzm) in {(1,1),(2,1),(3,1),(4,1),(8,1),(1,4),(2,4),(1,8),(2,8)}
 const void *kernel_3d(int method, int cpl, int gzm);
 
+// continuous refinement (refine.cuh), method 0/1/2
+const void *kernel_refine(int method);
+
 }  // namespace ants

@@ -75,6 +75,8 @@ def load():
     lib.ants_plan_kernel_name.argtypes = [vp, C.POINTER(GridParams), C.c_int32, C.c_char_p, C.c_int32]
     lib.ants_probe_throughput.restype = C.c_int
     lib.ants_probe_throughput.argtypes = [C.c_int32, C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+    lib.ants_refine.restype = C.c_int
+    lib.ants_refine.argtypes = [vp, vp, C.c_int64, C.c_int32, C.c_int32, C.c_int32, C.c_int32, vp, vp, vp]
     lib.ants_reconstruct.restype = C.c_int
     lib.ants_reconstruct.argtypes = [vp, vp, C.c_int64, C.POINTER(GridParams), C.c_int32, vp, vp, vp]
     lib.ants_reconstruct_trace.restype = C.c_int
@@ -338,6 +340,27 @@ def ants_reconstruct(handle, signals, grid: GridParams, method: int, out_xyzA, o
                                            out_xyzA.data_ptr(), out_score.data_ptr(), out_path.data_ptr(), st)
     if rc != 0:
         raise AntsError(rc, "ants_reconstruct")
+
+
+def ants_refine(handle, signals, method: int, xyzA, score, n_steps: int, dim: int = 2, seed_mode: int = 0,
+                stream=None) -> None:
+    """Continuous refinement in place (include/ants_recon.h): xyzA [E][4] holds the start positions on entry and the
+    refined positions and energies on return; score [E] receives the scores.  Contiguous float32 CUDA tensors."""
+    import torch
+    N = int(load().ants_lrf_n_sensors(handle))
+    if signals.dim() != 2 or int(signals.shape[1]) != N:
+        raise ValueError(f"ants_refine: signals must be [E][{N}]")
+    E = int(signals.shape[0])
+    for t in (signals, xyzA, score):
+        if not (t.is_cuda and t.is_contiguous() and t.dtype == torch.float32):
+            raise ValueError("ants_refine needs contiguous float32 CUDA tensors")
+    if tuple(xyzA.shape) != (E, 4) or tuple(score.shape) != (E,):
+        raise ValueError("ants_refine: xyzA must be [E][4] and score [E]")
+    st = torch.cuda.current_stream().cuda_stream if stream is None else int(stream)
+    rc = load().ants_refine(handle, signals.data_ptr(), E, int(method), int(dim), int(seed_mode), int(n_steps),
+                            xyzA.data_ptr(), score.data_ptr(), st)
+    if rc != 0:
+        raise AntsError(rc, "ants_refine")
 
 
 def _host_f32(a, shape, what):

@@ -689,20 +689,21 @@ static int validate_grid(const ants_lrf *h, const ants_grid_params_t *g, int32_t
     return ANTS_OK;
 }
 
-// first iteration k whose grid is small enough for the differential score:
-// every node within one knot interval of the centre (at most one knot crossed per
-// axis) and, for Poisson, |dL/L0| <= exp(max|dlnL/dr| reach) - 1 <= kQSeries.
-static int first_diff_iter(const ants_lrf *h, const ants_grid_params_t *g, int32_t method) {
-    if (!h->positive) return g->n_iter;
+// first iteration k whose grid is small enough for the differential score: every node within one knot interval
+// of the centre (at most one knot crossed per axis); k_series (Poisson): the first of those on which
+// |dL/L0| <= exp(max|dlnL/dr| reach) - 1 <= kQSeries, where log1p runs as a series (lg2(1 + q) before)
+static void first_diff_iter(const ants_lrf *h, const ants_grid_params_t *g, int32_t method, int &k_diff, int &k_series) {
+    k_diff = k_series = g->n_iter;
+    if (!h->positive) return;
     const double half = 0.5 * (g->nodes_per_axis - 1);
     double hxy = g->step0_xy;
     for (int k = 0; k < g->n_iter; ++k, hxy *= (double)g->factor) {
         const double reach = std::sqrt(2.0) * half * hxy * 1.001;
-        bool ok = reach <= 0.9 * h->knot_r;
-        if (method == ANTS_POISSON_ML) ok = ok && std::expm1(h->max_dlog * reach) <= kQSeries;
-        if (ok) return k;
+        if (!(reach <= 0.9 * h->knot_r)) continue;
+        // (tried in round 2: differential grids before the series is valid, with lg2(1 + q): most sensors then sit
+        // on the general list with four MUFU per pair, slower than the plain form -- so both switch together)
+        if (method != ANTS_POISSON_ML || std::expm1(h->max_dlog * reach) <= kQSeries) { k_diff = k_series = k; break; }
     }
-    return g->n_iter;
 }
 
 // CTA shape: the warps-per-CTA in {8, 4, 2, 1} that lets the most warps share an SM's shared memory
@@ -814,9 +815,8 @@ static int make_plan(const ants_lrf *h, const ants_grid_params_t *g, int32_t met
     pl.family = 0;
     pl.kernel = kernel_2d_pk(method, pl.npt);
     if (!pl.kernel) return ANTS_ERR_UNSUPPORTED;
-    pl.k_diff = first_diff_iter(h, g, method);
-    pl.k_series = pl.k_diff;
-    const size_t tables = (cta_table_bytes(m.N, m.n_lrf * (m.n_r + 1)) + 15) / 16 * 16;
+    first_diff_iter(h, g, method, pl.k_diff, pl.k_series);
+    const size_t tables = (cta_smem_bytes_pk(m.N, m.n_lrf * (m.n_r + 1)) + 15) / 16 * 16;
     const size_t per_warp = warp_smem_bytes_pk(m.N, method);
     pick_cta_shape(tables, per_warp, pl);
     if (pl.smem > 227 * 1024) return ANTS_ERR_UNSUPPORTED;

@@ -29,8 +29,9 @@ __host__ __device__ inline size_t warp_smem_bytes_pk(int N, int method) {
     const int narr = method == 0 ? 8 : kPkArrays;
     return ((size_t)pk_pairs(N) * 16 * narr + (size_t)N * 8 + 15) / 16 * 16;
 }
-// CTA-shared: sens_s [N] float4, poly_s [rows] float4, grp_s [N] int
-__host__ __device__ inline size_t cta_smem_bytes_pk(int N, int rows) { return cta_table_bytes(N, rows); }
+// CTA-shared: sens_s [N] float4, poly_s [rows] float4, grp_s [N] int, node_s [256] float2 (grid offsets of the
+// nodes in units of the step: a table look-up instead of an integer division wherever a lane needs its nodes)
+__host__ __device__ inline size_t cta_smem_bytes_pk(int N, int rows) { return cta_table_bytes(N, rows) + 256 * 8; }
 
 __device__ __forceinline__ WarpSmemPk carve_pk(unsigned char *base, int N, int method) {
     WarpSmemPk w;

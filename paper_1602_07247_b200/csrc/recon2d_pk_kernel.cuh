@@ -18,6 +18,14 @@ __global__ void __launch_bounds__(256, (NPT <= 3 ? 3 : 2)) recon2d_pk_kernel(con
     int *grp_s = reinterpret_cast<int *>(poly_s + rows);
     for (int i = threadIdx.x; i < N; i += blockDim.x) { sens_s[i] = m.sens[i]; grp_s[i] = m.grp[i]; }
     for (int i = threadIdx.x; i < rows; i += blockDim.x) poly_s[i] = m.poly[i];
+    float2 *node_s = reinterpret_cast<float2 *>(smem + cta_table_bytes(N, rows));
+    {
+        const float halfg = 0.5f * (float)(p.G - 1);
+        for (int n = threadIdx.x; n < 256; n += blockDim.x) {
+            const int iy = n / p.G, ix = n - iy * p.G;
+            node_s[n] = n < p.nodes ? make_float2((float)ix - halfg, (float)iy - halfg) : make_float2(0.f, 0.f);
+        }
+    }
     __syncthreads();
     WarpSmemPk w = carve_pk(smem + (cta_smem_bytes_pk(N, rows) + 15) / 16 * 16 +
                             (size_t)warp * warp_smem_bytes_pk(N, METHOD), N, METHOD);
@@ -26,16 +34,6 @@ __global__ void __launch_bounds__(256, (NPT <= 3 ? 3 : 2)) recon2d_pk_kernel(con
 
     // this lane's nodes: offsets from the grid centre in units of the step
     const float half = 0.5f * (float)(p.G - 1);
-    float fx[NPT], fy[NPT];
-    bool nv[NPT];
-#pragma unroll
-    for (int j = 0; j < NPT; ++j) {
-        int n = lane + 32 * j;
-        nv[j] = n < p.nodes;
-        int iy = n / p.G, ix = n - iy * p.G;
-        fx[j] = nv[j] ? (float)ix - half : 0.f;
-        fy[j] = nv[j] ? (float)iy - half : 0.f;
-    }
     const float half_diag_units = 1.41421356f * half;
     const f32x2 sc2 = pk1(m.sc), of2 = pk1(m.of), magic2 = pk1(kMagic), nmagic2 = pk1(-kMagic);
 
@@ -168,13 +166,9 @@ __global__ void __launch_bounds__(256, (NPT <= 3 ? 3 : 2)) recon2d_pk_kernel(con
                     float v = __shfl_sync(kFull, mine, bi & 31);
                     A_ref = METHOD == 0 ? sumS * rcp_approx(v) : v;
                 }
-                // the winner's grid offsets live in its owner lane (no integer division here)
-                float wx = 0.f, wy = 0.f;
-#pragma unroll
-                for (int j = 0; j < NPT; ++j)
-                    if ((bi >> 5) == j) { wx = fx[j]; wy = fy[j]; }
-                cx = fmaf(__shfl_sync(kFull, wx, bi & 31), h, cx);
-                cy = fmaf(__shfl_sync(kFull, wy, bi & 31), h, cy);
+                const float2 wo = node_s[bi];           // the winner's grid offsets (one broadcast load)
+                cx = fmaf(wo.x, h, cx);
+                cy = fmaf(wo.y, h, cy);
             }
             if (p.out_path && lane == 0) p.out_path[e * p.K + k] = found ? (uint16_t)bi : (uint16_t)0xFFFF;
             h *= p.factor;

@@ -174,7 +174,7 @@ __device__ __forceinline__ bool lm_step(const double Hs[6], const double g[3], d
 }
 
 template <int METHOD>
-__global__ void __launch_bounds__(256) refine_kernel(const RefineParams rp) {
+__global__ void __launch_bounds__(256, 2) refine_kernel(const RefineParams rp) {
     extern __shared__ __align__(16) unsigned char smem[];
     const ModelDev &m = rp.m;
     const int N = m.N;

@@ -17,6 +17,7 @@
 #include "recon2d.cuh"
 #include "recon2d_pk.cuh"
 #include "recon3d.cuh"
+#include "recon3d_pk.cuh"
 #include "recon_gen.cuh"
 #include "refine.cuh"
 #include "kernels.h"
@@ -34,7 +35,7 @@ static const unsigned kCtrSlots = 1024;
 struct Plan {
     int npt = 0;             // nodes per lane (template instantiation)
     int cpl = 0, gzm = 0;    // axial+z kernel: columns per lane, compiled z-levels
-    int family = 0;          // 0 recon2d_pk_kernel, 2 recon3d_kernel, 3 recon_gen_kernel (general)
+    int family = 0;          // 0 recon2d_pk_kernel, 2 recon3d_kernel, 3 recon_gen_kernel (general), 4 recon3d_pk_kernel
     int warps = 0;           // warps per CTA
     int ctas_per_sm = 0;     // resident CTAs per SM (cudaOccupancyMaxActiveBlocksPerMultiprocessor, capped by the tuning knob)
     size_t smem = 0;         // dynamic shared memory per CTA
@@ -650,6 +651,10 @@ const void *kernel_2d_pk_m0(int), *kernel_2d_pk_m1(int), *kernel_2d_pk_m2(int);
 const void *kernel_gen_m0(int), *kernel_gen_m1(int), *kernel_gen_m2(int);
 const void *kernel_3d_m0(int, int), *kernel_3d_m1(int, int);
 const void *kernel_refine(int);
+const void *kernel_3d_pk_m0(int, int), *kernel_3d_pk_m1(int, int);
+const void *kernel_3d_pk(int method, int cpl, int gzp) {
+    return method == 0 ? kernel_3d_pk_m0(cpl, gzp) : method == 1 ? kernel_3d_pk_m1(cpl, gzp) : nullptr;
+}
 const void *kernel_2d_pk(int method, int npt) {
     return method == 0 ? kernel_2d_pk_m0(npt) : method == 1 ? kernel_2d_pk_m1(npt) : method == 2 ? kernel_2d_pk_m2(npt) : nullptr;
 }
@@ -740,11 +745,15 @@ static int make_plan3d(const ants_lrf *h, const ants_grid_params_t *g, int32_t m
         for (int c : kNpt2D)
             if (c >= need) { cpl = c; break; }
     }
-    pl.family = 2;
+    // a 3-D search runs the kernel packed over pairs of z-levels; a 2-D search at fixed z the scalar one
+    const bool packed = g->dim == 3;
+    const int LP = (Gz + 1) / 2;
+    if (packed) gzm = G <= 4 ? 2 : 4;                     // compiled maximum of level pairs
+    pl.family = packed ? 4 : 2;
     pl.cpl = cpl;
     pl.gzm = gzm;
     pl.npt = cpl * Gz;
-    pl.kernel = kernel_3d(method, cpl, gzm);
+    pl.kernel = packed ? kernel_3d_pk(method, cpl, gzm) : kernel_3d(method, cpl, gzm);
     if (!pl.kernel) return ANTS_ERR_UNSUPPORTED;
     // differential from the first grid that stays within one knot interval of the centre (r and z);
     // Poisson log1p by series once |dL/L0| <= kQSeries on the whole grid
@@ -761,7 +770,7 @@ static int make_plan3d(const ants_lrf *h, const ants_grid_params_t *g, int32_t m
         if (pl.k_series < pl.k_diff) pl.k_series = pl.k_diff;
     }
     const size_t tables = (size_t)(m.N + (m.n_z + 3) * (m.n_r + 1)) * 16;
-    const size_t per_warp = warp_smem_bytes_3d(m.N, Gz, m.n_r + 1);
+    const size_t per_warp = packed ? warp_smem_bytes_3dpk(m.N, LP, m.n_r + 1, method) : warp_smem_bytes_3d(m.N, Gz, m.n_r + 1);
     pick_cta_shape(tables, per_warp, pl);
     if (pl.smem > 227 * 1024) return ANTS_ERR_UNSUPPORTED;
     return ANTS_OK;
@@ -869,6 +878,7 @@ static int get_plan(const ants_lrf *hc, const ants_grid_params_t *g, int32_t met
 static void kernel_name(const Plan &pl, int32_t method, int lrf_kind, char *buf, size_t n) {
     if (pl.family == 0) std::snprintf(buf, n, "ants::recon2d_pk_kernel<%d,%d>", pl.npt, (int)method);
     else if (pl.family == 3) std::snprintf(buf, n, "ants::recon_gen_kernel<%d,%d>", (int)method, lrf_kind);
+    else if (pl.family == 4) std::snprintf(buf, n, "ants::recon3d_pk_kernel<%d,%d,%d>", pl.cpl, pl.gzm, (int)method);
     else std::snprintf(buf, n, "ants::recon3d_kernel<%d,%d,%d>", pl.cpl, pl.gzm, (int)method);
 }
 

@@ -1,0 +1,12 @@
+// k3d_pk_m1.cu -- instantiations of recon3d_pk_kernel<CPL, GZP, 1> (axial+z LRFs, 3-D search, level pairs packed)
+#include "recon3d_pk.cuh"
+#include "kernels.h"
+
+namespace ants {
+const void *kernel_3d_pk_m1(int cpl, int gzp) {
+#define ANTS_K3(C, Z) if (cpl == C && gzp == Z) return (const void *)recon3d_pk_kernel<C, Z, 1>
+    ANTS_K3(1, 2); ANTS_K3(2, 2); ANTS_K3(1, 4); ANTS_K3(2, 4);
+#undef ANTS_K3
+    return nullptr;
+}
+}  // namespace ants

@@ -21,7 +21,7 @@
  *
  * Every step runs in hand-written sm_100a CUDA kernels; there is no CPU
  * fallback.  All functions return an ants_status code (0 = OK) and never throw.
- * Points on which the paper is silent follow DESIGN.md "Readings" (R1..R18).
+ * Points on which the paper is silent follow DESIGN.md "Readings" (R1..R34).
  */
 #ifndef ANTS_RECON_H
 #define ANTS_RECON_H

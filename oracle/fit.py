@@ -244,3 +244,59 @@ def group_by_symmetry(sensor_xy, n_fold, reflect=True, tol=1e-3):
                     break
         n_groups += 1
     return group, xform, n_groups
+
+
+def fit_xy(sensor_xy, gains, knots_xy, n_lrf, n_int_x, n_int_y, signals, xyzA, group=None, xform=None,
+           axial=None):
+    """LRF calculation for XY tables ("XY LRF"; PAPER.md:380 LRFs are calculated from signals and
+    positions) and for the XY component of a Composite LRF ("During LRF calculation, the axial
+    component is evaluated first, and the residual is used to calculate the XY LRF component").  Reading R35 =
+    R21-R23 carried to the sensor-local coordinates (u, v) = T_i (p - P_i) of R30/R33: unweighted least squares of
+        y = S / (A g_i)                              (XY LRF)
+        y = S / (A g_i) - s_ax,t(|p - P_i|)          (Composite: axial = (knots, n_int_r, coeffs [n_lrf][n_int_r+3]),
+                                                      the axial spline with its argument clamped as in R5)
+    against sum_b sum_a c[kv+b][ku+a] bv_b bu_a, over events with finite x, y, A and A > 0 and pairs with
+    u_lo <= u <= u_hi and v_lo <= v <= v_hi; table t = group[i], or 0 / i without a grouping; g_i = 1 for per-sensor
+    tables.  -> coefficients [n_lrf][n_int_y + 3][n_int_x + 3] (float64), pairs used [n_lrf].
+    Raises numpy.linalg.LinAlgError when a table is underdetermined (a cell without data)."""
+    xy = np.asarray(sensor_xy, np.float32).astype(np.float64).reshape(-1, 2)
+    N = xy.shape[0]
+    g = np.ones(N) if gains is None else np.asarray(gains, np.float32).astype(np.float64)
+    u_lo, u_hi, v_lo, v_hi = (float(np.float32(k)) for k in knots_xy[:4])
+    hu, hv = (u_hi - u_lo) / n_int_x, (v_hi - v_lo) / n_int_y
+    ncu, ncv = n_int_x + 3, n_int_y + 3
+    S = np.asarray(signals, np.float32).astype(np.float64).reshape(-1, N)
+    P = np.asarray(xyzA, np.float32).astype(np.float64).reshape(-1, 4)
+    T = None if xform is None else np.asarray(xform, np.float32).astype(np.float64).reshape(N, 4)
+    ok = np.isfinite(P[:, 0]) & np.isfinite(P[:, 1]) & np.isfinite(P[:, 3]) & (P[:, 3] > 0.0)
+    M = np.zeros((n_lrf, ncv * ncu, ncv * ncu))
+    b = np.zeros((n_lrf, ncv * ncu))
+    used = np.zeros(n_lrf)
+    for i in range(N):
+        if group is not None:
+            m, gi = int(group[i]), g[i]
+        else:
+            m = 0 if n_lrf == 1 else i
+            gi = g[i] if n_lrf == 1 else 1.0
+        with np.errstate(invalid="ignore"):
+            dx, dy = P[:, 0] - xy[i, 0], P[:, 1] - xy[i, 1]
+            u, v = (dx, dy) if T is None else (T[i, 0] * dx + T[i, 1] * dy, T[i, 2] * dx + T[i, 3] * dy)
+            use = ok & (u >= u_lo) & (u <= u_hi) & (v >= v_lo) & (v <= v_hi)
+        y = S[use, i] / (P[use, 3] * gi)
+        if axial is not None:
+            a_knots, a_n, a_c = axial
+            a_lo, a_hi = float(np.float32(a_knots[0])), float(np.float32(a_knots[1]))
+            r = np.clip(np.hypot(dx[use], dy[use]), a_lo, a_hi)
+            y = y - spline_values(np.asarray(a_c)[m], a_lo, a_hi, a_n, r)
+        tu, tv = (u[use] - u_lo) / hu, (v[use] - v_lo) / hv
+        ku = np.minimum(np.floor(tu).astype(np.int64), n_int_x - 1)
+        kv = np.minimum(np.floor(tv).astype(np.int64), n_int_y - 1)
+        Bu, Bv = basis4(tu - ku), basis4(tv - kv)
+        idx = [((kv + bb) * ncu + ku + aa, Bv[:, bb] * Bu[:, aa]) for bb in range(4) for aa in range(4)]
+        for j1, w1 in idx:
+            np.add.at(b[m], j1, w1 * y)
+            for j2, w2 in idx:
+                np.add.at(M[m], (j1, j2), w1 * w2)
+        used[m] += use.sum()
+    c = np.stack([np.linalg.solve(M[m], b[m]).reshape(ncv, ncu) for m in range(n_lrf)])
+    return c, used

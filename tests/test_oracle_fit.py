@@ -267,3 +267,61 @@ def test_gain_renormalisation_keeps_the_mean_and_the_ratios():
     assert abs(out[4] / prev[4] - ratio.mean()) <= 2e-7 * ratio.mean() and abs(out[9] / prev[9] - ratio.mean()) <= 2e-7 * ratio.mean()
     same = fit.renormalise_gains(prev, prev)
     assert np.abs(same.astype(np.float64) - prev).max() <= 1.2e-7 * prev.max()
+
+
+def _xy_problem(n_events, seed=0, composite=False):
+    """A small XY-type detector whose tables are fully covered by the events: 3 x 3 sensors (pitch 8 mm), XY range
+    +-12 mm around each sensor, events over a +-22 mm square, known smooth response, Gaussian noise."""
+    rng = np.random.default_rng(seed)
+    xy = synth.square_array(3, 8.0)
+    N = len(xy)
+    gains = rng.uniform(0.8, 1.2, N).astype(np.float32)
+    pos = np.zeros((n_events, 4), np.float32)
+    pos[:, :2] = rng.uniform(-22.0, 22.0, (n_events, 2))
+    pos[:, 3] = rng.uniform(200.0, 400.0, n_events)
+    dx = pos[:, None, 0].astype(np.float64) - xy[None, :, 0]
+    dy = pos[:, None, 1].astype(np.float64) - xy[None, :, 1]
+    resp = np.exp(-(dx * dx / 60.0 + dy * dy / 90.0)) * (1.0 + 0.02 * dx)
+    if composite:
+        resp = resp + 0.5 / (1.0 + (dx * dx + dy * dy) / 40.0)
+    sig = (pos[:, 3:4].astype(np.float64) * gains[None, :] * resp + rng.normal(0, 0.5, (n_events, N))).astype(np.float32)
+    return xy, gains, sig, pos
+
+
+def test_xy_fit_is_the_lstsq_of_the_tensor_design_matrix():
+    """R35 pinned against scipy design matrices + numpy.linalg.lstsq, per table: shared table with gains, symmetry
+    groups with frames, and the Composite residual fit."""
+    from scipy.interpolate import BSpline
+    xy, gains, sig, pos = _xy_problem(1500)
+    knots = np.array([-12, 12, -12, 12], np.float32)
+    nx, ny = 4, 5
+    tu, tv = synth.uniform_knot_vector(-12.0, 12.0, nx), synth.uniform_knot_vector(-12.0, 12.0, ny)
+    group, xform, n_groups = fit.group_by_symmetry(xy, 4, True)
+    ax_knots, ax_n = np.array([0.0, 34.0], np.float32), 6
+    ax_c = np.tile(synth.fit_axial(lambda r: 0.5 / (1.0 + r * r / 40.0), 0.0, 34.0, ax_n)[None, :], (n_groups, 1))
+    for kw in (dict(n_lrf=1), dict(n_lrf=n_groups, group=group, xform=xform),
+               dict(n_lrf=n_groups, group=group, xform=xform, axial=(ax_knots, ax_n, ax_c))):
+        c, used = fit.fit_xy(xy, gains, knots, kw["n_lrf"], nx, ny, sig, pos, group=kw.get("group"),
+                             xform=kw.get("xform"), axial=kw.get("axial"))
+        assert c.shape == (kw["n_lrf"], ny + 3, nx + 3)
+        for m in range(kw["n_lrf"]):
+            rows, ys = [], []
+            for i in range(len(xy)):
+                if (kw.get("group") is not None and group[i] != m):
+                    continue
+                dx = pos[:, 0].astype(float) - float(xy[i, 0])
+                dy = pos[:, 1].astype(float) - float(xy[i, 1])
+                T = np.eye(2) if kw.get("xform") is None else xform[i].astype(float).reshape(2, 2)
+                u, v = T[0, 0] * dx + T[0, 1] * dy, T[1, 0] * dx + T[1, 1] * dy
+                use = (u >= -12) & (u <= 12) & (v >= -12) & (v <= 12)
+                Bu = BSpline.design_matrix(u[use], tu, 3).toarray()
+                Bv = BSpline.design_matrix(v[use], tv, 3).toarray()
+                rows.append(np.einsum("kb,ka->kba", Bv, Bu).reshape(use.sum(), -1))
+                y = sig[use, i].astype(float) / (pos[use, 3].astype(float) * float(gains[i]))
+                if kw.get("axial") is not None:
+                    r = np.clip(np.hypot(dx[use], dy[use]), 0.0, 34.0)
+                    y = y - synth.eval_axial(ax_c[m], 0.0, 34.0, r)
+                ys.append(y)
+            ref, *_ = np.linalg.lstsq(np.vstack(rows), np.concatenate(ys), rcond=None)
+            assert np.abs(c[m].ravel() - ref).max() <= 1e-7 * max(1.0, np.abs(ref).max()), kw.keys()
+            assert used[m] == sum(len(y) for y in ys)

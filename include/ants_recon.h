@@ -336,6 +336,28 @@ int ants_lrf_fit_axial_z(const float *sensor_xy, const float *gains, const float
                          int32_t n_int_r, int32_t n_int_z, const float *signals, const float *xyzA,
                          int64_t n_events, float *coeffs_out, double *n_used_out, void *cuda_stream);
 
+/*
+ * ants_lrf_fit_xy -- LRF calculation for XY tables ("XY LRF") and for the XY component
+ * of a Composite LRF ("During LRF calculation, the axial component is evaluated first, and the
+ * residual is used to calculate the XY LRF component").  Reading R35 = R21-R23 in the sensor-local coordinates
+ * (u, v) = T_i (p - P_i): unweighted least squares of y = S / (A g_i) -- minus the table's axial spline at
+ * |p - P_i| (argument clamped, R5) when coeffs_ax is given -- against the tensor-product spline; an event takes
+ * part if x, y, A are finite and A > 0, a pair if u and v lie inside the tabulated ranges.
+ *   sensor_xy HOST [N][2]; gains HOST [N] or NULL; group HOST [N] int32 or NULL (n_lrf = 1 or N then); xform HOST
+ *   [N][4] or NULL; knots_xy HOST {u_lo, u_hi, v_lo, v_hi}; knots_ax HOST {r_lo, r_hi} and coeffs_ax HOST
+ *   [n_lrf][n_int_r + 3] for a Composite fit (first fitted with ants_lrf_fit_axial / _grouped), else NULL;
+ *   signals DEVICE [n_events][N]; xyzA DEVICE [n_events][4];
+ *   coeffs_out HOST [n_lrf][n_int_y + 3][n_int_x + 3] float; n_used_out HOST [n_lrf] double or NULL.
+ * One kernel launch (FP64 normal equations) and one dense Cholesky solve on the host per table; returns after the
+ * result is in host memory.  The result goes straight into ants_lrf_create_xy.  Sliced tables are not fitted by
+ * this library.  Errors: ANTS_ERR_INVALID, ANTS_ERR_SINGULAR (a cell of some table received no data),
+ * ANTS_ERR_UNSUPPORTED ((n_int_x + 3)(n_int_y + 3) > 768), ANTS_ERR_CUDA, ANTS_ERR_NOMEM.
+ */
+int ants_lrf_fit_xy(const float *sensor_xy, const float *gains, const int32_t *group, const float *xform,
+                    const float *knots_xy, int32_t n_sensors, int32_t n_lrf, int32_t n_int_x, int32_t n_int_y,
+                    const float *knots_ax, const float *coeffs_ax, int32_t n_int_r, const float *signals,
+                    const float *xyzA, int64_t n_events, float *coeffs_out, double *n_used_out, void *cuda_stream);
+
 /* Event-filter criteria (section 5.2); NaN switches a criterion off. */
 typedef struct {
     float score_max;    /* keep score <= score_max (chi-square / deviance of the reconstruction) */

@@ -1453,3 +1453,120 @@ extern "C" int ants_filter_events(float *xyzA, const float *score, int64_t n_eve
     if (!ok) { cudaGetLastError(); return ANTS_ERR_CUDA; }
     return ANTS_OK;
 }
+
+// ---------------------------------------------------------------------------
+// LRF calculation for XY tables / the XY component of a Composite LRF (R35): one launch and one dense
+// Cholesky solve per table
+// ---------------------------------------------------------------------------
+extern "C" int ants_lrf_fit_xy(const float *sensor_xy, const float *gains, const int32_t *group, const float *xform,
+                               const float *knots_xy, int32_t N, int32_t n_lrf, int32_t nx, int32_t ny,
+                               const float *knots_ax, const float *coeffs_ax, int32_t n_int_r, const float *signals,
+                               const float *xyzA, int64_t n_events, float *coeffs_out, double *n_used_out,
+                               void *cuda_stream) {
+    if (!sensor_xy || !knots_xy || !coeffs_out || N < 1 || nx < 1 || ny < 1 || n_events < 0) return ANTS_ERR_INVALID;
+    if (n_events > 0 && (!signals || !xyzA)) return ANTS_ERR_INVALID;
+    if (group) {
+        if (n_lrf < 1 || n_lrf > N) return ANTS_ERR_INVALID;
+        for (int i = 0; i < N; ++i)
+            if (group[i] < 0 || group[i] >= n_lrf) return ANTS_ERR_INVALID;
+    } else if (n_lrf != 1 && n_lrf != N) {
+        return ANTS_ERR_INVALID;
+    }
+    const double u_lo = knots_xy[0], u_hi = knots_xy[1], v_lo = knots_xy[2], v_hi = knots_xy[3];
+    if (!std::isfinite(u_lo) || !std::isfinite(u_hi) || !std::isfinite(v_lo) || !std::isfinite(v_hi) || !(u_hi > u_lo) ||
+        !(v_hi > v_lo))
+        return ANTS_ERR_INVALID;
+    const bool composite = coeffs_ax != nullptr;
+    double a_lo = 0.0, a_hi = 1.0;
+    if (composite) {
+        if (!knots_ax || n_int_r < 1 || n_int_r > 4096) return ANTS_ERR_INVALID;
+        a_lo = knots_ax[0];
+        a_hi = knots_ax[1];
+        if (!std::isfinite(a_lo) || !std::isfinite(a_hi) || !(a_lo >= 0.0) || !(a_hi > a_lo)) return ANTS_ERR_INVALID;
+    }
+    for (int i = 0; i < N; ++i)
+        if (gains && !(gains[i] > 0.f && std::isfinite(gains[i]))) return ANTS_ERR_INVALID;
+    const int ncu = nx + 3, nc = ncu * (ny + 3);
+    if (nc > 768) return ANTS_ERR_UNSUPPORTED;
+    const size_t total = (size_t)nc * 29, smem = total * sizeof(double);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+        cudaGetLastError();
+        return ANTS_ERR_CUDA;
+    }
+    const bool scaled = group != nullptr || n_lrf == 1;
+    std::vector<float> g(N, 1.f);
+    if (gains && scaled) std::copy(gains, gains + N, g.begin());
+    float *d_xy = nullptr, *d_g = nullptr, *d_xf = nullptr, *d_ax = nullptr;
+    int *d_mem = nullptr;
+    double *d_acc = nullptr;
+    unsigned long long *d_used = nullptr;
+    auto cleanup = [&]() { cudaFree(d_xy); cudaFree(d_g); cudaFree(d_xf); cudaFree(d_ax); cudaFree(d_mem); cudaFree(d_acc); cudaFree(d_used); cudaGetLastError(); };
+    if (cudaMalloc(&d_xy, (size_t)N * 2 * sizeof(float)) != cudaSuccess || cudaMalloc(&d_g, (size_t)N * sizeof(float)) != cudaSuccess ||
+        cudaMalloc(&d_mem, (size_t)N * sizeof(int)) != cudaSuccess || cudaMalloc(&d_acc, smem) != cudaSuccess ||
+        cudaMalloc(&d_used, sizeof(unsigned long long)) != cudaSuccess ||
+        (xform && cudaMalloc(&d_xf, (size_t)N * 4 * sizeof(float)) != cudaSuccess) ||
+        (composite && cudaMalloc(&d_ax, (size_t)(n_int_r + 3) * sizeof(float)) != cudaSuccess)) {
+        cleanup();
+        return ANTS_ERR_NOMEM;
+    }
+    bool ok = cudaMemcpyAsync(d_xy, sensor_xy, (size_t)N * 2 * sizeof(float), cudaMemcpyHostToDevice, st) == cudaSuccess &&
+              cudaMemcpyAsync(d_g, g.data(), (size_t)N * sizeof(float), cudaMemcpyHostToDevice, st) == cudaSuccess &&
+              (!xform || cudaMemcpyAsync(d_xf, xform, (size_t)N * 4 * sizeof(float), cudaMemcpyHostToDevice, st) == cudaSuccess);
+    const int warps = 8;
+    int occ = 0;
+    ok = ok && cudaFuncSetAttribute((const void *)lrf_fit_xy_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) == cudaSuccess &&
+         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void *)lrf_fit_xy_kernel, warps * 32, smem) == cudaSuccess && occ >= 1;
+    int rc = ok ? ANTS_OK : ANTS_ERR_CUDA;
+    std::vector<double> acc(total), M((size_t)nc * nc), b(nc);
+    std::vector<int> members;
+    for (int t = 0; t < n_lrf && rc == ANTS_OK; ++t) {
+        members.clear();
+        for (int i = 0; i < N; ++i)
+            if ((group ? group[i] : (n_lrf == 1 ? 0 : i)) == t) members.push_back(i);
+        unsigned long long used = 0;
+        ok = cudaMemsetAsync(d_acc, 0, smem, st) == cudaSuccess && cudaMemsetAsync(d_used, 0, sizeof(unsigned long long), st) == cudaSuccess &&
+             (members.empty() || cudaMemcpyAsync(d_mem, members.data(), members.size() * sizeof(int), cudaMemcpyHostToDevice, st) == cudaSuccess) &&
+             (!composite || cudaMemcpyAsync(d_ax, coeffs_ax + (size_t)t * (n_int_r + 3), (size_t)(n_int_r + 3) * sizeof(float),
+                                            cudaMemcpyHostToDevice, st) == cudaSuccess);
+        if (ok && n_events > 0 && !members.empty()) {
+            FitXYParams p{};
+            p.sens_xy = d_xy; p.gains = d_g; p.xform = xform ? d_xf : nullptr; p.members = d_mem; p.n_members = (int)members.size();
+            p.signals = signals; p.xyzA = xyzA; p.n_events = n_events; p.N = N; p.nx = nx; p.ny = ny; p.ncu = ncu; p.nc = nc;
+            p.u_lo = u_lo; p.u_hi = u_hi; p.hu = (u_hi - u_lo) / nx; p.v_lo = v_lo; p.v_hi = v_hi; p.hv = (v_hi - v_lo) / ny;
+            p.axial = composite ? d_ax : nullptr; p.a_n = n_int_r; p.a_lo = a_lo; p.a_hi = a_hi;
+            p.acc = d_acc; p.n_used = d_used;
+            const long long want = (n_events + warps - 1) / warps;
+            const int grid = (int)std::min<long long>(want, (long long)sms * occ);
+            void *args[] = {&p};
+            ok = cudaLaunchKernel((const void *)lrf_fit_xy_kernel, dim3(grid), dim3(warps * 32), args, smem, st) == cudaSuccess;
+            if (ok) g_launches.fetch_add(1);
+        }
+        // (the host buffers of this table are read by the stream: wait before they are reused for the next one)
+        ok = ok && cudaMemcpyAsync(acc.data(), d_acc, smem, cudaMemcpyDeviceToHost, st) == cudaSuccess &&
+             cudaMemcpyAsync(&used, d_used, sizeof(used), cudaMemcpyDeviceToHost, st) == cudaSuccess &&
+             cudaStreamSynchronize(st) == cudaSuccess;
+        if (!ok) { rc = ANTS_ERR_CUDA; break; }
+        if (n_used_out) n_used_out[t] = (double)used;
+        std::fill(M.begin(), M.end(), 0.0);
+        for (int j1 = 0; j1 < nc; ++j1) {
+            const int ju1 = j1 % ncu;
+            b[j1] = acc[(size_t)j1 * 29 + 28];
+            for (int dv = 0; dv < 4; ++dv)
+                for (int du = -3; du <= 3; ++du) {
+                    const int ju2 = ju1 + du, j2 = j1 + dv * ncu + du;
+                    if (ju2 < 0 || ju2 >= ncu || j2 >= nc || j2 < j1) continue;
+                    const double v = acc[(size_t)j1 * 29 + dv * 7 + du + 3];
+                    M[(size_t)j1 * nc + j2] = v;
+                    M[(size_t)j2 * nc + j1] = v;
+                }
+        }
+        if (!solve_dense_spd(M, b, nc)) { rc = ANTS_ERR_SINGULAR; break; }
+        for (int j = 0; j < nc; ++j) coeffs_out[(size_t)t * nc + j] = (float)b[j];
+    }
+    if (rc != ANTS_OK) cudaStreamSynchronize(st);
+    cleanup();
+    return rc;
+}

@@ -256,3 +256,91 @@ __global__ void __launch_bounds__(256) event_filter_kernel(const FilterParams p)
 }
 
 }  // namespace ants
+
+namespace ants {
+
+// ---- XY tables (R35) and the XY component of a Composite LRF: normal equations of
+// ONE table's tensor-product spline in the sensor-local coordinates (u, v) = T_i (p - P_i), accumulated exactly as
+// lrf_fit_rz_kernel does (per row the 4 x 7 block of the upper triangle + the right-hand side, 29 doubles).  Lanes
+// run over the table's member sensors; a Composite fit subtracts the table's axial spline from y first.
+struct FitXYParams {
+    const float *sens_xy, *gains, *xform;     // device [N][2], [N] (1 for per-sensor tables), [N][4] or nullptr
+    const int *members;                        // device [n_members] sensors of this table
+    int n_members;
+    const float *signals, *xyzA;
+    long long n_events;
+    int N, nx, ny, ncu, nc;
+    double u_lo, u_hi, hu, v_lo, v_hi, hv;
+    const float *axial;                        // device [a_n + 3] axial coefficients of this table, or nullptr
+    int a_n;
+    double a_lo, a_hi;
+    double *acc;                               // device [nc][29]
+    unsigned long long *n_used;                // device [1]
+};
+
+__global__ void __launch_bounds__(256) lrf_fit_xy_kernel(const FitXYParams p) {
+    extern __shared__ double xy_smem[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, warps = blockDim.x >> 5;
+    const int total = p.nc * 29;
+    for (int i = threadIdx.x; i < total; i += blockDim.x) xy_smem[i] = 0.0;
+    __syncthreads();
+    unsigned long long used = 0ULL;
+    for (long long e = (long long)blockIdx.x * warps + warp; e < p.n_events; e += (long long)gridDim.x * warps) {
+        const float4 pe = reinterpret_cast<const float4 *>(p.xyzA)[e];
+        const double x = (double)pe.x, y = (double)pe.y, A = (double)pe.w;
+        if (!(fabs(x) <= 1.7e308 && fabs(y) <= 1.7e308 && A > 0.0 && A <= 1.7e308)) continue;       // R22
+        const float *sig = p.signals + e * p.N;
+        for (int q = lane; q < p.n_members; q += 32) {
+            const int i = p.members[q];
+            const double dx = x - (double)p.sens_xy[2 * i], dy = y - (double)p.sens_xy[2 * i + 1];
+            double u = dx, v = dy;
+            if (p.xform) {
+                const float4 T = reinterpret_cast<const float4 *>(p.xform)[i];
+                u = (double)T.x * dx + (double)T.y * dy;
+                v = (double)T.z * dx + (double)T.w * dy;
+            }
+            if (!(u >= p.u_lo && u <= p.u_hi && v >= p.v_lo && v <= p.v_hi)) continue;              // R35
+            double yv = (double)__ldg(sig + i) / (A * (double)p.gains[i]);
+            if (p.axial) {
+                const double r = fmin(fmax(sqrt(dx * dx + dy * dy), p.a_lo), p.a_hi);
+                const double t = (r - p.a_lo) / ((p.a_hi - p.a_lo) / p.a_n);
+                const int k = min((int)floor(t), p.a_n - 1);
+                const double f = t - (double)k, o = 1.0 - f, f2 = f * f, f3 = f2 * f;
+                yv -= (double)p.axial[k] * (o * o * o / 6.0) + (double)p.axial[k + 1] * ((3.0 * f3 - 6.0 * f2 + 4.0) / 6.0) +
+                      (double)p.axial[k + 2] * ((-3.0 * f3 + 3.0 * f2 + 3.0 * f + 1.0) / 6.0) + (double)p.axial[k + 3] * (f3 / 6.0);
+            }
+            const double tu = (u - p.u_lo) / p.hu, tv = (v - p.v_lo) / p.hv;
+            const int ku = min((int)floor(tu), p.nx - 1), kv = min((int)floor(tv), p.ny - 1);
+            const double fu = tu - (double)ku, ou = 1.0 - fu, fu2 = fu * fu, fu3 = fu2 * fu;
+            const double fv = tv - (double)kv, ov = 1.0 - fv, fv2 = fv * fv, fv3 = fv2 * fv;
+            const double bu[4] = {ou * ou * ou / 6.0, (3.0 * fu3 - 6.0 * fu2 + 4.0) / 6.0,
+                                  (-3.0 * fu3 + 3.0 * fu2 + 3.0 * fu + 1.0) / 6.0, fu3 / 6.0};
+            const double bv[4] = {ov * ov * ov / 6.0, (3.0 * fv3 - 6.0 * fv2 + 4.0) / 6.0,
+                                  (-3.0 * fv3 + 3.0 * fv2 + 3.0 * fv + 1.0) / 6.0, fv3 / 6.0};
+#pragma unroll
+            for (int b1 = 0; b1 < 4; ++b1)
+#pragma unroll
+                for (int a1 = 0; a1 < 4; ++a1) {
+                    const double w1 = bv[b1] * bu[a1];
+                    double *row = xy_smem + (size_t)((kv + b1) * p.ncu + ku + a1) * 29;
+                    atomicAdd(row + 28, w1 * yv);
+#pragma unroll
+                    for (int b2 = b1; b2 < 4; ++b2)
+#pragma unroll
+                        for (int a2 = 0; a2 < 4; ++a2) {
+                            if (b2 == b1 && a2 < a1) continue;
+                            atomicAdd(row + (b2 - b1) * 7 + (a2 - a1) + 3, w1 * bv[b2] * bu[a2]);
+                        }
+                }
+            ++used;
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) used += __shfl_xor_sync(0xffffffffu, used, o);
+    if (lane == 0 && used) atomicAdd(p.n_used, used);
+    __syncthreads();
+    for (int i = threadIdx.x; i < total; i += blockDim.x)
+        if (xy_smem[i] != 0.0) atomicAdd(p.acc + i, xy_smem[i]);
+}
+
+}  // namespace ants

@@ -14,8 +14,8 @@ from . import recon
 def iterate_response(cfg, signals, n_cycles: int, score_max: float = float("nan"),
                      energy_min: float = float("nan"), energy_max: float = float("nan"),
                      radius_max: float = float("nan"), refit_gains: bool = False):
-    """cfg: a synth.Config-like record with the starting LRFs (axial, shared or per-sensor tables, or
-    axial+z); signals: CUDA float32 [E][N].  Yields (cycle, cfg_k, n_events_used) after every cycle, cfg_k
+    """cfg: a synth.Config-like record with the starting LRFs (axial, shared or per-sensor tables, axial+z,
+    XY or Composite); signals: CUDA float32 [E][N].  Yields (cycle, cfg_k, n_events_used) after every cycle, cfg_k
     carrying the refitted coefficients (and gains when refit_gains, shared axial profile only)."""
     cur = copy.copy(cfg)
     for cycle in range(n_cycles):
@@ -26,7 +26,18 @@ def iterate_response(cfg, signals, n_cycles: int, score_max: float = float("nan"
             r.close()
         n_pass = recon.ants_filter_events(xyzA, score, score_max, energy_min, energy_max, radius_max)
         nxt = copy.copy(cur)
-        if cur.lrf_dim == 2:
+        if cur.lrf_dim in (3, 4):
+            # XY tables; for a Composite LRF the axial component first, then the XY component on the residual
+            axial = None
+            if cur.lrf_dim == 4:
+                ca, _ = recon.ants_lrf_fit_axial(cur.sensor_xy, cur.gains, cur.knots, cur.n_lrf, cur.n_int_r, signals, xyzA,
+                                                 group=getattr(cur, "group", None))
+                nxt.coeffs = ca[:, None, :].astype(np.float32)
+                axial = (cur.knots, ca)
+            c, _ = recon.ants_lrf_fit_xy(cur.sensor_xy, cur.gains, cur.knots_xy, cur.n_lrf, cur.n_int_x, cur.n_int_y, signals,
+                                         xyzA, group=getattr(cur, "group", None), xform=getattr(cur, "xform", None), axial=axial)
+            nxt.coeffs_xy = c[:, None, :, :].astype(np.float32)
+        elif cur.lrf_dim == 2:
             c, _ = recon.ants_lrf_fit_axial_z(cur.sensor_xy, cur.gains, cur.knots, cur.n_int_r, cur.n_int_z, signals, xyzA)
             nxt.coeffs = c[None, :, :].astype(np.float32)
         else:

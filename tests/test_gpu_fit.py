@@ -233,3 +233,40 @@ def test_grouped_model_on_random_groups(method, seed):
     finally:
         r.close()
     parity_rules.assert_parity(parity_rules.compare(cfg, ev["signals"].cpu().numpy(), *out), f"random groups m{method}")
+
+
+def test_xy_and_composite_fit_parity():
+    """ants_lrf_fit_xy vs the oracle (R35): one shared XY table with gains, D4 symmetry groups with frames, and the
+    XY component of a Composite LRF fitted to the residual of a given axial component; the fitted tables go straight
+    into ants_lrf_create_xy."""
+    from test_oracle_fit import _xy_problem
+    xy, gains, sig, pos = _xy_problem(40_003, seed=3, composite=True)
+    knots = np.array([-12, 12, -12, 12], np.float32)
+    nx, ny = 6, 5
+    group, xform, n_groups = recon.ants_group_by_symmetry(xy, 4, True)
+    sig_d, pos_d = torch.from_numpy(sig).cuda(), torch.from_numpy(pos).cuda()
+    ax_knots, ax_n = np.array([0.0, 34.0], np.float32), 6
+    ax_c = np.tile(synth.fit_axial(lambda r: 0.5 / (1.0 + r * r / 40.0), 0.0, 34.0, ax_n)[None, :], (n_groups, 1))
+    for kw in (dict(n_lrf=1), dict(n_lrf=n_groups, group=group, xform=xform),
+               dict(n_lrf=n_groups, group=group, xform=xform, axial=(ax_knots, ax_c))):
+        c, used = recon.ants_lrf_fit_xy(xy, gains, knots, kw["n_lrf"], nx, ny, sig_d, pos_d, group=kw.get("group"),
+                                        xform=kw.get("xform"), axial=kw.get("axial"))
+        ax0 = None if "axial" not in kw else (ax_knots, ax_n, ax_c)
+        c0, used0 = ofit.fit_xy(xy, gains, knots, kw["n_lrf"], nx, ny, sig, pos, group=kw.get("group"),
+                                xform=kw.get("xform"), axial=ax0)
+        assert np.array_equal(used, used0), kw.keys()
+        scale = np.abs(c0).max(axis=(1, 2), keepdims=True)
+        assert (np.abs(c - c0) <= 5e-6 * scale).all(), (kw.keys(), np.abs(c - c0).max())
+    # the composite model built from the two fits reconstructs
+    dims = recon.LrfDims(len(xy), n_groups, 4, ax_n, 0)
+    h = recon.ants_lrf_create_xy(xy, gains, ax_knots, ax_c, dims, nx, ny, 0, knots, c, xform=xform, group=group)
+    grid = recon.GridParams(2, 7, 2.0, 0.0, 0.5, 6, 0, float("nan"))
+    out, score = torch.empty((256, 4), device="cuda"), torch.empty(256, device="cuda")
+    recon.ants_reconstruct(h, sig_d[:256].contiguous(), grid, 1, out, score)
+    torch.cuda.synchronize()
+    recon.ants_destroy(h)
+    assert torch.isfinite(out[:, :2]).all() and (out[:, :2].abs().max() <= 40.0)
+    # a cell without data: the table is underdetermined
+    with pytest.raises(recon.AntsError) as ei:
+        recon.ants_lrf_fit_xy(xy, gains, np.array([-60, 60, -60, 60], np.float32), 1, 12, 12, sig_d, pos_d)
+    assert ei.value.status == -5

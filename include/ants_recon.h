@@ -273,7 +273,8 @@ int ants_refine(const ants_lrf_t *lrf, const float *signals, int64_t n_events, i
  *              or true positions with A = the known light output);
  *   coeffs_out HOST [n_lrf][n_int_r + 3] float;  n_used_out HOST [n_lrf] double or NULL: pairs per table.
  * The normal equations are accumulated on the GPU in FP64 (one kernel launch on `cuda_stream`), the banded
- * systems are solved on the host; the call allocates scratch and returns after the result is in host memory.
+ * systems are solved on the host; scratch comes from a device arena the library keeps (fit calls are serialised
+ * by its lock); the call returns after the result is in host memory.
  * Errors: ANTS_ERR_INVALID, ANTS_ERR_SINGULAR (an interval of some table received no data), ANTS_ERR_CUDA,
  * ANTS_ERR_NOMEM, ANTS_ERR_UNSUPPORTED (accumulators larger than shared memory).
  */

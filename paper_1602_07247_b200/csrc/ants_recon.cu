@@ -1114,6 +1114,43 @@ extern "C" int ants_refine(const ants_lrf_t *lrf, const float *signals, int64_t 
 }
 
 // ---------------------------------------------------------------------------
+// scratch of the LRF-calculation calls: one device arena per process, grown on demand and kept, so that a call
+// costs no cudaMalloc / cudaFree (round 1: four or five of each per call).  The calls are serialised by its mutex;
+// each waits for its stream before it returns, so the next one may reuse the memory.
+// ---------------------------------------------------------------------------
+struct FitArena {
+    std::mutex mu;
+    unsigned char *buf = nullptr;
+    size_t cap = 0, used = 0;
+    int device = -1;
+    // reset for a new call that needs `bytes` in total
+    bool begin(size_t bytes) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return false; }
+        bytes += 4096;
+        if (dev != device || bytes > cap) {
+            if (buf) { cudaSetDevice(device); cudaFree(buf); cudaSetDevice(dev); }
+            buf = nullptr;
+            cap = 0;
+            const size_t want = std::max<size_t>(bytes, (size_t)1 << 20);
+            if (cudaMalloc(&buf, want) != cudaSuccess) { cudaGetLastError(); buf = nullptr; return false; }
+            cap = want;
+            device = dev;
+        }
+        used = 0;
+        return true;
+    }
+    template <typename T>
+    T *take(size_t count) {
+        used = (used + 255) / 256 * 256;
+        T *ptr = reinterpret_cast<T *>(buf + used);
+        used += count * sizeof(T);
+        return used <= cap ? ptr : nullptr;
+    }
+};
+static FitArena g_fit_arena;
+
+// ---------------------------------------------------------------------------
 // LRF calculation: normal equations on the GPU (lrf_fit.cuh), banded solve here
 // ---------------------------------------------------------------------------
 #include "lrf_fit.cuh"
@@ -1192,20 +1229,47 @@ static int fit_axial_impl(const float *sensor_xy, const float *gains, const int3
     float *d_xy = nullptr, *d_g = nullptr;
     double *d_acc = nullptr;
     unsigned long long *d_used = nullptr;
-    auto cleanup = [&]() { cudaFree(d_xy); cudaFree(d_g); cudaFree(d_acc); cudaFree(d_used); cudaFree(d_group); cudaGetLastError(); };
-    if (cudaMalloc(&d_xy, (size_t)N * 2 * sizeof(float)) != cudaSuccess || cudaMalloc(&d_g, (size_t)N * sizeof(float)) != cudaSuccess ||
-        (group && cudaMalloc(&d_group, (size_t)N * sizeof(int)) != cudaSuccess) ||
-        cudaMalloc(&d_acc, per_copy * sizeof(double)) != cudaSuccess ||
-        cudaMalloc(&d_used, (size_t)n_lrf * sizeof(unsigned long long)) != cudaSuccess) {
-        cleanup();
-        return ANTS_ERR_NOMEM;
-    }
+    auto cleanup = [&]() { cudaGetLastError(); };
+    std::lock_guard<std::mutex> arena_lock(g_fit_arena.mu);
+    if (!g_fit_arena.begin((size_t)N * 16 + per_copy * sizeof(double) + (size_t)n_lrf * 8 + 2048)) return ANTS_ERR_NOMEM;
+    d_xy = g_fit_arena.take<float>((size_t)N * 2);
+    d_g = g_fit_arena.take<float>(N);
+    if (group) d_group = g_fit_arena.take<int>(N);
+    d_acc = g_fit_arena.take<double>(per_copy);
+    d_used = g_fit_arena.take<unsigned long long>(n_lrf);
+    if (!d_xy || !d_g || !d_acc || !d_used || (group && !d_group)) return ANTS_ERR_NOMEM;
     bool ok = cudaMemcpyAsync(d_xy, sensor_xy, (size_t)N * 2 * sizeof(float), cudaMemcpyHostToDevice, st) == cudaSuccess &&
               cudaMemcpyAsync(d_g, g.data(), (size_t)N * sizeof(float), cudaMemcpyHostToDevice, st) == cudaSuccess &&
               (!group || cudaMemcpyAsync(d_group, group, (size_t)N * sizeof(int), cudaMemcpyHostToDevice, st) == cudaSuccess) &&
               cudaMemsetAsync(d_acc, 0, per_copy * sizeof(double), st) == cudaSuccess &&
               cudaMemsetAsync(d_used, 0, (size_t)n_lrf * sizeof(unsigned long long), st) == cudaSuccess;
-    if (ok && n_events > 0) {
+    // one shared profile whose band fits once per thread: the kernel without atomics in the loop
+    const size_t per_thread = (size_t)nc * 5 * sizeof(double);
+    int priv_threads = 0;
+    if (n_lrf == 1 && !std::getenv("ANTS_FIT_ATOMIC")) {
+        priv_threads = (int)std::min<size_t>(128, (113 * 1024 / per_thread) / 32 * 32);     // two CTAs per SM
+        if (priv_threads < 64) priv_threads = (int)std::min<size_t>(128, (226 * 1024 / per_thread) / 32 * 32);
+        if (priv_threads < 32) priv_threads = 0;
+    }
+    if (ok && n_events > 0 && priv_threads > 0) {
+        FitParams p{};
+        p.sens_xy = d_xy; p.gains = d_g; p.group = nullptr; p.signals = signals; p.xyzA = xyzA; p.n_events = n_events;
+        p.N = N; p.n_lrf = 1; p.n_int = n_int; p.nc = nc;
+        p.lo = lo; p.hi = hi; p.h = (hi - lo) / n_int;
+        p.acc = d_acc; p.n_used = d_used; p.copies = priv_threads; p.lane_split = 1;
+        const size_t psmem = per_thread * priv_threads;
+        const int pw = priv_threads / 32;
+        int occ = 0;
+        ok = cudaFuncSetAttribute((const void *)lrf_fit_shared_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)psmem) == cudaSuccess &&
+             cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void *)lrf_fit_shared_kernel, priv_threads, psmem) == cudaSuccess && occ >= 1;
+        if (ok) {
+            const long long want = (n_events + pw - 1) / pw;
+            const int grid = (int)std::min<long long>(want, (long long)sms * occ);
+            void *args[] = {&p};
+            ok = cudaLaunchKernel((const void *)lrf_fit_shared_kernel, dim3(grid), dim3(priv_threads), args, psmem, st) == cudaSuccess;
+            if (ok) g_launches.fetch_add(1);
+        }
+    } else if (ok && n_events > 0) {
         FitParams p{};
         p.sens_xy = d_xy; p.gains = d_g; p.group = d_group; p.signals = signals; p.xyzA = xyzA; p.n_events = n_events;
         p.N = N; p.n_lrf = n_lrf; p.n_int = n_int; p.nc = nc;
@@ -1275,13 +1339,14 @@ extern "C" int ants_lrf_fit_gains(const float *sensor_xy, const float *knots, co
     float *d_xy = nullptr, *d_c = nullptr;
     double *d_acc = nullptr;
     unsigned long long *d_used = nullptr;
-    auto cleanup = [&]() { cudaFree(d_xy); cudaFree(d_c); cudaFree(d_acc); cudaFree(d_used); cudaGetLastError(); };
-    if (cudaMalloc(&d_xy, (size_t)N * 2 * sizeof(float)) != cudaSuccess || cudaMalloc(&d_c, (size_t)(n_int + 3) * sizeof(float)) != cudaSuccess ||
-        cudaMalloc(&d_acc, (size_t)N * 2 * sizeof(double)) != cudaSuccess ||
-        cudaMalloc(&d_used, (size_t)N * sizeof(unsigned long long)) != cudaSuccess) {
-        cleanup();
-        return ANTS_ERR_NOMEM;
-    }
+    auto cleanup = [&]() { cudaGetLastError(); };
+    std::lock_guard<std::mutex> arena_lock(g_fit_arena.mu);
+    if (!g_fit_arena.begin((size_t)N * 32 + (size_t)(n_int + 3) * 4 + 2048)) return ANTS_ERR_NOMEM;
+    d_xy = g_fit_arena.take<float>((size_t)N * 2);
+    d_c = g_fit_arena.take<float>(n_int + 3);
+    d_acc = g_fit_arena.take<double>((size_t)N * 2);
+    d_used = g_fit_arena.take<unsigned long long>(N);
+    if (!d_xy || !d_c || !d_acc || !d_used) return ANTS_ERR_NOMEM;
     bool ok = cudaMemcpyAsync(d_xy, sensor_xy, (size_t)N * 2 * sizeof(float), cudaMemcpyHostToDevice, st) == cudaSuccess &&
               cudaMemcpyAsync(d_c, coeffs, (size_t)(n_int + 3) * sizeof(float), cudaMemcpyHostToDevice, st) == cudaSuccess &&
               cudaMemsetAsync(d_acc, 0, (size_t)N * 2 * sizeof(double), st) == cudaSuccess &&
@@ -1371,12 +1436,14 @@ extern "C" int ants_lrf_fit_axial_z(const float *sensor_xy, const float *gains, 
     float *d_xy = nullptr, *d_g = nullptr;
     double *d_acc = nullptr;
     unsigned long long *d_used = nullptr;
-    auto cleanup = [&]() { cudaFree(d_xy); cudaFree(d_g); cudaFree(d_acc); cudaFree(d_used); cudaGetLastError(); };
-    if (cudaMalloc(&d_xy, (size_t)N * 2 * sizeof(float)) != cudaSuccess || cudaMalloc(&d_g, (size_t)N * sizeof(float)) != cudaSuccess ||
-        cudaMalloc(&d_acc, smem) != cudaSuccess || cudaMalloc(&d_used, sizeof(unsigned long long)) != cudaSuccess) {
-        cleanup();
-        return ANTS_ERR_NOMEM;
-    }
+    auto cleanup = [&]() { cudaGetLastError(); };
+    std::lock_guard<std::mutex> arena_lock(g_fit_arena.mu);
+    if (!g_fit_arena.begin((size_t)N * 12 + smem + 2048)) return ANTS_ERR_NOMEM;
+    d_xy = g_fit_arena.take<float>((size_t)N * 2);
+    d_g = g_fit_arena.take<float>(N);
+    d_acc = g_fit_arena.take<double>(total);
+    d_used = g_fit_arena.take<unsigned long long>(1);
+    if (!d_xy || !d_g || !d_acc || !d_used) return ANTS_ERR_NOMEM;
     bool ok = cudaMemcpyAsync(d_xy, sensor_xy, (size_t)N * 2 * sizeof(float), cudaMemcpyHostToDevice, st) == cudaSuccess &&
               cudaMemcpyAsync(d_g, g.data(), (size_t)N * sizeof(float), cudaMemcpyHostToDevice, st) == cudaSuccess &&
               cudaMemsetAsync(d_acc, 0, smem, st) == cudaSuccess &&
@@ -1390,13 +1457,17 @@ extern "C" int ants_lrf_fit_axial_z(const float *sensor_xy, const float *gains, 
         p.acc = d_acc; p.n_used = d_used;
         const int warps = 8;
         int occ = 0;
-        ok = cudaFuncSetAttribute((const void *)lrf_fit_rz_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) == cudaSuccess &&
-             cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void *)lrf_fit_rz_kernel, warps * 32, smem) == cudaSuccess && occ >= 1;
+        // the per-event factorised kernel (r-part per warp, one expansion per event) unless told otherwise
+        const bool factorised = !std::getenv("ANTS_FIT_ATOMIC") && smem + (size_t)warps * ncr * 5 * sizeof(double) <= 227 * 1024;
+        const void *kern = factorised ? (const void *)lrf_fit_rz2_kernel : (const void *)lrf_fit_rz_kernel;
+        const size_t ksmem = factorised ? smem + (size_t)warps * ncr * 5 * sizeof(double) : smem;
+        ok = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ksmem) == cudaSuccess &&
+             cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, warps * 32, ksmem) == cudaSuccess && occ >= 1;
         if (ok) {
             const long long want = (n_events + warps - 1) / warps;
             const int grid = (int)std::min<long long>(want, (long long)sms * occ);
             void *args[] = {&p};
-            ok = cudaLaunchKernel((const void *)lrf_fit_rz_kernel, dim3(grid), dim3(warps * 32), args, smem, st) == cudaSuccess;
+            ok = cudaLaunchKernel(kern, dim3(grid), dim3(warps * 32), args, ksmem, st) == cudaSuccess;
             if (ok) g_launches.fetch_add(1);
         }
     }
@@ -1503,15 +1574,17 @@ extern "C" int ants_lrf_fit_xy(const float *sensor_xy, const float *gains, const
     int *d_mem = nullptr;
     double *d_acc = nullptr;
     unsigned long long *d_used = nullptr;
-    auto cleanup = [&]() { cudaFree(d_xy); cudaFree(d_g); cudaFree(d_xf); cudaFree(d_ax); cudaFree(d_mem); cudaFree(d_acc); cudaFree(d_used); cudaGetLastError(); };
-    if (cudaMalloc(&d_xy, (size_t)N * 2 * sizeof(float)) != cudaSuccess || cudaMalloc(&d_g, (size_t)N * sizeof(float)) != cudaSuccess ||
-        cudaMalloc(&d_mem, (size_t)N * sizeof(int)) != cudaSuccess || cudaMalloc(&d_acc, smem) != cudaSuccess ||
-        cudaMalloc(&d_used, sizeof(unsigned long long)) != cudaSuccess ||
-        (xform && cudaMalloc(&d_xf, (size_t)N * 4 * sizeof(float)) != cudaSuccess) ||
-        (composite && cudaMalloc(&d_ax, (size_t)(n_int_r + 3) * sizeof(float)) != cudaSuccess)) {
-        cleanup();
-        return ANTS_ERR_NOMEM;
-    }
+    auto cleanup = [&]() { cudaGetLastError(); };
+    std::lock_guard<std::mutex> arena_lock(g_fit_arena.mu);
+    if (!g_fit_arena.begin((size_t)N * 32 + smem + (size_t)(n_int_r + 3) * 4 + 4096)) return ANTS_ERR_NOMEM;
+    d_xy = g_fit_arena.take<float>((size_t)N * 2);
+    d_g = g_fit_arena.take<float>(N);
+    d_mem = g_fit_arena.take<int>(N);
+    d_acc = g_fit_arena.take<double>(total);
+    d_used = g_fit_arena.take<unsigned long long>(1);
+    if (xform) d_xf = g_fit_arena.take<float>((size_t)N * 4);
+    if (composite) d_ax = g_fit_arena.take<float>(n_int_r + 3);
+    if (!d_xy || !d_g || !d_mem || !d_acc || !d_used || (xform && !d_xf) || (composite && !d_ax)) return ANTS_ERR_NOMEM;
     bool ok = cudaMemcpyAsync(d_xy, sensor_xy, (size_t)N * 2 * sizeof(float), cudaMemcpyHostToDevice, st) == cudaSuccess &&
               cudaMemcpyAsync(d_g, g.data(), (size_t)N * sizeof(float), cudaMemcpyHostToDevice, st) == cudaSuccess &&
               (!xform || cudaMemcpyAsync(d_xf, xform, (size_t)N * 4 * sizeof(float), cudaMemcpyHostToDevice, st) == cudaSuccess);

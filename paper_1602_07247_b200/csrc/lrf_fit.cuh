@@ -344,3 +344,226 @@ __global__ void __launch_bounds__(256) lrf_fit_xy_kernel(const FitXYParams p) {
 }
 
 }  // namespace ants
+
+namespace ants {
+
+// ---- axial LRF calculation, ONE shared profile (n_lrf = 1), without atomics in the loop (round 2) ----------------
+// lrf_fit_kernel spends its time in shared-memory FP64 CAS loops (14 per pair, several lanes of a warp hitting the
+// same interval).  Here every THREAD owns a private copy of the 5 (n + 3) band entries in shared memory, laid out
+// [entry][thread] so that a warp's accesses to one entry are consecutive doubles: the 14 updates of a pair are plain
+// load-add-store, free of conflicts and of retries, and the bound becomes the shared-memory bandwidth (224 B per
+// pair).  The copies are summed once at the end and added to the global accumulators.
+__global__ void __launch_bounds__(128) lrf_fit_shared_kernel(const FitParams p) {
+    extern __shared__ double fs_smem[];                 // [nc * 5][blockDim.x]
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, warps = blockDim.x >> 5, T = blockDim.x;
+    const int entries = p.nc * 5;
+    for (int i = threadIdx.x; i < entries * T; i += T) fs_smem[i] = 0.0;
+    __syncthreads();
+    double *mine = fs_smem + threadIdx.x;
+    unsigned long long used = 0ULL;
+    // a lane keeps the sensors i = lane + 32 c: their constants stay in registers for all events
+    double sx[4], sy[4], ginv[4];
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+        const int i = lane + 32 * c;
+        sx[c] = i < p.N ? (double)p.sens_xy[2 * i] : 0.0;
+        sy[c] = i < p.N ? (double)p.sens_xy[2 * i + 1] : 0.0;
+        ginv[c] = i < p.N ? 1.0 / (double)p.gains[i] : 0.0;
+    }
+    const double inv_h = 1.0 / p.h;
+    // few warps fit beside the private copies, so latency is covered inside the warp: the position rows and the
+    // signals of the next two events wait in registers, and the (independent) arithmetic of a lane's four sensors
+    // is written side by side before their updates
+    const long long stride = (long long)gridDim.x * warps;
+    constexpr int kAhead = 2;
+    float4 pe_q[kAhead + 1];
+    float sg_q[kAhead + 1][4];
+    auto fetch = [&](int slot, long long ev) {
+        const bool in = ev < p.n_events;
+        pe_q[slot] = in ? __ldg(reinterpret_cast<const float4 *>(p.xyzA) + ev) : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            const int i = lane + 32 * c;
+            sg_q[slot][c] = (in && i < p.N) ? __ldg(p.signals + ev * p.N + i) : 0.f;
+        }
+    };
+    // one pair's update of this thread's private band: all loads, then the adds, then the stores
+    auto update = [&](int k, const double b4[4], double yv) {
+        double *row = mine + (size_t)k * 5 * T;
+        double v[14];
+        int n = 0;
+#pragma unroll
+        for (int a = 0; a < 4; ++a) {
+            v[n++] = row[(a * 5 + 4) * T];
+#pragma unroll
+            for (int c = a; c < 4; ++c) v[n++] = row[(a * 5 + c - a) * T];
+        }
+        n = 0;
+#pragma unroll
+        for (int a = 0; a < 4; ++a) {
+            v[n++] += b4[a] * yv;
+#pragma unroll
+            for (int c = a; c < 4; ++c) v[n++] += b4[a] * b4[c];
+        }
+        n = 0;
+#pragma unroll
+        for (int a = 0; a < 4; ++a) {
+            row[(a * 5 + 4) * T] = v[n++];
+#pragma unroll
+            for (int c = a; c < 4; ++c) row[(a * 5 + c - a) * T] = v[n++];
+        }
+    };
+    auto prepare = [&](double x, double y, double sxi, double syi, double sv, double invAg, int &k, double b4[4], double &yv) -> bool {
+        const double dx = x - sxi, dy = y - syi;
+        const double r = sqrt(dx * dx + dy * dy);
+        yv = sv * invAg;                                                                          // R21, R23
+        const double t = (r - p.lo) * inv_h;
+        k = min(max((int)floor(t), 0), p.n_int - 1);
+        const double u = t - (double)k, o = 1.0 - u, u2 = u * u, u3 = u2 * u;
+        b4[0] = o * o * o * (1.0 / 6.0);
+        b4[1] = (3.0 * u3 - 6.0 * u2 + 4.0) * (1.0 / 6.0);
+        b4[2] = (-3.0 * u3 + 3.0 * u2 + 3.0 * u + 1.0) * (1.0 / 6.0);
+        b4[3] = u3 * (1.0 / 6.0);
+        return r >= p.lo && r <= p.hi;                                                            // R22
+    };
+    const long long e0 = (long long)blockIdx.x * warps + warp;
+#pragma unroll
+    for (int a = 0; a < kAhead; ++a) fetch(a, e0 + a * stride);
+    for (long long e = e0; e < p.n_events; e += stride) {
+        fetch(kAhead, e + kAhead * stride);
+        const float4 pe = pe_q[0];
+        float sg[4];
+#pragma unroll
+        for (int c = 0; c < 4; ++c) sg[c] = sg_q[0][c];
+#pragma unroll
+        for (int a = 0; a < kAhead; ++a) {
+            pe_q[a] = pe_q[a + 1];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) sg_q[a][c] = sg_q[a + 1][c];
+        }
+        const double x = (double)pe.x, y = (double)pe.y, A = (double)pe.w;
+        if (!(fabs(x) <= 1.7e308 && fabs(y) <= 1.7e308 && A > 0.0 && A <= 1.7e308)) continue;     // R22
+        const double invA = 1.0 / A;
+        int kk[4];
+        double bb[4][4], yy[4];
+        bool ok[4];
+#pragma unroll
+        for (int c = 0; c < 4; ++c)
+            ok[c] = prepare(x, y, sx[c], sy[c], (double)sg[c], invA * ginv[c], kk[c], bb[c], yy[c]) && lane + 32 * c < p.N;
+#pragma unroll
+        for (int c = 0; c < 4; ++c)
+            if (ok[c]) { update(kk[c], bb[c], yy[c]); ++used; }
+        for (int i = lane + 128; i < p.N; i += 32) {                     // arrays of more than 128 sensors
+            int k;
+            double b4[4], yv;
+            if (prepare(x, y, (double)p.sens_xy[2 * i], (double)p.sens_xy[2 * i + 1], (double)__ldg(p.signals + e * p.N + i),
+                        invA / (double)p.gains[i], k, b4, yv)) {
+                update(k, b4, yv);
+                ++used;
+            }
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) used += __shfl_xor_sync(0xffffffffu, used, o);
+    if (lane == 0 && used) atomicAdd(p.n_used, used);
+    __syncthreads();
+    for (int i = threadIdx.x; i < entries; i += T) {
+        double s = 0.0;
+        for (int c = 0; c < T; ++c) s += fs_smem[(size_t)i * T + (c + threadIdx.x) % T];     // staggered: no bank conflicts
+        if (s != 0.0) atomicAdd(p.acc + i, s);
+    }
+}
+
+}  // namespace ants
+
+namespace ants {
+
+// ---- axial+z tensor LRF calculation, factorised per event (round 2) ------------------------------------------------
+// All pairs of one event share the event's z, hence the same four z-basis weights bz: the event's contribution to
+// the normal equations is (bz bz^T) (x) (sum_i br_i br_i^T) and to the right-hand side bz (x) (sum_i br_i y_i).  The
+// warp therefore first accumulates the event's r-part -- the banded 4-wide matrix and the vector of an axial fit,
+// 14 entries per pair -- in a buffer of its own, and then expands it once into the CTA's accumulators: about
+// 1,200 conflict-free adds per event instead of 152 per pair (lrf_fit_rz_kernel; 4,500 per event on config 4).
+__global__ void __launch_bounds__(256) lrf_fit_rz2_kernel(const FitRZParams p) {
+    extern __shared__ double rz2_smem[];                // [nc][29] CTA accumulators, then [warps][ncr][5] r-parts
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, warps = blockDim.x >> 5;
+    const int total = p.nc * 29, rlen = p.ncr * 5;
+    for (int i = threadIdx.x; i < total + warps * rlen; i += blockDim.x) rz2_smem[i] = 0.0;
+    __syncthreads();
+    double *Rb = rz2_smem + total + (size_t)warp * rlen;      // [ncr][5]: {R[j][j], R[j][j+1], R[j][j+2], R[j][j+3], rhs[j]}
+    unsigned long long used = 0ULL;
+    for (long long e = (long long)blockIdx.x * warps + warp; e < p.n_events; e += (long long)gridDim.x * warps) {
+        const float4 pe = reinterpret_cast<const float4 *>(p.xyzA)[e];
+        const double x = (double)pe.x, y = (double)pe.y, z = (double)pe.z, A = (double)pe.w;
+        if (!(fabs(x) <= 1.7e308 && fabs(y) <= 1.7e308 && A > 0.0 && A <= 1.7e308 && z >= p.z_lo && z <= p.z_hi)) continue;
+        const double tz = (z - p.z_lo) / p.hz;
+        const int kz = min((int)floor(tz), p.n_z - 1);
+        const double uz = tz - (double)kz, oz = 1.0 - uz, uz2 = uz * uz, uz3 = uz2 * uz;
+        const double bz[4] = {oz * oz * oz / 6.0, (3.0 * uz3 - 6.0 * uz2 + 4.0) / 6.0,
+                              (-3.0 * uz3 + 3.0 * uz2 + 3.0 * uz + 1.0) / 6.0, uz3 / 6.0};
+        const float *sig = p.signals + e * p.N;
+        int k_min = p.ncr, k_max = -1;
+        for (int i = lane; i < p.N; i += 32) {
+            const double dx = x - (double)p.sens_xy[2 * i], dy = y - (double)p.sens_xy[2 * i + 1];
+            const double r = sqrt(dx * dx + dy * dy);
+            if (!(r >= p.r_lo && r <= p.r_hi)) continue;
+            const double yv = (double)__ldg(sig + i) / (A * (double)p.gains[i]);
+            const double tr = (r - p.r_lo) / p.hr;
+            const int kr = min((int)floor(tr), p.n_r - 1);
+            const double u = tr - (double)kr, o = 1.0 - u, u2 = u * u, u3 = u2 * u;
+            const double br[4] = {o * o * o / 6.0, (3.0 * u3 - 6.0 * u2 + 4.0) / 6.0,
+                                  (-3.0 * u3 + 3.0 * u2 + 3.0 * u + 1.0) / 6.0, u3 / 6.0};
+#pragma unroll
+            for (int a = 0; a < 4; ++a) {
+                double *row = Rb + (size_t)(kr + a) * 5;
+                atomicAdd(row + 4, br[a] * yv);
+#pragma unroll
+                for (int c = a; c < 4; ++c) atomicAdd(row + (c - a), br[a] * br[c]);
+            }
+            k_min = min(k_min, kr);
+            k_max = max(k_max, kr + 3);
+            ++used;
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            k_min = min(k_min, __shfl_xor_sync(0xffffffffu, k_min, o));
+            k_max = max(k_max, __shfl_xor_sync(0xffffffffu, k_max, o));
+        }
+        __syncwarp();
+        // expand: rows (kz + b1) ncr + ja, slots (dz, dr) of the 4 x 7 block and the right-hand side
+        const int n_rows = k_max - k_min + 1;
+        for (int it = lane; it < n_rows * 29; it += 32) {
+            const int s = it % 29, ja = k_min + it / 29;
+            if (s == 28) {
+                const double rv = Rb[(size_t)ja * 5 + 4];
+                if (rv != 0.0) {
+#pragma unroll
+                    for (int b1 = 0; b1 < 4; ++b1) atomicAdd(rz2_smem + (size_t)((kz + b1) * p.ncr + ja) * 29 + 28, bz[b1] * rv);
+                }
+            } else {
+                const int dz = s / 7, dr = s - dz * 7 - 3, jc = ja + dr;
+                if (jc < 0 || jc >= p.ncr || (dz == 0 && dr < 0)) continue;
+                const double rv = Rb[(size_t)min(ja, jc) * 5 + (dr < 0 ? -dr : dr)];
+                if (rv == 0.0) continue;
+#pragma unroll
+                for (int b1 = 0; b1 < 4; ++b1) {
+                    // b2 = b1 + dz <= 3; the weights are picked by compile-time b1 and a small select on dz
+                    if (b1 + dz > 3) continue;
+                    const double w2 = dz == 0 ? bz[b1] : dz == 1 ? bz[(b1 + 1) & 3] : dz == 2 ? bz[(b1 + 2) & 3] : bz[3];
+                    atomicAdd(rz2_smem + (size_t)((kz + b1) * p.ncr + ja) * 29 + s, bz[b1] * w2 * rv);
+                }
+            }
+        }
+        __syncwarp();
+        for (int it = lane; it < n_rows * 5; it += 32) Rb[(size_t)k_min * 5 + it] = 0.0;
+        __syncwarp();
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) used += __shfl_xor_sync(0xffffffffu, used, o);
+    if (lane == 0 && used) atomicAdd(p.n_used, used);
+    __syncthreads();
+    for (int i = threadIdx.x; i < total; i += blockDim.x)
+        if (rz2_smem[i] != 0.0) atomicAdd(p.acc + i, rz2_smem[i]);
+}
+
+}  // namespace ants

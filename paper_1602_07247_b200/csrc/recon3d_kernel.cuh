@@ -42,72 +42,10 @@ __global__ void __launch_bounds__(256) recon3d_kernel(const Params p) {
     long long e_next = grab_event(p.ctr, lane);
     for (long long e = e_next; e < p.n_events; e = e_next) {
         e_next = grab_event(p.ctr, lane);
-        // ---- a1: load signals, prepare, centroid ----
-        const float *sig = p.signals + e * N;
-        float sumS = 0.f, sw = 0.f, sxw = 0.f, syw = 0.f;
-        bool finite = true;
-        for (int i = lane; i < N; i += 32) {
-            if (m.passive && m.passive[i]) {             // R19: out of everything, signal not looked at
-                w.SC[i] = make_float2(0.f, ANTS_QNAN);
-                continue;
-            }
-            float S = __ldg(sig + i);
-            finite = finite && (fabsf(S) <= 3.402823466e38f);
-            if (METHOD == 0) S = fmaxf(S, 0.f);          // R18
-            float4 sn = sens_s[i];
-            float wgt = S * sn.w;
-            sumS += S;
-            sw += wgt;
-            sxw = fmaf(sn.x, wgt, sxw);
-            syw = fmaf(sn.y, wgt, syw);
-            float cs = 0.f;
-            if (METHOD == 0 && S > 0.f) cs = log2f(S * sn.w);
-            w.SC[i] = make_float2(S, cs);
-        }
-        finite = __all_sync(kFull, finite);
-        sumS = warp_sum(sumS);
-        sw = warp_sum(sw);
-        sxw = warp_sum(sxw);
-        syw = warp_sum(syw);
-        __syncwarp();
-        if (!finite || !(sumS > 0.f) || (p.seed_mode == 0 && !(sw > 0.f))) {
-            if (lane == 0) {
-                const float qnan = __int_as_float(0x7fc00000);
-                reinterpret_cast<float4 *>(p.out_xyzA)[e] = make_float4(qnan, qnan, qnan, qnan);
-                p.out_score[e] = kInf;
-            }
-            if (p.out_path)
-                for (int k = lane; k < p.K; k += 32) p.out_path[e * p.K + k] = 0xFFFF;
-            continue;
-        }
-        float cx = sxw / sw, cy = syw / sw, cz = z_start;
-        if (p.seed_mode == 1) strongest_sensor(w.SC, sens_s, N, lane, cx, cy);    // R20
-        float A_ref = 1.f;
-        if (m.select) {
-            // R19: the sensors of the statistical part, fixed for the event (threshold, distance from start)
-            float s_act = 0.f;
-            for (int i = lane; i < N; i += 32) {
-                float2 sc = w.SC[i];
-                if (sc.y == sc.y) {
-                    const float4 sn = sens_s[i];
-                    const float dx = cx - sn.x, dy = cy - sn.y;
-                    const bool keep = !(sc.x < m.signal_min) && !(sqrtf(fmaf(dx, dx, dy * dy)) > m.dist_max);
-                    if (keep) s_act += sc.x;
-                    else w.SC[i] = make_float2(0.f, ANTS_QNAN);
-                }
-            }
-            sumS = warp_sum(s_act);
-            __syncwarp();
-            if (!(sumS > 0.f)) {
-                if (lane == 0) {
-                    reinterpret_cast<float4 *>(p.out_xyzA)[e] = make_float4(ANTS_QNAN, ANTS_QNAN, ANTS_QNAN, ANTS_QNAN);
-                    p.out_score[e] = kInf;
-                }
-                if (p.out_path)
-                    for (int k = lane; k < p.K; k += 32) p.out_path[e * p.K + k] = 0xFFFF;
-                continue;
-            }
-        }
+        // ---- a1: signals, centroid / strongest-sensor start, selection (prepare_event, recon_common.cuh) ----
+        float sumS, cx, cy;
+        if (!prepare_event<METHOD>(p, sens_s, w.SC, e, lane, sumS, cx, cy)) continue;
+        float cz = z_start, A_ref = 1.f;
 
         float h = p.h0_xy, hz = p.h0_z;
         for (int k = 0; k < p.K; ++k) {

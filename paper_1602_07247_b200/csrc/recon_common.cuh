@@ -185,9 +185,10 @@ __device__ __forceinline__ void strongest_sensor(const float2 *SC, const float4 
 // {S_i, log2(S_i / gL_i) or 0}, an inactive sensor is flagged by NaN in .y.  Returns false when the event fails
 // (its outputs are written here: NaN row, score +inf, path 0xFFFF).
 struct Params;
+// `pre` (optional): the event's first 128 signals already in registers, pre[c] = signal of sensor lane + 32 c.
 template <int METHOD>
 __device__ bool prepare_event(const Params &p, const float4 *sens_s, float2 *SC, long long e, int lane,
-                              float &sumS, float &cx, float &cy);
+                              float &sumS, float &cx, float &cy, const float *pre = nullptr);
 
 // same result as warp_argmin through two integer reductions (REDUX): scores mapped to order-preserving
 // unsigned keys, then the lowest index among the lanes holding the minimum.  s must not be NaN.
@@ -225,20 +226,23 @@ __device__ __forceinline__ float horner(const float4 p, float v) {
 }
 
 template <int METHOD>
-__device__ bool prepare_event(const Params &p, const float4 *sens_s, float2 *SC, long long e, int lane,
-                              float &sumS, float &cx, float &cy) {
+__device__ __forceinline__ bool prepare_event(const Params &p, const float4 *sens_s, float2 *SC, long long e, int lane,
+                                              float &sumS, float &cx, float &cy, const float *pre) {
     const ModelDev &m = p.m;
     const int N = m.N;
     const float *sig = p.signals + e * N;
     float sw = 0.f, sxw = 0.f, syw = 0.f;
     sumS = 0.f;
     bool finite = true;
-    for (int i = lane; i < N; i += 32) {
+#pragma unroll 4
+    for (int i = lane, c = 0; i < N; i += 32, ++c) {
         if (m.passive && m.passive[i]) {             // R19: out of everything, signal not looked at
             SC[i] = make_float2(0.f, ANTS_QNAN);
             continue;
         }
-        float S = __ldg(sig + i);
+        float S;
+        if (pre && c < 4) S = c == 0 ? pre[0] : c == 1 ? pre[1] : c == 2 ? pre[2] : pre[3];
+        else S = __ldg(sig + i);
         finite = finite && (fabsf(S) <= 3.402823466e38f);
         if (METHOD == 0) S = fmaxf(S, 0.f);          // R18
         const float4 sn = sens_s[i];

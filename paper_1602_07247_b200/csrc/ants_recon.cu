@@ -41,6 +41,7 @@ struct Plan {
     size_t smem = 0;         // dynamic shared memory per CTA
     int k_diff = 0;          // first differential iteration (K = never)
     int k_series = 0;        // axial+z Poisson: first iteration with the log1p series
+    int gen_dtab = 0;        // general kernel: double copy of the XY coefficients in shared memory
     const void *kernel = nullptr;
     bool ready = false;      // cudaFuncSetAttribute + occupancy done (needs the device)
 };
@@ -786,19 +787,27 @@ static int make_plan_gen(const ants_lrf *h, const ants_grid_params_t *g, int32_t
     pl.npt = (int)((nodes + 31) / 32);
     pl.kernel = kernel_gen(method, m.lrf_kind);
     if (!pl.kernel) return ANTS_ERR_UNSUPPORTED;
-    // FP64 scores from the first grid that reaches less than one knot interval of any spline axis from its
-    // centre (the grids the packed kernels score differentially)
+    // FP64 scores from the first grid whose reach is a small fraction of a knot interval of every spline axis:
+    // 0.225 for Poisson (with a contraction of 0.5, two iterations after the grids the packed kernels start to
+    // score differentially), 0.1 for the chi-square forms, whose FP32 residual form keeps resolving neighbouring
+    // nodes much longer.  Measured in round 2 on configs 6 and 8 (6,007 events each): with FP32 two iterations
+    // beyond these switch points the oracle's best-to-second gap at a diverging node stays below 2.5e-5
+    // (Poisson) and 6e-7 (chi-square, FP32 to the last iteration) against the 1e-4 the index rule allows.
+    const double frac = method == ANTS_POISSON_ML ? 0.225 : 0.1;
     pl.k_diff = g->n_iter;
     const double half = 0.5 * (G - 1);
     double knot = std::fmin(h->knot_r > 0.0 ? h->knot_r : 1e300, h->knot_xy > 0.0 ? h->knot_xy : 1e300);
     const double plane = m.lrf_kind == 5 ? ((double)m.z_hi - (double)m.z_lo) / (m.n_planes - 1) : 1e300;
     double hxy = g->step0_xy, hz = g->dim == 3 ? g->step0_z : 0.0;
     for (int k = 0; k < g->n_iter; ++k, hxy *= (double)g->factor, hz *= (double)g->factor)
-        if (std::sqrt(2.0) * half * hxy * 1.001 <= 0.9 * knot && half * hz * 1.001 <= 0.9 * plane) { pl.k_diff = k; break; }
+        if (std::sqrt(2.0) * half * hxy * 1.001 <= frac * knot && half * hz * 1.001 <= frac * plane) { pl.k_diff = k; break; }
+    if (const char *e = std::getenv("ANTS_GEN_KFINE")) pl.k_diff = std::min(g->n_iter, std::max(0, std::atoi(e)));   // experiment knob
     pl.k_series = pl.k_diff;
     const int rows = (m.lrf_kind == 1 || m.lrf_kind == 4) ? m.n_lrf * (m.n_r + 1) : 0;
     const int ncxy = m.lrf_kind >= 3 ? m.n_lrf * std::max(m.n_planes, 1) * (m.nx + 3) * (m.ny + 3) : 0;
-    pick_cta_shape(cta_smem_bytes_gen(m.N, rows, ncxy), warp_smem_bytes_gen(m.N), pl);
+    // the double copy of the XY coefficients when the CTA's tables stay below 100 KB with it
+    pl.gen_dtab = ncxy > 0 && cta_smem_bytes_gen(m.N, rows, ncxy, 1) <= 100 * 1024 ? 1 : 0;
+    pick_cta_shape(cta_smem_bytes_gen(m.N, rows, ncxy, pl.gen_dtab), warp_smem_bytes_gen(m.N), pl);
     if (pl.smem > 227 * 1024) return ANTS_ERR_UNSUPPORTED;
     return ANTS_OK;
 }
@@ -952,6 +961,7 @@ static int launch(const ants_lrf *h, const float *signals, int64_t n_events, con
     p.seed_mode = g->seed_mode;
     p.warps_per_cta = pl.warps;
     p.tile_events = pl.warps;
+    p.gen_dtab = pl.gen_dtab;
 
     long long want = (n_events + pl.warps - 1) / pl.warps;
     long long cap = (long long)h->sm_count * pl.ctas_per_sm;
@@ -1085,7 +1095,8 @@ extern "C" int ants_refine(const ants_lrf_t *lrf, const float *signals, int64_t 
     const void *kernel = kernel_refine(method);
     const int warps = 8;
     const int ncxy = m.lrf_kind >= 3 ? m.n_lrf * std::max(m.n_planes, 1) * (m.nx + 3) * (m.ny + 3) : 0;
-    const size_t smem = cta_smem_bytes_gen(m.N, 0, ncxy) + (size_t)warps * ((size_t)m.N * 40 + 8);
+    const int dtab = ncxy > 0 && cta_smem_bytes_gen(m.N, 0, ncxy, 1) <= 100 * 1024 ? 1 : 0;
+    const size_t smem = cta_smem_bytes_gen(m.N, 0, ncxy, dtab) + (size_t)warps * ((size_t)m.N * 40 + 8);
     if (smem > 227 * 1024) return ANTS_ERR_UNSUPPORTED;
     int occ = 0;
     if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
@@ -1102,6 +1113,7 @@ extern "C" int ants_refine(const ants_lrf_t *lrf, const float *signals, int64_t 
     rp.dim = dim;
     rp.seed_mode = seed_mode;
     rp.n_steps = n_steps;
+    rp.dtab = dtab;
     const long long want = (n_events + warps - 1) / warps;
     const int grid = (int)std::min<long long>(want, (long long)lrf->sm_count * occ);
     void *args[] = {&rp};

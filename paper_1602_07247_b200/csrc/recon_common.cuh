@@ -63,6 +63,7 @@ struct Params {
     int total_warps;        // gridDim.x * warps_per_cta
     int warps_per_cta;
     int tile_events;        // events staged per CTA tile (= warps_per_cta)
+    int gen_dtab;           // general kernel: a double copy of the XY coefficients sits in shared memory
 };
 
 __device__ __forceinline__ float sqrt_approx(float x) {

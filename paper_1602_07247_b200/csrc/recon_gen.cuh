@@ -29,8 +29,12 @@ __host__ __device__ inline size_t warp_smem_bytes_gen(int N) {
     return ((size_t)N * 8 + (size_t)N * 2 + 15) / 16 * 16;
 }
 // CTA-shared tables: sens_s [N] float4, xf_s [N] float4, poly_s [rows] float4, grp_s [N] int, cxy_s [ncxy] float
-__host__ __device__ inline size_t cta_smem_bytes_gen(int N, int rows, int ncxy) {
-    return (size_t)(2 * N + rows) * 16 + ((size_t)N * 4 + 15) / 16 * 16 + ((size_t)ncxy * 4 + 15) / 16 * 16;
+// and, when it fits (dtab), cxyd_s [ncxy] double: the FP64 evaluations then read their coefficients without a
+// conversion (F2F runs on the XU pipe at 16 lanes/clk/SM: 16 conversions per pair made the FP64 grids XU-bound,
+// 71 % XU-pipe busy in the first round-2 capture)
+__host__ __device__ inline size_t cta_smem_bytes_gen(int N, int rows, int ncxy, int dtab) {
+    return (size_t)(2 * N + rows) * 16 + ((size_t)N * 4 + 15) / 16 * 16 + ((size_t)ncxy * 4 + 15) / 16 * 16 +
+           (dtab ? (size_t)ncxy * 8 : 0);
 }
 
 // uniform cubic B-spline basis weights of the local coordinate f in [0, 1] (R7)
@@ -43,7 +47,9 @@ __device__ __forceinline__ void basis4(T f, T b[4]) {
     b[3] = f3 * T(1.0 / 6.0);
 }
 
-// interval and local coordinate of x on [lo, lo + n / sc], clamped into the range (R5)
+// interval and local coordinate of x on [lo, lo + n / sc], clamped into the range (R5).  (A magic-number rounding
+// in place of the two conversions was measured slower in round 2: it trades two XU-pipe conversions for five more
+// FP32 / FP64 adds, and once the coefficients need no conversion the XU pipe is no longer the bound.)
 template <typename T>
 __device__ __forceinline__ void locate(T x, T lo, T sc, int n, int &k, T &f) {
     T t = (x - lo) * sc;
@@ -53,9 +59,9 @@ __device__ __forceinline__ void locate(T x, T lo, T sc, int n, int &k, T &f) {
 }
 
 // tensor-product spline value from the coefficient table c [ny + 3][nx + 3] (u fastest), R30
-template <typename T>
-__device__ __forceinline__ T xy_value(const float *c, int nu3, int ku, int kv, const T bu[4], const T bv[4]) {
-    const float *q = c + kv * nu3 + ku;
+template <typename T, typename TC>
+__device__ __forceinline__ T xy_value(const TC *c, int nu3, int ku, int kv, const T bu[4], const T bv[4]) {
+    const TC *q = c + kv * nu3 + ku;
     T s = T(0);
 #pragma unroll
     for (int b = 0; b < 4; ++b) {
@@ -86,8 +92,8 @@ struct NodeLrf {
 };
 
 template <int LRFK, typename T>
-__device__ __forceinline__ T lrf_value(const ModelDev &m, const float4 *poly_s, const float *cxy_s, const float4 sn,
-                                       const float4 xf, int tab, T x, T y, int pz, T wz) {
+__device__ __forceinline__ T lrf_value(const ModelDev &m, const float4 *poly_s, const float *cxy_s, const double *cxyd_s,
+                                       const float4 sn, const float4 xf, int tab, T x, T y, int pz, T wz) {
     const T dx = x - T(sn.x), dy = y - T(sn.y);
     T s = T(0);
     if (LRFK == kAxial || LRFK == kComposite) {
@@ -101,17 +107,28 @@ __device__ __forceinline__ T lrf_value(const ModelDev &m, const float4 *poly_s, 
         const T u = T(xf.x) * dx + T(xf.y) * dy, v = T(xf.z) * dx + T(xf.w) * dy;
         int ku, kv;
         T fu, fv, bu[4], bv[4];
-        locate<T>(u, T(m.u_lo), T(m.su), m.nx, ku, fu);
-        locate<T>(v, T(m.v_lo), T(m.sv), m.ny, kv, fv);
+        locate(u, T(m.u_lo), T(m.su), m.nx, ku, fu);
+        locate(v, T(m.v_lo), T(m.sv), m.ny, kv, fv);
         basis4<T>(fu, bu);
         basis4<T>(fv, bv);
         const int nu3 = m.nx + 3, per_plane = nu3 * (m.ny + 3);
-        if (LRFK == kSliced) {
-            const float *c0 = cxy_s + ((size_t)tab * m.n_planes + pz) * per_plane;
-            const T s0 = xy_value<T>(c0, nu3, ku, kv, bu, bv), s1 = xy_value<T>(c0 + per_plane, nu3, ku, kv, bu, bv);
-            s += (T(1) - wz) * s0 + wz * s1;                   // R32: linear interpolation between the two planes
+        const size_t off = LRFK == kSliced ? ((size_t)tab * m.n_planes + pz) * per_plane : (size_t)tab * per_plane;
+        if (sizeof(T) == 8 && cxyd_s) {
+            const double *c0 = cxyd_s + off;
+            if (LRFK == kSliced) {
+                const T s0 = xy_value<T, double>(c0, nu3, ku, kv, bu, bv), s1 = xy_value<T, double>(c0 + per_plane, nu3, ku, kv, bu, bv);
+                s += (T(1) - wz) * s0 + wz * s1;
+            } else {
+                s += xy_value<T, double>(c0, nu3, ku, kv, bu, bv);
+            }
         } else {
-            s += xy_value<T>(cxy_s + (size_t)tab * per_plane, nu3, ku, kv, bu, bv);
+            const float *c0 = cxy_s + off;
+            if (LRFK == kSliced) {
+                const T s0 = xy_value<T, float>(c0, nu3, ku, kv, bu, bv), s1 = xy_value<T, float>(c0 + per_plane, nu3, ku, kv, bu, bv);
+                s += (T(1) - wz) * s0 + wz * s1;               // R32: linear interpolation between the two planes
+            } else {
+                s += xy_value<T, float>(c0, nu3, ku, kv, bu, bv);
+            }
         }
     }
     return s;
@@ -149,9 +166,14 @@ __global__ void __launch_bounds__(256, 2) recon_gen_kernel(const Params p) {
         xf_s[i] = m.xf ? m.xf[i] : make_float4(1.f, 0.f, 0.f, 1.f);
     }
     for (int i = threadIdx.x; i < rows; i += blockDim.x) poly_s[i] = m.poly[i];
-    for (int i = threadIdx.x; i < ncxy; i += blockDim.x) cxy_s[i] = m.cxy[i];
+    double *cxyd_s = p.gen_dtab ? reinterpret_cast<double *>(reinterpret_cast<unsigned char *>(cxy_s) + ((size_t)ncxy * 4 + 15) / 16 * 16)
+                                : nullptr;
+    for (int i = threadIdx.x; i < ncxy; i += blockDim.x) {
+        cxy_s[i] = m.cxy[i];
+        if (cxyd_s) cxyd_s[i] = (double)m.cxy[i];
+    }
     __syncthreads();
-    unsigned char *wbase = smem + cta_smem_bytes_gen(N, rows, ncxy) + (size_t)warp * warp_smem_bytes_gen(N);
+    unsigned char *wbase = smem + cta_smem_bytes_gen(N, rows, ncxy, p.gen_dtab) + (size_t)warp * warp_smem_bytes_gen(N);
     float2 *SC = reinterpret_cast<float2 *>(wbase);                       // {S_i prepared, log2(S_i / gL_i) or 0}
     unsigned short *act = reinterpret_cast<unsigned short *>(SC + N);     // indices of the event's active sensors
 
@@ -211,7 +233,7 @@ __global__ void __launch_bounds__(256, 2) recon_gen_kernel(const Params p) {
             for (int q = 0; q < n_act; ++q) {
                 const int i = act[q];
                 const float4 sn = sens_s[i];
-                const double L = (double)sn.z * lrf_value<LRFK, double>(m, poly_s, cxy_s, sn, xf_s[i], grp_s[i], x, y, pz, wz);
+                const double L = (double)sn.z * lrf_value<LRFK, double>(m, poly_s, cxy_s, cxyd_s, sn, xf_s[i], grp_s[i], x, y, pz, wz);
                 const double S = (double)SC[i].x;
                 sumL += L;
                 if (METHOD == 0) {
@@ -253,7 +275,7 @@ __global__ void __launch_bounds__(256, 2) recon_gen_kernel(const Params p) {
             for (int q = lane; q < n_act; q += 32) {
                 const int i = act[q];
                 const float4 sn = sens_s[i];
-                sl += sn.z * lrf_value<LRFK, float>(m, poly_s, cxy_s, sn, xf_s[i], grp_s[i], (float)cx, (float)cy, pz, wz);
+                sl += sn.z * lrf_value<LRFK, float>(m, poly_s, cxy_s, cxyd_s, sn, xf_s[i], grp_s[i], (float)cx, (float)cy, pz, wz);
             }
             sl = warp_sum(sl);
             A_ref = sl > 0.f ? sumS / sl : 1.f;
@@ -315,7 +337,7 @@ __global__ void __launch_bounds__(256, 2) recon_gen_kernel(const Params p) {
                         const float fourth = METHOD == 0 ? (sc2.x > 0.f ? sc2.y - lA : 0.f) : 1.f / fmaxf(sc2.x, 1.f);
 #pragma unroll
                         for (int j = 0; j < kNB; ++j) {
-                            float s = lrf_value<LRFK, float>(m, poly_s, cxy_s, sn, xf, tab, xf32[j], yf32[j], pzf[j], wzf[j]);
+                            float s = lrf_value<LRFK, float>(m, poly_s, cxy_s, cxyd_s, sn, xf, tab, xf32[j], yf32[j], pzf[j], wzf[j]);
                             if (METHOD == 0) {
                                 bad[j] = bad[j] || (s <= 0.f && sc2.x > 0.f);
                                 a2[j] = fmaf(sn.z, s, a2[j]);
@@ -393,7 +415,7 @@ __global__ void __launch_bounds__(256, 2) recon_gen_kernel(const Params p) {
                     if (q < n_act) {
                         const int i = act[q];
                         const float4 sn = sens_s[i];
-                        const double L = (double)sn.z * lrf_value<LRFK, double>(m, poly_s, cxy_s, sn, xf_s[i], grp_s[i], cx, cy, pz, wz);
+                        const double L = (double)sn.z * lrf_value<LRFK, double>(m, poly_s, cxy_s, cxyd_s, sn, xf_s[i], grp_s[i], cx, cy, pz, wz);
                         const double S = (double)SC[i].x, wi = 1.0 / fmax(S, 1.0);
                         Lq[t] = L;
                         sumL += L;
@@ -419,7 +441,7 @@ __global__ void __launch_bounds__(256, 2) recon_gen_kernel(const Params p) {
                         double L = Lq[t];
                         if (n_act > 256) {
                             const float4 sn = sens_s[i];
-                            L = (double)sn.z * lrf_value<LRFK, double>(m, poly_s, cxy_s, sn, xf_s[i], grp_s[i], cx, cy, pz, wz);
+                            L = (double)sn.z * lrf_value<LRFK, double>(m, poly_s, cxy_s, cxyd_s, sn, xf_s[i], grp_s[i], cx, cy, pz, wz);
                         }
                         const double S = (double)SC[i].x;
                         if (METHOD == 0) {

@@ -22,6 +22,7 @@ struct RefineParams {
     float *score;           // [E] out
     int dim;                // 2: (x, y); 3: (x, y, z)
     int seed_mode, n_steps;
+    int dtab;               // a double copy of the XY coefficients sits in shared memory
     // fields prepare_event reads through a Params view
     unsigned long long *ctr;
     int total_warps;
@@ -37,10 +38,11 @@ __device__ __forceinline__ void dbasis4(T f, T d[4]) {
 }
 
 // tensor-product spline value and partial derivatives (per unit of the local coordinates) from c [.][nu3]
-__device__ __forceinline__ double xy_value_grad(const float *c, int nu3, int ku, int kv, const double bu[4],
+template <typename TC>
+__device__ __forceinline__ double xy_value_grad(const TC *c, int nu3, int ku, int kv, const double bu[4],
                                                 const double bv[4], const double du[4], const double dv[4],
                                                 double &s_u, double &s_v) {
-    const float *q = c + kv * nu3 + ku;
+    const TC *q = c + kv * nu3 + ku;
     double s = 0.0;
     s_u = s_v = 0.0;
 #pragma unroll
@@ -57,7 +59,7 @@ __device__ __forceinline__ double xy_value_grad(const float *c, int nu3, int ku,
 }
 
 // L_i / gL_i and its gradient with respect to (x, y, z), FP64, any parameterisation
-static __device__ double lrf_value_grad(const ModelDev &m, const float *cxy_s, const float4 sn, const float4 xf, int tab,
+static __device__ double lrf_value_grad(const ModelDev &m, const float *cxy_s, const double *cxyd_s, const float4 sn, const float4 xf, int tab,
                                  double x, double y, double z, double grad[3]) {
     const double dx = x - (double)sn.x, dy = y - (double)sn.y;
     double s = 0.0, gx = 0.0, gy = 0.0, gz = 0.0;
@@ -109,8 +111,8 @@ static __device__ double lrf_value_grad(const ModelDev &m, const float *cxy_s, c
         const double u = T0 * dx + T1 * dy, v = T2 * dx + T3 * dy;
         int ku, kv;
         double fu, fv, bu[4], bv[4], du[4], dv[4];
-        locate<double>(u, (double)m.u_lo, (double)m.su, m.nx, ku, fu);
-        locate<double>(v, (double)m.v_lo, (double)m.sv, m.ny, kv, fv);
+        locate(u, (double)m.u_lo, (double)m.su, m.nx, ku, fu);
+        locate(v, (double)m.v_lo, (double)m.sv, m.ny, kv, fv);
         basis4<double>(fu, bu);
         basis4<double>(fv, bv);
         dbasis4<double>(fu, du);
@@ -126,16 +128,22 @@ static __device__ double lrf_value_grad(const ModelDev &m, const float *cxy_s, c
             const double zc = fmin(fmax(z, z_lo), z_hi);
             const int pz = min(max((int)floor((zc - z_lo) / dzp), 0), m.n_planes - 2);
             const double w = (zc - (z_lo + (double)pz * dzp)) / dzp;
-            const float *c0 = cxy_s + ((size_t)tab * m.n_planes + pz) * per_plane;
-            double su0, sv0, su1, sv1;
-            const double s0 = xy_value_grad(c0, nu3, ku, kv, bu, bv, du, dv, su0, sv0);
-            const double s1 = xy_value_grad(c0 + per_plane, nu3, ku, kv, bu, bv, du, dv, su1, sv1);
+            const size_t off = ((size_t)tab * m.n_planes + pz) * per_plane;
+            double su0, sv0, su1, sv1, s0, s1;
+            if (cxyd_s) {
+                s0 = xy_value_grad(cxyd_s + off, nu3, ku, kv, bu, bv, du, dv, su0, sv0);
+                s1 = xy_value_grad(cxyd_s + off + per_plane, nu3, ku, kv, bu, bv, du, dv, su1, sv1);
+            } else {
+                s0 = xy_value_grad(cxy_s + off, nu3, ku, kv, bu, bv, du, dv, su0, sv0);
+                s1 = xy_value_grad(cxy_s + off + per_plane, nu3, ku, kv, bu, bv, du, dv, su1, sv1);
+            }
             val = (1.0 - w) * s0 + w * s1;
             su = (1.0 - w) * su0 + w * su1;
             sv = (1.0 - w) * sv0 + w * sv1;
             gz += (z >= z_lo && z <= z_hi) ? (s1 - s0) / dzp : 0.0;
         } else {
-            val = xy_value_grad(cxy_s + (size_t)tab * per_plane, nu3, ku, kv, bu, bv, du, dv, su, sv);
+            val = cxyd_s ? xy_value_grad(cxyd_s + (size_t)tab * per_plane, nu3, ku, kv, bu, bv, du, dv, su, sv)
+                         : xy_value_grad(cxy_s + (size_t)tab * per_plane, nu3, ku, kv, bu, bv, du, dv, su, sv);
         }
         su *= ku_in;
         sv *= kv_in;
@@ -191,9 +199,14 @@ __global__ void __launch_bounds__(256, 2) refine_kernel(const RefineParams rp) {
         grp_s[i] = m.grp[i];
         xf_s[i] = m.xf ? m.xf[i] : make_float4(1.f, 0.f, 0.f, 1.f);
     }
-    for (int i = threadIdx.x; i < ncxy; i += blockDim.x) cxy_s[i] = m.cxy[i];
+    double *cxyd_s = rp.dtab ? reinterpret_cast<double *>(reinterpret_cast<unsigned char *>(cxy_s) + ((size_t)ncxy * 4 + 15) / 16 * 16)
+                             : nullptr;
+    for (int i = threadIdx.x; i < ncxy; i += blockDim.x) {
+        cxy_s[i] = m.cxy[i];
+        if (cxyd_s) cxyd_s[i] = (double)m.cxy[i];
+    }
     __syncthreads();
-    unsigned char *wbase = smem + cta_smem_bytes_gen(N, 0, ncxy) + (size_t)warp * ((size_t)N * 40 + 8);
+    unsigned char *wbase = smem + cta_smem_bytes_gen(N, 0, ncxy, rp.dtab) + (size_t)warp * ((size_t)N * 40 + 8);
     double *LG = reinterpret_cast<double *>(wbase);                       // [N][4] {L, dL/dx, dL/dy, dL/dz}
     float2 *SC = reinterpret_cast<float2 *>(LG + (size_t)4 * N);          // [N] prepared signals
 
@@ -236,7 +249,7 @@ __global__ void __launch_bounds__(256, 2) refine_kernel(const RefineParams rp) {
                 const float4 sn = sens_s[i];
                 double gr[3];
                 const double gL = (double)sn.z;
-                const double L = gL * lrf_value_grad(m, cxy_s, sn, xf_s[i], grp_s[i], p[0], p[1], p[2], gr);
+                const double L = gL * lrf_value_grad(m, cxy_s, cxyd_s, sn, xf_s[i], grp_s[i], p[0], p[1], p[2], gr);
                 gr[0] *= gL;
                 gr[1] *= gL;
                 gr[2] = dim == 3 ? gr[2] * gL : 0.0;

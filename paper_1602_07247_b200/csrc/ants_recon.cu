@@ -42,6 +42,7 @@ struct Plan {
     int k_diff = 0;          // first differential iteration (K = never)
     int k_series = 0;        // axial+z Poisson: first iteration with the log1p series
     int gen_dtab = 0;        // general kernel: double copy of the XY coefficients in shared memory
+    int reuse = 0;           // packed 2-D kernel: the node-reuse instantiation
     const void *kernel = nullptr;
     bool ready = false;      // cudaFuncSetAttribute + occupancy done (needs the device)
 };
@@ -648,7 +649,7 @@ extern "C" int64_t ants_launch_count(void) { return g_launches.load(); }
 // ---------------------------------------------------------------------------
 // kernel look-ups: the instantiations live in k2d_pk_m*.cu, k2d_gen_m*.cu, k3d_m*.cu (kernels.h)
 namespace ants {
-const void *kernel_2d_pk_m0(int), *kernel_2d_pk_m1(int), *kernel_2d_pk_m2(int);
+const void *kernel_2d_pk_m0(int, int), *kernel_2d_pk_m1(int, int), *kernel_2d_pk_m2(int, int);
 const void *kernel_gen_m0(int), *kernel_gen_m1(int), *kernel_gen_m2(int);
 const void *kernel_3d_m0(int, int), *kernel_3d_m1(int, int);
 const void *kernel_refine(int);
@@ -656,8 +657,9 @@ const void *kernel_3d_pk_m0(int, int), *kernel_3d_pk_m1(int, int);
 const void *kernel_3d_pk(int method, int cpl, int gzp) {
     return method == 0 ? kernel_3d_pk_m0(cpl, gzp) : method == 1 ? kernel_3d_pk_m1(cpl, gzp) : nullptr;
 }
-const void *kernel_2d_pk(int method, int npt) {
-    return method == 0 ? kernel_2d_pk_m0(npt) : method == 1 ? kernel_2d_pk_m1(npt) : method == 2 ? kernel_2d_pk_m2(npt) : nullptr;
+const void *kernel_2d_pk(int method, int npt, int reuse) {
+    return method == 0 ? kernel_2d_pk_m0(npt, reuse) : method == 1 ? kernel_2d_pk_m1(npt, reuse)
+         : method == 2 ? kernel_2d_pk_m2(npt, reuse) : nullptr;
 }
 const void *kernel_gen(int method, int lrf_kind) {
     return method == 0 ? kernel_gen_m0(lrf_kind) : method == 1 ? kernel_gen_m1(lrf_kind) : method == 2 ? kernel_gen_m2(lrf_kind) : nullptr;
@@ -676,6 +678,8 @@ static int env_knob(const char *name) {
     return e ? std::atoi(e) : 0;
 }
 static int knob_warps_per_cta() { static const int v = env_knob("ANTS_WARPS_PER_CTA"); return v; }
+static int env_knob_force_reuse() { static const int v = env_knob("ANTS_FORCE_NODE_REUSE"); return v; }
+static int knob_no_reuse() { static const int v = env_knob("ANTS_NO_NODE_REUSE"); return v; }
 static int knob_max_ctas_per_sm() { static const int v = env_knob("ANTS_MAX_CTAS_PER_SM"); return v; }
 
 static int validate_grid(const ants_lrf *h, const ants_grid_params_t *g, int32_t method) {
@@ -831,11 +835,14 @@ static int make_plan(const ants_lrf *h, const ants_grid_params_t *g, int32_t met
     if (!pl.npt) return ANTS_ERR_UNSUPPORTED;
     // strictly positive axial LRFs (the normal case): the sensor-pair-packed kernel
     pl.family = 0;
-    pl.kernel = kernel_2d_pk(method, pl.npt);
+    // node reuse (recon2d_pk_kernel.cuh): contraction 1/2, odd G, and an array large enough for it to pay
+    pl.reuse = g->factor == 0.5f && (g->nodes_per_axis & 1) && m.N >= 96 && !knob_no_reuse() ? 1 : 0;
+    if (env_knob_force_reuse()) pl.reuse = g->factor == 0.5f && (g->nodes_per_axis & 1) ? 1 : 0;
+    pl.kernel = kernel_2d_pk(method, pl.npt, pl.reuse);
     if (!pl.kernel) return ANTS_ERR_UNSUPPORTED;
     first_diff_iter(h, g, method, pl.k_diff, pl.k_series);
     const size_t tables = (cta_smem_bytes_pk(m.N, m.n_lrf * (m.n_r + 1)) + 15) / 16 * 16;
-    const size_t per_warp = warp_smem_bytes_pk(m.N, method);
+    const size_t per_warp = warp_smem_bytes_pk(m.N, method, (int)nodes);
     pick_cta_shape(tables, per_warp, pl);
     if (pl.smem > 227 * 1024) return ANTS_ERR_UNSUPPORTED;
     return ANTS_OK;
@@ -885,7 +892,7 @@ static int get_plan(const ants_lrf *hc, const ants_grid_params_t *g, int32_t met
 }
 
 static void kernel_name(const Plan &pl, int32_t method, int lrf_kind, char *buf, size_t n) {
-    if (pl.family == 0) std::snprintf(buf, n, "ants::recon2d_pk_kernel<%d,%d>", pl.npt, (int)method);
+    if (pl.family == 0) std::snprintf(buf, n, "ants::recon2d_pk_kernel<%d,%d,%s>", pl.npt, (int)method, pl.reuse ? "true" : "false");
     else if (pl.family == 3) std::snprintf(buf, n, "ants::recon_gen_kernel<%d,%d>", (int)method, lrf_kind);
     else if (pl.family == 4) std::snprintf(buf, n, "ants::recon3d_pk_kernel<%d,%d,%d>", pl.cpl, pl.gzm, (int)method);
     else std::snprintf(buf, n, "ants::recon3d_kernel<%d,%d,%d>", pl.cpl, pl.gzm, (int)method);
@@ -962,6 +969,7 @@ static int launch(const ants_lrf *h, const float *signals, int64_t n_events, con
     p.warps_per_cta = pl.warps;
     p.tile_events = pl.warps;
     p.gen_dtab = pl.gen_dtab;
+    p.reuse = pl.reuse;
 
     long long want = (n_events + pl.warps - 1) / pl.warps;
     long long cap = (long long)h->sm_count * pl.ctas_per_sm;

@@ -1,16 +1,12 @@
-// k2d_pk_m1.cu -- instantiations of recon2d_pk_kernel<NPT, 1> (one translation unit per method: parallel build)
+// k2d_pk_m1.cu -- instantiations of recon2d_pk_kernel<NPT, 1, REUSE> (one translation unit per method: parallel build)
 #include "recon2d_pk.cuh"
 #include "kernels.h"
 
 namespace ants {
-const void *kernel_2d_pk_m1(int npt) {
-    switch (npt) {
-        case 1: return (const void *)recon2d_pk_kernel<1, 1>;
-        case 2: return (const void *)recon2d_pk_kernel<2, 1>;
-        case 3: return (const void *)recon2d_pk_kernel<3, 1>;
-        case 4: return (const void *)recon2d_pk_kernel<4, 1>;
-        case 8: return (const void *)recon2d_pk_kernel<8, 1>;
-    }
+const void *kernel_2d_pk_m1(int npt, int reuse) {
+#define ANTS_K2(NP) if (npt == NP) return reuse ? (const void *)recon2d_pk_kernel<NP, 1, true> : (const void *)recon2d_pk_kernel<NP, 1, false>
+    ANTS_K2(1); ANTS_K2(2); ANTS_K2(3); ANTS_K2(4); ANTS_K2(8);
+#undef ANTS_K2
     return nullptr;
 }
 }  // namespace ants

@@ -6,7 +6,7 @@
 namespace ants {
 
 // axial LRFs, strictly positive: sensor-pair-packed kernel (recon2d_pk.cuh).  method 0/1/2, npt in {1,2,3,4,8}
-const void *kernel_2d_pk(int method, int npt);
+const void *kernel_2d_pk(int method, int npt, int reuse);
 // axial+z LRFs searched in 3-D, packed over pairs of z-levels (recon3d_pk.cuh).  method 0/1,
 // (cpl, gzp) in {(1,2),(2,2),(1,4),(2,4)}
 const void *kernel_3d_pk(int method, int cpl, int gzp);

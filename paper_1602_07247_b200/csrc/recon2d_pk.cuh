@@ -22,23 +22,30 @@ constexpr int kPkArrays = 10;   // D0..D7, E0, E1 (float4 [Np + 1] each)
 struct WarpSmemPk {
     float4 *D[kPkArrays];   // per-pair records of the current iteration (plain mode uses D[0] only)
     float2 *SC;             // [N] {S_i (prepared), log2(S_i / g_i) or 0}
+    float *S0, *S1;         // [nodes] node scores of the previous and of the current iteration (node reuse)
+    unsigned char *L;       // [nodes] the nodes that have to be evaluated in this iteration, compacted
 };
 
 __host__ __device__ inline int pk_pairs(int N) { return (N + 1) / 2 + 1; }   // +1: a pad on each list
-__host__ __device__ inline size_t warp_smem_bytes_pk(int N, int method) {
+__host__ __device__ inline size_t warp_smem_bytes_pk(int N, int method, int nodes) {
     const int narr = method == 0 ? 8 : kPkArrays;
-    return ((size_t)pk_pairs(N) * 16 * narr + (size_t)N * 8 + 15) / 16 * 16;
+    const size_t np4 = ((size_t)nodes + 3) / 4 * 4;
+    return ((size_t)pk_pairs(N) * 16 * narr + ((size_t)N * 8 + 15) / 16 * 16 + np4 * 9 + 15) / 16 * 16;
 }
 // CTA-shared: sens_s [N] float4, poly_s [rows] float4, grp_s [N] int, node_s [256] float2 (grid offsets of the
 // nodes in units of the step: a table look-up instead of an integer division wherever a lane needs its nodes)
 __host__ __device__ inline size_t cta_smem_bytes_pk(int N, int rows) { return cta_table_bytes(N, rows) + 256 * 8; }
 
-__device__ __forceinline__ WarpSmemPk carve_pk(unsigned char *base, int N, int method) {
+__device__ __forceinline__ WarpSmemPk carve_pk(unsigned char *base, int N, int method, int nodes) {
     WarpSmemPk w;
     const int np1 = pk_pairs(N), narr = method == 0 ? 8 : kPkArrays;
     float4 *f = reinterpret_cast<float4 *>(base);
     for (int a = 0; a < kPkArrays; ++a) w.D[a] = f + (size_t)(a < narr ? a : 0) * np1;
     w.SC = reinterpret_cast<float2 *>(f + (size_t)narr * np1);
+    const size_t np4 = ((size_t)nodes + 3) / 4 * 4;
+    w.S0 = reinterpret_cast<float *>(reinterpret_cast<unsigned char *>(w.SC) + ((size_t)N * 8 + 15) / 16 * 16);
+    w.S1 = w.S0 + np4;
+    w.L = reinterpret_cast<unsigned char *>(w.S1 + np4);
     return w;
 }
 

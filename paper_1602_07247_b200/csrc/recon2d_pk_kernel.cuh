@@ -4,7 +4,10 @@
 namespace ants {
 
 // METHOD 0 Poisson ML, 1 weighted chi-square.  Requires every LRF strictly positive (host-checked).
-template <int NPT, int METHOD>
+// REUSE: carry the scores of coinciding nodes over from the previous grid (see below); the host picks it for large
+// arrays, where it pays (config 5: +7 %); the kernel is latency-bound, and with a round of nodes less per lane the
+// smaller arrays lose more instruction-level parallelism than they save work (config 3: -13 %).
+template <int NPT, int METHOD, bool REUSE>
 __global__ void __launch_bounds__(256, (NPT <= 3 ? 3 : 2)) recon2d_pk_kernel(const Params p) {
     extern __shared__ __align__(16) unsigned char smem[];
     const ModelDev &m = p.m;
@@ -28,7 +31,7 @@ __global__ void __launch_bounds__(256, (NPT <= 3 ? 3 : 2)) recon2d_pk_kernel(con
     }
     __syncthreads();
     WarpSmemPk w = carve_pk(smem + (cta_smem_bytes_pk(N, rows) + 15) / 16 * 16 +
-                            (size_t)warp * warp_smem_bytes_pk(N, METHOD), N, METHOD);
+                            (size_t)warp * warp_smem_bytes_pk(N, METHOD, p.nodes), N, METHOD, p.nodes);
     const int np1 = pk_pairs(N);
     const unsigned poly_base = (unsigned)__cvta_generic_to_shared(poly_s) - ((unsigned)kMagicBits << 4);
 
@@ -73,32 +76,94 @@ __global__ void __launch_bounds__(256, (NPT <= 3 ? 3 : 2)) recon2d_pk_kernel(con
             A_ref = sl > 0.f ? sumS * rcp_approx(sl) : 1.f;   // only conditions the plain score
         }
 
+        // Node reuse.  With a contraction of 1/2 and an odd G the nodes of the new grid that sit an even number of
+        // steps from its centre coincide with nodes of the previous grid (25 of 81, 25 of 121): their scores are
+        // carried over -- a plain score as it is, a differential one minus the new centre's -- and only the other
+        // nodes are evaluated, compacted onto the lanes (9 x 9: two rounds of 32 instead of three).  Not across the
+        // switch from the plain to the differential score, nor after an iteration without a valid node.
+        const bool reuse_ok = REUSE && p.factor == 0.5f && (p.G & 1);
+        float *sc_prev = w.S0, *sc_cur = w.S1;
+        bool have_prev = false;
+        int prev_bi = 0, prev_mode = -1;
+        const unsigned lt = (1u << lane) - 1u;
+
         float h = p.h0_xy;
         for (int k = 0; k < p.K; ++k) {
-            float sc_node[NPT];          // node scores (lower is better), +inf = invalid
+            const int mode = k < p.k_diff ? 0 : 1;
+            // ---- the nodes of this iteration: carried over or to be evaluated ----
+            int count = REUSE ? 0 : p.nodes;
+            if (REUSE) {
+                const bool reuse = reuse_ok && have_prev && mode == prev_mode;
+                const int by = prev_bi / p.G, bx = prev_bi - by * p.G;
+                const float off = (reuse && mode == 1) ? sc_prev[prev_bi] : 0.f;
+#pragma unroll
+                for (int j = 0; j < NPT; ++j) {
+                    const int n = lane + 32 * j;
+                    bool todo = n < p.nodes;
+                    if (reuse && todo) {
+                        const float2 no = node_s[n];
+                        const int dxn = (int)no.x, dyn = (int)no.y;          // steps from the centre (G odd: integers)
+                        const int ox = bx + (dxn >> 1), oy = by + (dyn >> 1);
+                        if (!((dxn | dyn) & 1) && (unsigned)ox < (unsigned)p.G && (unsigned)oy < (unsigned)p.G) {
+                            sc_cur[n] = sc_prev[oy * p.G + ox] - off;
+                            todo = false;
+                        }
+                    }
+                    const unsigned mk = __ballot_sync(kFull, todo);
+                    if (todo) w.L[count + __popc(mk & lt)] = (unsigned char)n;
+                    count += __popc(mk);
+                }
+                __syncwarp();
+            }
+            int nid[NPT];
+#pragma unroll
+            for (int j = 0; j < NPT; ++j)
+                nid[j] = !REUSE ? lane + 32 * j : lane + 32 * j < count ? (int)w.L[lane + 32 * j] : 0;
+
+            float sc_node[NPT];          // scores of this lane's nodes (lower is better), +inf = invalid
             float aux_node[NPT];         // plain mode: sum L (Poisson) / A (chi2) at the node
-            if (k < p.k_diff) {
+            // (the sensor-pair loops inside are compiled for NPT and for NPT - 1 nodes per lane, statically unrolled:
+            // the shorter ones serve when the carried-over nodes free a whole round of 32 lanes)
+            const bool short_round = REUSE && NPT > 1 && count <= 32 * (NPT - 1);
+            if (mode == 0) {
 #include "recon2d_pk_plain.inc"
             } else {
 #include "recon2d_pk_diff.inc"
             }
+            if (REUSE) {
+#pragma unroll
+                for (int j = 0; j < NPT; ++j)
+                    if (lane + 32 * j < count) sc_cur[nid[j]] = sc_node[j];
+                __syncwarp();
+            }
 
-            // ---- a5: argmin over the G^2 nodes, recentre, contract ----
+            // ---- a5: argmin over the G^2 nodes in their natural order (R9), recentre, contract ----
             float bs = kInf;
             int bi = 0x7fffffff;
 #pragma unroll
-            for (int j = 0; j < NPT; ++j)
-                if (sc_node[j] < bs) { bs = sc_node[j]; bi = lane + 32 * j; }
+            for (int j = 0; j < NPT; ++j) {
+                const int n = lane + 32 * j;
+                const float sv = !REUSE ? sc_node[j] : n < p.nodes ? sc_cur[n] : kInf;
+                if (sv < bs) { bs = sv; bi = n; }
+            }
             warp_argmin_redux(bs, bi);
             const bool found = bs < kInf;
             if (found) {
-                if (k < p.k_diff) {
+                if (mode == 0 && !REUSE) {
+                    // (with node reuse the reference energy stays at its seed value: the plain score's rounding
+                    // error depends on it, alike for all nodes of one grid but not from one grid to the next, and
+                    // carried-over scores are compared with fresh ones)
+                    // the winner's energy, if it was evaluated in this iteration, lives in the lane that scored it
                     float mine = 0.f;
+                    bool has = false;
 #pragma unroll
                     for (int j = 0; j < NPT; ++j)
-                        if ((bi >> 5) == j) mine = aux_node[j];
-                    float v = __shfl_sync(kFull, mine, bi & 31);
-                    A_ref = METHOD == 0 ? sumS * rcp_approx(v) : v;
+                        if (lane + 32 * j < count && nid[j] == bi) { mine = aux_node[j]; has = true; }
+                    const unsigned who = __ballot_sync(kFull, has);
+                    if (who) {
+                        const float v = __shfl_sync(kFull, mine, __ffs(who) - 1);
+                        A_ref = METHOD == 0 ? sumS * rcp_approx(v) : v;
+                    }
                 }
                 const float2 wo = node_s[bi];           // the winner's grid offsets (one broadcast load)
                 cx = fmaf(wo.x, h, cx);
@@ -106,6 +171,12 @@ __global__ void __launch_bounds__(256, (NPT <= 3 ? 3 : 2)) recon2d_pk_kernel(con
             }
             if (p.out_path && lane == 0) p.out_path[e * p.K + k] = found ? (uint16_t)bi : (uint16_t)0xFFFF;
             h *= p.factor;
+            have_prev = found;
+            prev_bi = found ? bi : 0;
+            prev_mode = mode;
+            float *tmp = sc_prev;
+            sc_prev = sc_cur;
+            sc_cur = tmp;
             __syncwarp();
         }
 

@@ -64,6 +64,7 @@ struct Params {
     int warps_per_cta;
     int tile_events;        // events staged per CTA tile (= warps_per_cta)
     int gen_dtab;           // general kernel: a double copy of the XY coefficients sits in shared memory
+    int reuse;              // packed 2-D kernel: carry coinciding nodes' scores over from the previous grid
 };
 
 __device__ __forceinline__ float sqrt_approx(float x) {

@@ -1,4 +1,4 @@
-"""CPU ORACLE of the axial LRF calculation (TEST INFRASTRUCTURE, NOT THE PRODUCT).
+"""CPU ORACLE of the LRF calculation (TEST INFRASTRUCTURE, NOT THE PRODUCT).
 
 PAPER.md:380 (section 6): "The LRF module calculates these functions from datasets containing
 photosensor signals and the corresponding event positions"; the LRFs are B-splines of the
@@ -299,4 +299,67 @@ def fit_xy(sensor_xy, gains, knots_xy, n_lrf, n_int_x, n_int_y, signals, xyzA, g
                 np.add.at(M[m], (j1, j2), w1 * w2)
         used[m] += use.sum()
     c = np.stack([np.linalg.solve(M[m], b[m]).reshape(ncv, ncu) for m in range(n_lrf)])
+    return c, used
+
+
+def fit_sliced(sensor_xy, gains, knots_xy, n_lrf, n_int_x, n_int_y, n_planes, signals, xyzA, group=None, xform=None):
+    """LRF calculation for Sliced tables ("a set of several XY LRFs, each defined on a specific Z
+    plane.  The LRF values for the points between the planes are calculated using linear interpolation of the LRF
+    values at two closest points from two closest planes"; PAPER.md:380 LRFs are calculated from signals and
+    positions).  The paper does not say how the planes' tables are obtained; reading R36 = R21-R23 and R35 carried
+    through the evaluation rule R32, all planes of a table fitted JOINTLY: unweighted least squares of
+        y = S / (A g_i)   against   (1 - w) s_p(u, v) + w s_{p+1}(u, v),
+    s_p the tensor-product spline of plane p, p = min(floor((z - z_lo)/dz), n_planes - 2), w = (z - z_p)/dz,
+    dz = (z_hi - z_lo)/(n_planes - 1) -- exactly the value oracle_lrf returns for the pair -- over events with
+    finite x, y, z, A, A > 0 and z_lo <= z <= z_hi (no extrapolation data, as in R25) and pairs with (u, v) inside the
+    tabulated ranges; table t = group[i], or 0 / i without a grouping; g_i = 1 for per-sensor tables.
+    knots_xy = {u_lo, u_hi, v_lo, v_hi, z_lo, z_hi}.
+    -> coefficients [n_lrf][n_planes][n_int_y + 3][n_int_x + 3] (float64), pairs used [n_lrf].
+    Raises numpy.linalg.LinAlgError when a table is underdetermined."""
+    xy = np.asarray(sensor_xy, np.float32).astype(np.float64).reshape(-1, 2)
+    N = xy.shape[0]
+    g = np.ones(N) if gains is None else np.asarray(gains, np.float32).astype(np.float64)
+    u_lo, u_hi, v_lo, v_hi, z_lo, z_hi = (float(np.float32(k)) for k in knots_xy[:6])
+    hu, hv = (u_hi - u_lo) / n_int_x, (v_hi - v_lo) / n_int_y
+    dz = (z_hi - z_lo) / (n_planes - 1)
+    ncu, ncv = n_int_x + 3, n_int_y + 3
+    per_plane = ncu * ncv
+    n_unknown = n_planes * per_plane
+    S = np.asarray(signals, np.float32).astype(np.float64).reshape(-1, N)
+    P = np.asarray(xyzA, np.float32).astype(np.float64).reshape(-1, 4)
+    T = None if xform is None else np.asarray(xform, np.float32).astype(np.float64).reshape(N, 4)
+    with np.errstate(invalid="ignore"):
+        ok = np.isfinite(P).all(axis=1) & (P[:, 3] > 0.0) & (P[:, 2] >= z_lo) & (P[:, 2] <= z_hi)
+    M = np.zeros((n_lrf, n_unknown, n_unknown))
+    b = np.zeros((n_lrf, n_unknown))
+    used = np.zeros(n_lrf)
+    for i in range(N):
+        if group is not None:
+            m, gi = int(group[i]), g[i]
+        else:
+            m = 0 if n_lrf == 1 else i
+            gi = g[i] if n_lrf == 1 else 1.0
+        with np.errstate(invalid="ignore"):
+            dx, dy = P[:, 0] - xy[i, 0], P[:, 1] - xy[i, 1]
+            u, v = (dx, dy) if T is None else (T[i, 0] * dx + T[i, 1] * dy, T[i, 2] * dx + T[i, 3] * dy)
+            use = ok & (u >= u_lo) & (u <= u_hi) & (v >= v_lo) & (v <= v_hi)
+        y = S[use, i] / (P[use, 3] * gi)
+        z = P[use, 2]
+        p = np.clip(np.floor((z - z_lo) / dz).astype(np.int64), 0, n_planes - 2)
+        w = (z - (z_lo + p * dz)) / dz
+        tu, tv = (u[use] - u_lo) / hu, (v[use] - v_lo) / hv
+        ku = np.minimum(np.floor(tu).astype(np.int64), n_int_x - 1)
+        kv = np.minimum(np.floor(tv).astype(np.int64), n_int_y - 1)
+        Bu, Bv = basis4(tu - ku), basis4(tv - kv)
+        idx = []
+        for side, wz in ((0, 1.0 - w), (1, w)):
+            for bb in range(4):
+                for aa in range(4):
+                    idx.append(((p + side) * per_plane + (kv + bb) * ncu + ku + aa, wz * Bv[:, bb] * Bu[:, aa]))
+        for j1, w1 in idx:
+            np.add.at(b[m], j1, w1 * y)
+            for j2, w2 in idx:
+                np.add.at(M[m], (j1, j2), w1 * w2)
+        used[m] += use.sum()
+    c = np.stack([np.linalg.solve(M[m], b[m]).reshape(n_planes, ncv, ncu) for m in range(n_lrf)])
     return c, used

@@ -325,3 +325,88 @@ def test_xy_fit_is_the_lstsq_of_the_tensor_design_matrix():
             ref, *_ = np.linalg.lstsq(np.vstack(rows), np.concatenate(ys), rcond=None)
             assert np.abs(c[m].ravel() - ref).max() <= 1e-7 * max(1.0, np.abs(ref).max()), kw.keys()
             assert used[m] == sum(len(y) for y in ys)
+
+
+def _sliced_problem(n_events, seed=0, noise=0.5):
+    """The XY problem of _xy_problem with a depth: z uniform over (and a little beyond) the planes' range, a response
+    that widens with z."""
+    rng = np.random.default_rng(seed + 50)
+    xy = synth.square_array(3, 8.0)
+    N = len(xy)
+    gains = rng.uniform(0.8, 1.2, N).astype(np.float32)
+    pos = np.zeros((n_events, 4), np.float32)
+    pos[:, :2] = rng.uniform(-22.0, 22.0, (n_events, 2))
+    pos[:, 2] = rng.uniform(-1.0, 13.0, n_events)
+    pos[:, 3] = rng.uniform(200.0, 400.0, n_events)
+    dx = pos[:, None, 0].astype(np.float64) - xy[None, :, 0]
+    dy = pos[:, None, 1].astype(np.float64) - xy[None, :, 1]
+    wd = 60.0 + 4.0 * pos[:, None, 2].astype(np.float64)
+    resp = np.exp(-(dx * dx + dy * dy * 0.7) / wd) * (1.0 + 0.02 * dx)
+    sig = (pos[:, 3:4].astype(np.float64) * gains[None, :] * resp + rng.normal(0, noise, (n_events, N))).astype(np.float32)
+    return xy, gains, sig, pos
+
+
+def test_sliced_fit_is_the_lstsq_of_the_interpolated_design_matrix():
+    """R36 pinned against scipy design matrices, the interpolation weights of PAPER.md:396 written out here, and
+    numpy.linalg.lstsq over all planes at once: a shared table with gains, and symmetry groups with frames."""
+    xy, gains, sig, pos = _sliced_problem(2500)
+    knots = np.array([-12, 12, -12, 12, 0, 12], np.float32)
+    nx, ny, n_planes = 4, 3, 4
+    tu, tv = synth.uniform_knot_vector(-12.0, 12.0, nx), synth.uniform_knot_vector(-12.0, 12.0, ny)
+    per_plane = (nx + 3) * (ny + 3)
+    group, xform, n_groups = fit.group_by_symmetry(xy, 4, True)
+    z = pos[:, 2].astype(float)
+    inside = (z >= 0.0) & (z <= 12.0)
+    assert 0 < (~inside).sum() < len(z)                       # some events lie outside the planes and are left out
+    plane_z = np.linspace(0.0, 12.0, n_planes)
+    for kw in (dict(n_lrf=1), dict(n_lrf=n_groups, group=group, xform=xform)):
+        c, used = fit.fit_sliced(xy, gains, knots, kw["n_lrf"], nx, ny, n_planes, sig, pos, group=kw.get("group"),
+                                 xform=kw.get("xform"))
+        assert c.shape == (kw["n_lrf"], n_planes, ny + 3, nx + 3)
+        for m in range(kw["n_lrf"]):
+            rows, ys = [], []
+            for i in range(len(xy)):
+                if kw.get("group") is not None and group[i] != m:
+                    continue
+                dx = pos[:, 0].astype(float) - float(xy[i, 0])
+                dy = pos[:, 1].astype(float) - float(xy[i, 1])
+                T = np.eye(2) if kw.get("xform") is None else xform[i].astype(float).reshape(2, 2)
+                u, v = T[0, 0] * dx + T[0, 1] * dy, T[1, 0] * dx + T[1, 1] * dy
+                use = inside & (u >= -12) & (u <= 12) & (v >= -12) & (v <= 12)
+                Bu = BSpline.design_matrix(u[use], tu, 3).toarray()
+                Bv = BSpline.design_matrix(v[use], tv, 3).toarray()
+                B = np.einsum("kb,ka->kba", Bv, Bu).reshape(use.sum(), -1)
+                # hat functions of the planes: the linear interpolation between the two closest planes
+                hat = np.maximum(0.0, 1.0 - np.abs(z[use, None] - plane_z[None, :]) / (plane_z[1] - plane_z[0]))
+                assert np.allclose(hat.sum(axis=1), 1.0)
+                rows.append(np.einsum("kp,kj->kpj", hat, B).reshape(use.sum(), n_planes * per_plane))
+                ys.append(sig[use, i].astype(float) / (pos[use, 3].astype(float) * float(gains[i])))
+            ref, *_ = np.linalg.lstsq(np.vstack(rows), np.concatenate(ys), rcond=None)
+            assert np.abs(c[m].ravel() - ref).max() <= 1e-6 * max(1.0, np.abs(ref).max()), kw.keys()
+            assert used[m] == sum(len(y) for y in ys)
+
+
+def test_sliced_fit_recovers_the_tables_the_oracle_evaluates():
+    """Noise-free signals generated with oracle_lrf (R32) from known Sliced tables: the joint fit returns those tables,
+    which ties R36 to the evaluation rule of the reconstruction oracle (a per-plane binning of the events would not)."""
+    from oracle import oracle
+    rng = np.random.default_rng(5)
+    xy = synth.square_array(3, 8.0)
+    N = len(xy)
+    nx, ny, n_planes = 3, 3, 3
+    knots = np.array([-29, 29, -29, 29, 2, 10], np.float32)        # events reach u, v = +-28: tables covered to the ends
+    truth = rng.uniform(0.5, 1.5, (1, n_planes, ny + 3, nx + 3)).astype(np.float32)
+    gains = rng.uniform(0.8, 1.2, N).astype(np.float32)
+    m = oracle.Model(xy, gains, None, None, 1, 5, 0, 0, n_int_x=nx, n_int_y=ny, n_planes=n_planes, knots_xy=knots,
+                     coeffs_xy=truth)
+    n_events = 600
+    pos = np.zeros((n_events, 4), np.float32)
+    pos[:, :2] = rng.uniform(-20.0, 20.0, (n_events, 2))
+    pos[:, 2] = rng.uniform(2.0, 10.0, n_events)
+    pos[:, 3] = rng.uniform(100.0, 200.0, n_events)
+    sig = np.array([[float(pos[e, 3]) * m.lrf(i, float(pos[e, 0]), float(pos[e, 1]), float(pos[e, 2])) for i in range(N)]
+                    for e in range(n_events)])
+    c, used = fit.fit_sliced(xy, gains, knots, 1, nx, ny, n_planes, sig.astype(np.float32), pos)
+    assert used[0] == n_events * N
+    # float32 signals (6e-8 relative) through a fit whose end coefficients are conditioned ~1e2..1e3: observed 1.5e-5
+    assert np.abs(c - truth).max() <= 1e-4

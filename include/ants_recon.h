@@ -21,7 +21,7 @@
  *
  * Every step runs in hand-written sm_100a CUDA kernels; there is no CPU
  * fallback.  All functions return an ants_status code (0 = OK) and never throw.
- * Points on which the paper is silent follow DESIGN.md "Readings" (R1..R34).
+ * Points on which the paper is silent follow DESIGN.md "Readings" (R1..R36).
  */
 #ifndef ANTS_RECON_H
 #define ANTS_RECON_H
@@ -350,14 +350,37 @@ int ants_lrf_fit_axial_z(const float *sensor_xy, const float *gains, const float
  *   signals DEVICE [n_events][N]; xyzA DEVICE [n_events][4];
  *   coeffs_out HOST [n_lrf][n_int_y + 3][n_int_x + 3] float; n_used_out HOST [n_lrf] double or NULL.
  * One kernel launch (FP64 normal equations) and one dense Cholesky solve on the host per table; returns after the
- * result is in host memory.  The result goes straight into ants_lrf_create_xy.  Sliced tables are not fitted by
- * this library.  Errors: ANTS_ERR_INVALID, ANTS_ERR_SINGULAR (a cell of some table received no data),
+ * result is in host memory.  The result goes straight into ants_lrf_create_xy.  Sliced tables: ants_lrf_fit_sliced.
+ * Errors: ANTS_ERR_INVALID, ANTS_ERR_SINGULAR (a cell of some table received no data),
  * ANTS_ERR_UNSUPPORTED ((n_int_x + 3)(n_int_y + 3) > 768), ANTS_ERR_CUDA, ANTS_ERR_NOMEM.
  */
 int ants_lrf_fit_xy(const float *sensor_xy, const float *gains, const int32_t *group, const float *xform,
                     const float *knots_xy, int32_t n_sensors, int32_t n_lrf, int32_t n_int_x, int32_t n_int_y,
                     const float *knots_ax, const float *coeffs_ax, int32_t n_int_r, const float *signals,
                     const float *xyzA, int64_t n_events, float *coeffs_out, double *n_used_out, void *cuda_stream);
+
+/*
+ * ants_lrf_fit_sliced -- LRF calculation for Sliced tables ("a set of several XY LRFs, each defined on
+ * a specific Z plane.  The LRF values for the points between the planes are calculated using linear interpolation of
+ * the LRF values at two closest points from two closest planes").  The paper does not say how the
+ * planes' tables are obtained; reading R36: ALL planes of a table are fitted jointly, unweighted least squares of
+ * y = S / (A g_i) against (1 - w) s_p(u, v) + w s_{p+1}(u, v) -- the value the reconstruction evaluates for the pair,
+ * p = min(floor((z - z_lo)/dz), n_planes - 2), w = (z - z_p)/dz, dz = (z_hi - z_lo)/(n_planes - 1); an event takes
+ * part if x, y, z, A are finite, A > 0 and z_lo <= z <= z_hi, a pair if u and v lie inside the tabulated ranges.
+ *   sensor_xy HOST [N][2]; gains HOST [N] or NULL; group HOST [N] int32 or NULL (n_lrf = 1 or N then); xform HOST
+ *   [N][4] or NULL; knots_xy HOST {u_lo, u_hi, v_lo, v_hi, z_lo, z_hi}; signals DEVICE [n_events][N];
+ *   xyzA DEVICE [n_events][4];
+ *   coeffs_out HOST [n_lrf][n_planes][n_int_y + 3][n_int_x + 3] float; n_used_out HOST [n_lrf] double or NULL.
+ * Per table 3 (n_planes - 1) kernel launches (FP64 normal equations: per slab the blocks plane-plane, next-next and
+ * plane-next of the block-tridiagonal matrix) and one banded Cholesky solve on the host; returns after the result is
+ * in host memory.  The result goes straight into ants_lrf_create_xy (lrf_dim 5).  Errors: ANTS_ERR_INVALID,
+ * ANTS_ERR_SINGULAR (some coefficient received no data), ANTS_ERR_UNSUPPORTED ((n_int_x + 3)(n_int_y + 3) > 768 or
+ * more than 8192 unknowns per table), ANTS_ERR_CUDA, ANTS_ERR_NOMEM.
+ */
+int ants_lrf_fit_sliced(const float *sensor_xy, const float *gains, const int32_t *group, const float *xform,
+                        const float *knots_xy, int32_t n_sensors, int32_t n_lrf, int32_t n_int_x, int32_t n_int_y,
+                        int32_t n_planes, const float *signals, const float *xyzA, int64_t n_events,
+                        float *coeffs_out, double *n_used_out, void *cuda_stream);
 
 /* Event-filter criteria (section 5.2); NaN switches a criterion off. */
 typedef struct {

@@ -1630,7 +1630,7 @@ extern "C" int ants_lrf_fit_xy(const float *sensor_xy, const float *gains, const
             p.signals = signals; p.xyzA = xyzA; p.n_events = n_events; p.N = N; p.nx = nx; p.ny = ny; p.ncu = ncu; p.nc = nc;
             p.u_lo = u_lo; p.u_hi = u_hi; p.hu = (u_hi - u_lo) / nx; p.v_lo = v_lo; p.v_hi = v_hi; p.hv = (v_hi - v_lo) / ny;
             p.axial = composite ? d_ax : nullptr; p.a_n = n_int_r; p.a_lo = a_lo; p.a_hi = a_hi;
-            p.acc = d_acc; p.n_used = d_used;
+            p.acc = d_acc; p.n_used = d_used; p.slab = -1;
             const long long want = (n_events + warps - 1) / warps;
             const int grid = (int)std::min<long long>(want, (long long)sms * occ);
             void *args[] = {&p};
@@ -1661,5 +1661,169 @@ extern "C" int ants_lrf_fit_xy(const float *sensor_xy, const float *gains, const
     }
     if (rc != ANTS_OK) cudaStreamSynchronize(st);
     cleanup();
+    return rc;
+}
+
+// ---------------------------------------------------------------------------
+// LRF calculation for Sliced tables (R36): all planes of a table jointly.  The normal matrix is block tridiagonal in
+// the planes, every block banded like an XY table's; per table 3 (n_planes - 1) launches of lrf_fit_xy_kernel (one
+// per slab and kind of block), one download, one banded Cholesky on the host.
+// ---------------------------------------------------------------------------
+// banded Cholesky solve: lower band storage B [n][bw + 1], B[i][bw - (i - j)] = M[i][j] for i - bw <= j <= i
+static bool solve_banded_spd(std::vector<double> &B, std::vector<double> &b, int n, int bw) {
+    const size_t ld = (size_t)bw + 1;
+    for (int i = 0; i < n; ++i) {
+        double *ri = &B[(size_t)i * ld];
+        const int j0 = std::max(0, i - bw);
+        for (int j = j0; j <= i; ++j) {
+            const double *rj = &B[(size_t)j * ld];
+            const int k0 = std::max(j0, j - bw);
+            double s = ri[bw - (i - j)];
+            const double *a = ri + (bw - (i - k0)), *c = rj + (bw - (j - k0));
+            for (int k = 0; k < j - k0; ++k) s -= a[k] * c[k];
+            if (j < i) {
+                ri[bw - (i - j)] = s / rj[bw];
+            } else {
+                if (!(s > 0.0) || !std::isfinite(s)) return false;
+                ri[bw] = std::sqrt(s);
+            }
+        }
+    }
+    for (int i = 0; i < n; ++i) {
+        const double *ri = &B[(size_t)i * ld];
+        const int j0 = std::max(0, i - bw);
+        double s = b[i];
+        for (int j = j0; j < i; ++j) s -= ri[bw - (i - j)] * b[j];
+        b[i] = s / ri[bw];
+    }
+    for (int i = n - 1; i >= 0; --i) {
+        double s = b[i];
+        const int j1 = std::min(n - 1, i + bw);
+        for (int j = i + 1; j <= j1; ++j) s -= B[(size_t)j * ld + (bw - (j - i))] * b[j];
+        b[i] = s / B[(size_t)i * ld + bw];
+    }
+    return true;
+}
+
+extern "C" int ants_lrf_fit_sliced(const float *sensor_xy, const float *gains, const int32_t *group, const float *xform,
+                                   const float *knots_xy, int32_t N, int32_t n_lrf, int32_t nx, int32_t ny,
+                                   int32_t n_planes, const float *signals, const float *xyzA, int64_t n_events,
+                                   float *coeffs_out, double *n_used_out, void *cuda_stream) {
+    if (!sensor_xy || !knots_xy || !coeffs_out || N < 1 || nx < 1 || ny < 1 || n_planes < 2 || n_events < 0)
+        return ANTS_ERR_INVALID;
+    if (n_events > 0 && (!signals || !xyzA)) return ANTS_ERR_INVALID;
+    if (group) {
+        if (n_lrf < 1 || n_lrf > N) return ANTS_ERR_INVALID;
+        for (int i = 0; i < N; ++i)
+            if (group[i] < 0 || group[i] >= n_lrf) return ANTS_ERR_INVALID;
+    } else if (n_lrf != 1 && n_lrf != N) {
+        return ANTS_ERR_INVALID;
+    }
+    const double u_lo = knots_xy[0], u_hi = knots_xy[1], v_lo = knots_xy[2], v_hi = knots_xy[3];
+    const double z_lo = knots_xy[4], z_hi = knots_xy[5];
+    for (int k = 0; k < 6; ++k)
+        if (!std::isfinite(knots_xy[k])) return ANTS_ERR_INVALID;
+    if (!(u_hi > u_lo) || !(v_hi > v_lo) || !(z_hi > z_lo)) return ANTS_ERR_INVALID;
+    for (int i = 0; i < N; ++i)
+        if (gains && !(gains[i] > 0.f && std::isfinite(gains[i]))) return ANTS_ERR_INVALID;
+    const int ncu = nx + 3, nc = ncu * (ny + 3);
+    const long long n_unknown = (long long)n_planes * nc;
+    if (nc > 768 || n_unknown > 8192) return ANTS_ERR_UNSUPPORTED;
+    const int n = (int)n_unknown, bw = nc + 3 * ncu + 3, n_slabs = n_planes - 1;
+    const size_t block = (size_t)nc * 29, total = block * 3 * n_slabs, smem = block * sizeof(double);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+        cudaGetLastError();
+        return ANTS_ERR_CUDA;
+    }
+    const bool scaled = group != nullptr || n_lrf == 1;
+    std::vector<float> g(N, 1.f);
+    if (gains && scaled) std::copy(gains, gains + N, g.begin());
+    std::lock_guard<std::mutex> arena_lock(g_fit_arena.mu);
+    if (!g_fit_arena.begin((size_t)N * 32 + total * sizeof(double) + 4096)) return ANTS_ERR_NOMEM;
+    float *d_xy = g_fit_arena.take<float>((size_t)N * 2);
+    float *d_g = g_fit_arena.take<float>(N);
+    int *d_mem = g_fit_arena.take<int>(N);
+    double *d_acc = g_fit_arena.take<double>(total);
+    unsigned long long *d_used = g_fit_arena.take<unsigned long long>(1);
+    float *d_xf = xform ? g_fit_arena.take<float>((size_t)N * 4) : nullptr;
+    if (!d_xy || !d_g || !d_mem || !d_acc || !d_used || (xform && !d_xf)) return ANTS_ERR_NOMEM;
+    bool ok = cudaMemcpyAsync(d_xy, sensor_xy, (size_t)N * 2 * sizeof(float), cudaMemcpyHostToDevice, st) == cudaSuccess &&
+              cudaMemcpyAsync(d_g, g.data(), (size_t)N * sizeof(float), cudaMemcpyHostToDevice, st) == cudaSuccess &&
+              (!xform || cudaMemcpyAsync(d_xf, xform, (size_t)N * 4 * sizeof(float), cudaMemcpyHostToDevice, st) == cudaSuccess);
+    const int warps = 8;
+    int occ = 0;
+    ok = ok && cudaFuncSetAttribute((const void *)lrf_fit_xy_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) == cudaSuccess &&
+         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void *)lrf_fit_xy_kernel, warps * 32, smem) == cudaSuccess && occ >= 1;
+    int rc = ok ? ANTS_OK : ANTS_ERR_CUDA;
+    std::vector<double> acc(total), B, b(n);
+    std::vector<int> members;
+    for (int t = 0; t < n_lrf && rc == ANTS_OK; ++t) {
+        members.clear();
+        for (int i = 0; i < N; ++i)
+            if ((group ? group[i] : (n_lrf == 1 ? 0 : i)) == t) members.push_back(i);
+        unsigned long long used = 0;
+        ok = cudaMemsetAsync(d_acc, 0, total * sizeof(double), st) == cudaSuccess &&
+             cudaMemsetAsync(d_used, 0, sizeof(unsigned long long), st) == cudaSuccess &&
+             (members.empty() || cudaMemcpyAsync(d_mem, members.data(), members.size() * sizeof(int), cudaMemcpyHostToDevice, st) == cudaSuccess);
+        if (ok && n_events > 0 && !members.empty()) {
+            FitXYParams p{};
+            p.sens_xy = d_xy; p.gains = d_g; p.xform = xform ? d_xf : nullptr; p.members = d_mem; p.n_members = (int)members.size();
+            p.signals = signals; p.xyzA = xyzA; p.n_events = n_events; p.N = N; p.nx = nx; p.ny = ny; p.ncu = ncu; p.nc = nc;
+            p.u_lo = u_lo; p.u_hi = u_hi; p.hu = (u_hi - u_lo) / nx; p.v_lo = v_lo; p.v_hi = v_hi; p.hv = (v_hi - v_lo) / ny;
+            p.axial = nullptr; p.n_used = d_used;
+            p.n_planes = n_planes; p.z_lo = z_lo; p.z_hi = z_hi; p.dz = (z_hi - z_lo) / (n_planes - 1);
+            const long long want = (n_events + warps - 1) / warps;
+            const int grid = (int)std::min<long long>(want, (long long)sms * occ);
+            for (int s = 0; s < n_slabs && ok; ++s)
+                for (int part = 0; part < 3 && ok; ++part) {
+                    p.slab = s; p.part = part; p.acc = d_acc + (size_t)(3 * s + part) * block;
+                    void *args[] = {&p};
+                    ok = cudaLaunchKernel((const void *)lrf_fit_xy_kernel, dim3(grid), dim3(warps * 32), args, smem, st) == cudaSuccess;
+                    if (ok) g_launches.fetch_add(1);
+                }
+        }
+        ok = ok && cudaMemcpyAsync(acc.data(), d_acc, total * sizeof(double), cudaMemcpyDeviceToHost, st) == cudaSuccess &&
+             cudaMemcpyAsync(&used, d_used, sizeof(used), cudaMemcpyDeviceToHost, st) == cudaSuccess &&
+             cudaStreamSynchronize(st) == cudaSuccess;
+        if (!ok) { rc = ANTS_ERR_CUDA; break; }
+        if (n_used_out) n_used_out[t] = (double)used;
+        // assemble the lower band: rows/columns ordered plane by plane
+        const size_t ld = (size_t)bw + 1;
+        B.assign((size_t)n * ld, 0.0);
+        std::fill(b.begin(), b.end(), 0.0);
+        auto at = [&](int i, int j) -> double & { return i >= j ? B[(size_t)i * ld + (bw - (i - j))] : B[(size_t)j * ld + (bw - (j - i))]; };
+        auto band = [&](const double *blk, int j1, int dv, int du, int &j2) -> const double * {
+            const int ju2 = j1 % ncu + du;
+            j2 = j1 + dv * ncu + du;
+            if (ju2 < 0 || ju2 >= ncu || j2 >= nc || j2 < j1) return nullptr;
+            return blk + (size_t)j1 * 29 + dv * 7 + du + 3;
+        };
+        for (int s = 0; s < n_slabs; ++s) {
+            const double *b0 = &acc[(size_t)(3 * s) * block], *b1 = b0 + block, *b2 = b1 + block;
+            const int o0 = s * nc, o1 = (s + 1) * nc;
+            for (int j1 = 0; j1 < nc; ++j1) {
+                b[o0 + j1] += b0[(size_t)j1 * 29 + 28];
+                b[o1 + j1] += b1[(size_t)j1 * 29 + 28];
+                for (int dv = 0; dv < 4; ++dv)
+                    for (int du = -3; du <= 3; ++du) {
+                        int j2;
+                        const double *v0 = band(b0, j1, dv, du, j2);
+                        if (!v0) continue;
+                        at(o0 + j2, o0 + j1) += *v0;                                   // plane s with itself
+                        at(o1 + j2, o1 + j1) += *band(b1, j1, dv, du, j2);             // plane s + 1 with itself
+                        const double x = *band(b2, j1, dv, du, j2);                    // plane s with plane s + 1
+                        at(o1 + j2, o0 + j1) += x;
+                        if (j2 != j1) at(o1 + j1, o0 + j2) += x;
+                    }
+            }
+        }
+        if (!solve_banded_spd(B, b, n, bw)) { rc = ANTS_ERR_SINGULAR; break; }
+        for (int j = 0; j < n; ++j) coeffs_out[(size_t)t * n + j] = (float)b[j];
+    }
+    if (rc != ANTS_OK) cudaStreamSynchronize(st);
+    cudaGetLastError();
     return rc;
 }

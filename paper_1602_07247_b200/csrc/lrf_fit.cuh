@@ -276,6 +276,13 @@ struct FitXYParams {
     double a_lo, a_hi;
     double *acc;                               // device [nc][29]
     unsigned long long *n_used;                // device [1]
+    // Sliced tables (R36): this launch takes the events between planes `slab` and `slab + 1` and adds
+    // one of the three sums the joint normal equations are made of, the pair's basis products weighted by
+    // (1-w)^2 (part 0: plane `slab` with itself; right-hand side weighted by 1-w), w^2 (part 1: plane `slab + 1`
+    // with itself; right-hand side by w) or (1-w) w (part 2: the two planes with each other; no right-hand side).
+    // slab < 0: a plain XY table.
+    int slab, part, n_planes;
+    double z_lo, z_hi, dz;
 };
 
 __global__ void __launch_bounds__(256) lrf_fit_xy_kernel(const FitXYParams p) {
@@ -289,6 +296,16 @@ __global__ void __launch_bounds__(256) lrf_fit_xy_kernel(const FitXYParams p) {
         const float4 pe = reinterpret_cast<const float4 *>(p.xyzA)[e];
         const double x = (double)pe.x, y = (double)pe.y, A = (double)pe.w;
         if (!(fabs(x) <= 1.7e308 && fabs(y) <= 1.7e308 && A > 0.0 && A <= 1.7e308)) continue;       // R22
+        double wm = 1.0, wy = 1.0;
+        if (p.slab >= 0) {
+            const double z = (double)pe.z;
+            if (!(z >= p.z_lo && z <= p.z_hi)) continue;                                            // R36
+            const int pl = max(min((int)floor((z - p.z_lo) / p.dz), p.n_planes - 2), 0);
+            if (pl != p.slab) continue;
+            const double w = (z - (p.z_lo + (double)pl * p.dz)) / p.dz;
+            wm = p.part == 0 ? (1.0 - w) * (1.0 - w) : p.part == 1 ? w * w : (1.0 - w) * w;
+            wy = p.part == 0 ? 1.0 - w : p.part == 1 ? w : 0.0;
+        }
         const float *sig = p.signals + e * p.N;
         for (int q = lane; q < p.n_members; q += 32) {
             const int i = p.members[q];
@@ -321,9 +338,9 @@ __global__ void __launch_bounds__(256) lrf_fit_xy_kernel(const FitXYParams p) {
             for (int b1 = 0; b1 < 4; ++b1)
 #pragma unroll
                 for (int a1 = 0; a1 < 4; ++a1) {
-                    const double w1 = bv[b1] * bu[a1];
+                    const double w0 = bv[b1] * bu[a1], w1 = w0 * wm;
                     double *row = xy_smem + (size_t)((kv + b1) * p.ncu + ku + a1) * 29;
-                    atomicAdd(row + 28, w1 * yv);
+                    if (wy != 0.0) atomicAdd(row + 28, w0 * wy * yv);
 #pragma unroll
                     for (int b2 = b1; b2 < 4; ++b2)
 #pragma unroll
@@ -337,7 +354,7 @@ __global__ void __launch_bounds__(256) lrf_fit_xy_kernel(const FitXYParams p) {
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) used += __shfl_xor_sync(0xffffffffu, used, o);
-    if (lane == 0 && used) atomicAdd(p.n_used, used);
+    if (lane == 0 && used && (p.slab < 0 || p.part == 0)) atomicAdd(p.n_used, used);
     __syncthreads();
     for (int i = threadIdx.x; i < total; i += blockDim.x)
         if (xy_smem[i] != 0.0) atomicAdd(p.acc + i, xy_smem[i]);

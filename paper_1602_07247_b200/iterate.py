@@ -37,6 +37,11 @@ def iterate_response(cfg, signals, n_cycles: int, score_max: float = float("nan"
             c, _ = recon.ants_lrf_fit_xy(cur.sensor_xy, cur.gains, cur.knots_xy, cur.n_lrf, cur.n_int_x, cur.n_int_y, signals,
                                          xyzA, group=getattr(cur, "group", None), xform=getattr(cur, "xform", None), axial=axial)
             nxt.coeffs_xy = c[:, None, :, :].astype(np.float32)
+        elif cur.lrf_dim == 5:
+            c, _ = recon.ants_lrf_fit_sliced(cur.sensor_xy, cur.gains, cur.knots_xy, cur.n_lrf, cur.n_int_x, cur.n_int_y,
+                                             cur.n_planes, signals, xyzA, group=getattr(cur, "group", None),
+                                             xform=getattr(cur, "xform", None))
+            nxt.coeffs_xy = c.astype(np.float32)
         elif cur.lrf_dim == 2:
             c, _ = recon.ants_lrf_fit_axial_z(cur.sensor_xy, cur.gains, cur.knots, cur.n_int_r, cur.n_int_z, signals, xyzA)
             nxt.coeffs = c[None, :, :].astype(np.float32)

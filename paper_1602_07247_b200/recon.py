@@ -75,6 +75,9 @@ def load():
     lib.ants_plan_kernel_name.argtypes = [vp, C.POINTER(GridParams), C.c_int32, C.c_char_p, C.c_int32]
     lib.ants_probe_throughput.restype = C.c_int
     lib.ants_probe_throughput.argtypes = [C.c_int32, C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+    lib.ants_lrf_fit_sliced.restype = C.c_int
+    lib.ants_lrf_fit_sliced.argtypes = [vp, vp, vp, vp, vp, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, vp, vp,
+                                        C.c_int64, vp, vp, vp]
     lib.ants_lrf_fit_xy.restype = C.c_int
     lib.ants_lrf_fit_xy.argtypes = [vp, vp, vp, vp, vp, C.c_int32, C.c_int32, C.c_int32, C.c_int32, vp, vp, C.c_int32,
                                     vp, vp, C.c_int64, vp, vp, vp]
@@ -320,6 +323,33 @@ def ants_lrf_fit_xy(sensor_xy, gains, knots_xy, n_lrf: int, n_int_x: int, n_int_
                                 int(n_r), signals.data_ptr(), xyzA.data_ptr(), E, coeffs.ctypes.data, used.ctypes.data, st)
     if rc != 0:
         raise AntsError(rc, "ants_lrf_fit_xy")
+    return coeffs, used
+
+
+def ants_lrf_fit_sliced(sensor_xy, gains, knots_xy, n_lrf: int, n_int_x: int, n_int_y: int, n_planes: int, signals, xyzA,
+                        group=None, xform=None, stream=None):
+    """Sliced LRF calculation, all planes of a table jointly (include/ants_recon.h).
+    -> (coeffs float32 [n_lrf][n_planes][n_int_y+3][n_int_x+3], pairs used float64 [n_lrf])."""
+    import torch
+    xy, kn = _f32(sensor_xy).reshape(-1, 2), _f32(knots_xy)
+    N, E = xy.shape[0], int(signals.shape[0])
+    g = None if gains is None else _f32(gains)
+    gr = None if group is None else np.ascontiguousarray(np.asarray(group, dtype=np.int32))
+    xf = None if xform is None else _f32(xform).reshape(N, 4)
+    for t in (signals, xyzA):
+        if not (t.is_cuda and t.is_contiguous() and t.dtype == torch.float32):
+            raise ValueError("ants_lrf_fit_sliced needs contiguous float32 CUDA tensors")
+    if signals.shape[1] != N or tuple(xyzA.shape) != (E, 4) or kn.size < 6:
+        raise ValueError("ants_lrf_fit_sliced: shape mismatch")
+    coeffs = np.zeros((int(n_lrf), int(n_planes), int(n_int_y) + 3, int(n_int_x) + 3), np.float32)
+    used = np.zeros(int(n_lrf), np.float64)
+    st = torch.cuda.current_stream().cuda_stream if stream is None else int(stream)
+    rc = load().ants_lrf_fit_sliced(xy.ctypes.data, None if g is None else g.ctypes.data,
+                                    None if gr is None else gr.ctypes.data, None if xf is None else xf.ctypes.data,
+                                    kn.ctypes.data, N, int(n_lrf), int(n_int_x), int(n_int_y), int(n_planes),
+                                    signals.data_ptr(), xyzA.data_ptr(), E, coeffs.ctypes.data, used.ctypes.data, st)
+    if rc != 0:
+        raise AntsError(rc, "ants_lrf_fit_sliced")
     return coeffs, used
 
 

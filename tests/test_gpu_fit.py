@@ -270,3 +270,70 @@ def test_xy_and_composite_fit_parity():
     with pytest.raises(recon.AntsError) as ei:
         recon.ants_lrf_fit_xy(xy, gains, np.array([-60, 60, -60, 60], np.float32), 1, 12, 12, sig_d, pos_d)
     assert ei.value.status == -5
+
+
+def test_sliced_fit_parity():
+    """ants_lrf_fit_sliced vs the oracle (R36): all planes of a table jointly; one shared table with gains and D4
+    symmetry groups with frames; events outside the planes' range and failed events are left out; the fitted tables go
+    straight into ants_lrf_create_xy (lrf_dim 5) and reconstruct in 3-D."""
+    from test_oracle_fit import _sliced_problem
+    xy, gains, sig, pos = _sliced_problem(30_011, seed=4)
+    pos[17] = np.nan
+    pos[101, 3] = -1.0
+    knots = np.array([-12, 12, -12, 12, 0, 12], np.float32)
+    nx, ny, n_planes = 5, 4, 4
+    group, xform, n_groups = recon.ants_group_by_symmetry(xy, 4, True)
+    sig_d, pos_d = torch.from_numpy(sig).cuda(), torch.from_numpy(pos).cuda()
+    for kw in (dict(n_lrf=1), dict(n_lrf=n_groups, group=group, xform=xform)):
+        c, used = recon.ants_lrf_fit_sliced(xy, gains, knots, kw["n_lrf"], nx, ny, n_planes, sig_d, pos_d,
+                                            group=kw.get("group"), xform=kw.get("xform"))
+        c0, used0 = ofit.fit_sliced(xy, gains, knots, kw["n_lrf"], nx, ny, n_planes, sig, pos, group=kw.get("group"),
+                                    xform=kw.get("xform"))
+        assert c.shape == c0.shape == (kw["n_lrf"], n_planes, ny + 3, nx + 3)
+        assert np.array_equal(used, used0), kw.keys()
+        scale = np.abs(c0).max(axis=(1, 2, 3), keepdims=True)
+        assert (np.abs(c - c0) <= 5e-6 * scale).all(), (kw.keys(), np.abs(c - c0).max())
+    dims = recon.LrfDims(len(xy), n_groups, 5, 0, 0)
+    h = recon.ants_lrf_create_xy(xy, gains, None, None, dims, nx, ny, n_planes, knots, c, xform=xform, group=group)
+    grid = recon.GridParams(3, 5, 2.0, 1.5, 0.5, 6, 0, 6.0)
+    out, score = torch.empty((256, 4), device="cuda"), torch.empty(256, device="cuda")
+    recon.ants_reconstruct(h, sig_d[:256].contiguous(), grid, 0, out, score)
+    torch.cuda.synchronize()
+    recon.ants_destroy(h)
+    ok = torch.isfinite(out[:, 0])
+    assert ok.float().mean() > 0.9 and (out[ok, :2].abs().max() <= 40.0)
+    # a plane without data: underdetermined
+    with pytest.raises(recon.AntsError) as ei:
+        recon.ants_lrf_fit_sliced(xy, gains, np.array([-12, 12, -12, 12, 0, 40], np.float32), 1, nx, ny, n_planes, sig_d, pos_d)
+    assert ei.value.status == -5
+    # limits
+    with pytest.raises(recon.AntsError) as ei:
+        recon.ants_lrf_fit_sliced(xy, gains, knots, 1, nx, ny, 1, sig_d, pos_d)
+    assert ei.value.status == -1                     # ANTS_ERR_INVALID: a Sliced LRF has at least two planes
+
+
+def test_sliced_fit_at_config7_table_sizes():
+    """Config 7's own tables (5 planes of 23 x 23 coefficients: 2,645 unknowns, banded solve) from 200 k synthetic
+    events at their true positions: the well-covered centre of every plane comes back within the Poisson noise, and
+    the pair count is the definition's."""
+    cfg = synth.make_config(7)
+    ev = synth.generate_events(cfg, 200_000)
+    sig = ev["signals"].cuda().contiguous()
+    pos_h = torch.cat([ev["true_xyz"], 0.1 * ev["n_ph"][:, None]], 1).float().contiguous()
+    c, used = recon.ants_lrf_fit_sliced(cfg.sensor_xy, cfg.gains, cfg.knots_xy, 1, cfg.n_int_x, cfg.n_int_y, cfg.n_planes,
+                                        sig, pos_h.cuda())
+    assert c.shape == cfg.coeffs_xy.shape
+    p = pos_h.numpy().astype(np.float64)
+    xy = cfg.sensor_xy.astype(np.float64)
+    inside = (p[:, 2] >= 0.0) & (p[:, 2] <= 20.0)
+    du, dv = p[:, None, 0] - xy[None, :, 0], p[:, None, 1] - xy[None, :, 1]
+    n_pairs = (inside[:, None] & (np.abs(du) <= 120.0) & (np.abs(dv) <= 120.0)).sum()
+    assert used[0] == n_pairs
+    d = np.abs(c - cfg.coeffs_xy)[0, :, 6:17, 6:17]
+    assert d.max() <= 0.05, d.max()                       # coefficients there are 0.3 .. 7.8
+    # one reconstruct -> filter -> refit cycle of the iterative loop on the Sliced model (PAPER.md:428)
+    from paper_1602_07247_b200 import iterate
+    (cycle, cur, n_pass), = list(iterate.iterate_response(cfg, sig, 1))
+    assert n_pass > 0.9 * sig.shape[0] and cur.coeffs_xy.shape == cfg.coeffs_xy.shape
+    d = np.abs(cur.coeffs_xy - cfg.coeffs_xy)[0, :, 6:17, 6:17]
+    assert d.max() <= 0.4, d.max()                        # reconstructed positions: resolution smears the peak

@@ -8,7 +8,9 @@ synthetic flood-field events = ONE kernel launch through the C ABI (ants_reconst
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config 5] [--impl ours|reference]
 
 The headline is config 5 (the largest single-GPU configuration: 127 PMTs, 16 M events in 8 batches of
-2 M); `per_config` carries the same measurements for all five BASELINE.json configs (N = 1).
+2 M); `per_config` carries the same measurements for all five BASELINE.json configs (N = 1), each
+with `cycle`: one reconstruct -> filter -> LRF-calculation cycle of the iterative response
+reconstruction on one batch.
 Prints ONE JSON line (rank 0).  `value` is device-resident throughput (CUDA events on the
 launching stream, L2 flushed between steps, max over ranks); `e2e` is the same metric through
 ants_reconstruct_host with pinned HOST buffers (H2D and D2H inside the timed region);
@@ -370,6 +372,17 @@ def measure_config(idx: int, args, device, rank: int, world: int, dist, steps: i
     out["plan"] = r.plan()
     out["roofline"] = roofline_of(cfg, out["plan"], E, local_ms / max(gpu_launches, 1), prop, max_mhz)
 
+    # ---- one reconstruct -> filter -> LRF-calculation cycle on the first resident batch (N = 1) ----------------
+    if world == 1 and not args.no_cycle:
+        try:
+            res = time_cycle(recon, cfg, r, sigs[0], xyzA, score, stream, 3, 1)
+            t_c = sum(res["ms"]) / len(res["ms"])
+            out["cycle"] = {"value": E / (t_c * 1e-3), "unit": "events/s through one reconstruct -> filter -> LRF calculation",
+                            "ms_per_cycle": t_c, "lrf_calculation_ms": sum(res["fit_ms"]) / len(res["fit_ms"]),
+                            "events_passing_filter": res["n_pass"], "gpu_launches": res["gpu_launches"]}
+        except recon.AntsError as ex:      # e.g. a table the batch does not cover
+            out["cycle"] = {"unavailable": str(ex)}
+
     # ---- oracle beside it (rank 0, N = 1) --------------------------------------------------------------
     if rank == 0 and world == 1 and not args.no_cpu_baseline and cpu_seconds > 0:
         n_pool = min(E, 262_144)
@@ -406,8 +419,9 @@ def run_ours(args):
             "plan": head["plan"]}
     if "cpu_baseline" in head:
         line["cpu_baseline"] = head["cpu_baseline"]
-    if "us_per_call" in head:
-        line["us_per_call"] = head["us_per_call"]
+    for k in ("us_per_call", "cycle"):
+        if k in head:
+            line[k] = head[k]
 
     # ---- every BASELINE.json config beside the headline (N = 1 only: north_star asks for all five) -----
     if world == 1 and not args.no_per_config and args.events is None:
@@ -418,7 +432,7 @@ def run_ours(args):
             entry = {k: m[k] for k in ("value", "unit", "ms_per_step", "steps", "warmup", "gpu_launches", "roofline",
                                         "e2e", "plan", "clocks", "config") if k in m}
             entry["config_index"] = idx
-            for k in ("cpu_baseline", "us_per_call"):
+            for k in ("cpu_baseline", "us_per_call", "cycle"):
                 if k in m:
                     entry[k] = m[k]
             per.append(entry)
@@ -524,6 +538,57 @@ def run_fit(args):
     return 0
 
 
+def lrf_calculation(recon, cfg, sig, xyzA):
+    """The LRF calculation that belongs to the config's parameterisation (PAPER.md:380-396), as iterate.py calls it;
+    per-sensor axial tables are fitted up to 30 mm (a flood batch does not cover every sensor's far intervals)."""
+    knots = cfg.knots.copy()
+    if cfg.n_lrf > 1 and cfg.lrf_dim == 1:
+        knots[1] = min(float(knots[1]), 30.0)
+    group, xform = getattr(cfg, "group", None), getattr(cfg, "xform", None)
+    if cfg.lrf_dim == 2:
+        return recon.ants_lrf_fit_axial_z(cfg.sensor_xy, cfg.gains, knots, cfg.n_int_r, cfg.n_int_z, sig, xyzA)
+    if cfg.lrf_dim == 5:
+        return recon.ants_lrf_fit_sliced(cfg.sensor_xy, cfg.gains, cfg.knots_xy, cfg.n_lrf, cfg.n_int_x, cfg.n_int_y,
+                                         cfg.n_planes, sig, xyzA, group=group, xform=xform)
+    axial = None
+    if cfg.lrf_dim in (1, 4):
+        ca, used = recon.ants_lrf_fit_axial(cfg.sensor_xy, cfg.gains, knots, cfg.n_lrf, cfg.n_int_r, sig, xyzA, group=group)
+        if cfg.lrf_dim == 1:
+            return ca, used
+        axial = (knots, ca)
+    return recon.ants_lrf_fit_xy(cfg.sensor_xy, cfg.gains, cfg.knots_xy, cfg.n_lrf, cfg.n_int_x, cfg.n_int_y, sig, xyzA,
+                                 group=group, xform=xform, axial=axial)
+
+
+def time_cycle(recon, cfg, r, sig, xyzA, score, stream, steps, warmup):
+    """One cycle of the iterative response reconstruction: reconstruct the batch, filter on the score,
+    recalculate the LRFs; CUDA events on the launching stream around the cycle and around its LRF calculation."""
+    import torch
+
+    def cycle(ev=None):
+        recon.ants_reconstruct(r.handle, sig, r.grid, r.method, xyzA, score, stream.cuda_stream)
+        n_pass = recon.ants_filter_events(xyzA, score, score_max=4.0 * cfg.n_sensors)
+        if ev:
+            ev[0].record(stream)
+        lrf_calculation(recon, cfg, sig, xyzA)
+        if ev:
+            ev[1].record(stream)
+        return n_pass
+
+    for _ in range(warmup):
+        cycle()
+    n0 = recon.launch_count()
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(steps)]
+    for a, f0, f1, b in ev:
+        a.record(stream)
+        n_pass = cycle((f0, f1))
+        b.record(stream)
+    torch.cuda.synchronize()
+    ms = [a.elapsed_time(b) for a, _, _, b in ev]
+    fit_ms = [f0.elapsed_time(f1) for _, f0, f1, _ in ev]
+    return {"ms": ms, "fit_ms": fit_ms, "n_pass": int(n_pass), "gpu_launches": int(recon.launch_count() - n0)}
+
+
 def run_cycle(args):
     """Times one cycle of the iterative response reconstruction: reconstruct the batch,
     filter on the score, recalculate the LRFs.  Secondary workload (`--workload cycle`)."""
@@ -535,33 +600,11 @@ def run_cycle(args):
     cfg = synth.make_config(args.config)
     E = cfg.n_events // cfg.n_batches if args.events is None else args.events
     sig = synth.generate_events(cfg, E, device=device)["signals"]
-    knots = cfg.knots.copy()
-    if cfg.n_lrf > 1:
-        knots[1] = min(float(knots[1]), 30.0)
     r = recon.Reconstructor(cfg)
     xyzA = torch.empty((E, 4), dtype=torch.float32, device=device)
     score = torch.empty((E,), dtype=torch.float32, device=device)
-    stream = torch.cuda.current_stream()
-
-    def cycle():
-        recon.ants_reconstruct(r.handle, sig, r.grid, r.method, xyzA, score, stream.cuda_stream)
-        n_pass = recon.ants_filter_events(xyzA, score, score_max=4.0 * cfg.n_sensors)
-        if cfg.lrf_dim == 2:
-            recon.ants_lrf_fit_axial_z(cfg.sensor_xy, cfg.gains, knots, cfg.n_int_r, cfg.n_int_z, sig, xyzA)
-        else:
-            recon.ants_lrf_fit_axial(cfg.sensor_xy, cfg.gains, knots, cfg.n_lrf, cfg.n_int_r, sig, xyzA)
-        return n_pass
-
-    for _ in range(args.warmup):
-        cycle()
-    n0 = recon.launch_count()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    for a, b in ev:
-        a.record(stream)
-        n_pass = cycle()
-        b.record(stream)
-    torch.cuda.synchronize()
-    ms = [a.elapsed_time(b) for a, b in ev]
+    res = time_cycle(recon, cfg, r, sig, xyzA, score, torch.cuda.current_stream(), args.steps, args.warmup)
+    ms, n_pass = res["ms"], res["n_pass"]
     t = sum(ms) / len(ms) * 1e-3
     r.close()
     print(json.dumps({"metric": "events/s through one reconstruct -> filter -> LRF-calculation cycle", "value": E / t,
@@ -569,7 +612,7 @@ def run_cycle(args):
                       "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32+f64",
                       "data": "synthetic", "config": {"workload": cfg.name + " response-reconstruction cycle",
                                                       "events_per_step_per_gpu": E, "events_passing_filter": n_pass},
-                      "gpu_launches": recon.launch_count() - n0, "step_ms": ms}), flush=True)
+                      "gpu_launches": res["gpu_launches"], "step_ms": ms, "lrf_calculation_ms": res["fit_ms"]}), flush=True)
     return 0
 
 
@@ -640,6 +683,7 @@ def main(argv=None):
     ap.add_argument("--config", type=int, default=5,
                     help="BASELINE.json config 1..5 of the headline (default 5 = the largest single-GPU config: "
                          "16 M events as 8 batches of 2 M); 6, 7, 8 = the XY / Sliced / Composite LRF workloads")
+    ap.add_argument("--no-cycle", action="store_true", help="skip the response-reconstruction cycle entries")
     ap.add_argument("--no-per-config", action="store_true", help="skip the per_config entries of the other configs")
     ap.add_argument("--per-config-cpu-seconds", type=float, default=5.0)
     ap.add_argument("--events", type=int, default=None, help="events per step per GPU (default: the config's batch)")

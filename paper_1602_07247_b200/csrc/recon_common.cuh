@@ -254,7 +254,9 @@ __device__ __forceinline__ bool prepare_event(const Params &p, const float4 *sen
         sxw = fmaf(sn.x, wgt, sxw);
         syw = fmaf(sn.y, wgt, syw);
         float cs = 0.f;
-        if (METHOD == 0 && S > 0.f) cs = log2f(S / sn.z);
+        // c_i = log2(S_i / g_i) only conditions the plain score (sum_i S_i c_i is the same at every node), so the
+        // fast forms do: an error in it shifts all scores of the event alike
+        if (METHOD == 0 && S > 0.f) cs = lg2_approx(fmaxf(S * rcp_approx(sn.z), 1e-30f));
         SC[i] = make_float2(S, cs);
     }
     finite = __all_sync(kFull, finite);

@@ -835,8 +835,11 @@ static int make_plan(const ants_lrf *h, const ants_grid_params_t *g, int32_t met
     if (!pl.npt) return ANTS_ERR_UNSUPPORTED;
     // strictly positive axial LRFs (the normal case): the sensor-pair-packed kernel
     pl.family = 0;
-    // node reuse (recon2d_pk_kernel.cuh): contraction 1/2, odd G, and an array large enough for it to pay
-    pl.reuse = g->factor == 0.5f && (g->nodes_per_axis & 1) && m.N >= 96 && !knob_no_reuse() ? 1 : 0;
+    // node reuse (recon2d_pk_kernel.cuh): contraction 1/2, odd G, and where it was measured to pay: large arrays
+    // (config 5 +7 %), and the Poisson kernel with up to three nodes per lane at any size (configs 1, 2: +2..3 %);
+    // the chi-square kernel with four nodes per lane loses with it on a 64-sensor array (config 3: -7 %)
+    const bool pays = m.N >= 96 || (method == ANTS_POISSON_ML && pl.npt <= 3);
+    pl.reuse = g->factor == 0.5f && (g->nodes_per_axis & 1) && pays && !knob_no_reuse() ? 1 : 0;
     if (env_knob_force_reuse()) pl.reuse = g->factor == 0.5f && (g->nodes_per_axis & 1) ? 1 : 0;
     pl.kernel = kernel_2d_pk(method, pl.npt, pl.reuse);
     if (!pl.kernel) return ANTS_ERR_UNSUPPORTED;

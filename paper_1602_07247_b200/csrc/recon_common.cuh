@@ -124,6 +124,24 @@ __device__ __forceinline__ float hsum2(f32x2 v) {
     return a + b;
 }
 
+// log2 of two positive, normal, finite numbers to a few ulp (relative, also next to 1, where lg2.approx has only an
+// absolute bound), in a third of the instructions of two inlined log2f: x = 2^e m with m in [2/3, 4/3),
+// log2 m = (2 / ln 2) atanh(s), s = (m - 1)/(m + 1), |s| <= 0.2, odd series to s^11 (next term 6e-11); the division
+// is rcp.approx (1 ulp).  The plain score's term sumS log2(A_ref sumL / sumS) needs the relative accuracy: its
+// argument is ~1 at the nodes that compete for the minimum (an absolute error of 2^-22 sumS broke the node-index
+// rule on config 1 in round 2).
+__device__ __forceinline__ f32x2 log2_pos2(float x0, float x1) {
+    const int b0 = __float_as_int(x0), b1 = __float_as_int(x1);
+    const int e0 = (b0 - 0x3f2aaaab) >> 23, e1 = (b1 - 0x3f2aaaab) >> 23;
+    const f32x2 f = add2(pk(__int_as_float(b0 - (e0 << 23)), __int_as_float(b1 - (e1 << 23))), pk1(-1.f));
+    float d0, d1;
+    upk(add2(f, pk1(2.f)), d0, d1);
+    const f32x2 s = mul2(f, pk(rcp_approx(d0), rcp_approx(d1))), t = mul2(s, s);
+    const f32x2 poly = fma2(t, fma2(t, fma2(t, fma2(t, fma2(t, pk1(0.262308189f), pk1(0.320598898f)), pk1(0.412198583f)),
+                                            pk1(0.577078016f)), pk1(0.961796694f)), pk1(2.885390082f));
+    return fma2(s, poly, pk((float)e0, (float)e1));
+}
+
 __device__ __forceinline__ float warp_sum(float v) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(kFull, v, o);

@@ -844,7 +844,7 @@ static int make_plan(const ants_lrf *h, const ants_grid_params_t *g, int32_t met
     pl.kernel = kernel_2d_pk(method, pl.npt, pl.reuse);
     if (!pl.kernel) return ANTS_ERR_UNSUPPORTED;
     first_diff_iter(h, g, method, pl.k_diff, pl.k_series);
-    const size_t tables = (cta_smem_bytes_pk(m.N, m.n_lrf * (m.n_r + 1)) + 15) / 16 * 16;
+    const size_t tables = (cta_smem_bytes_pk(m.N, m.n_lrf * (m.n_r + 1), pl.npt) + 15) / 16 * 16;
     const size_t per_warp = warp_smem_bytes_pk(m.N, method, (int)nodes);
     pick_cta_shape(tables, per_warp, pl);
     if (pl.smem > 227 * 1024) return ANTS_ERR_UNSUPPORTED;

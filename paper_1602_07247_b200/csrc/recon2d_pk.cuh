@@ -32,9 +32,13 @@ __host__ __device__ inline size_t warp_smem_bytes_pk(int N, int method, int node
     const size_t np4 = ((size_t)nodes + 3) / 4 * 4;
     return ((size_t)pk_pairs(N) * 16 * narr + ((size_t)N * 8 + 15) / 16 * 16 + np4 * 9 + 15) / 16 * 16;
 }
-// CTA-shared: sens_s [N] float4, poly_s [rows] float4, grp_s [N] int, node_s [256] float2 (grid offsets of the
-// nodes in units of the step: a table look-up instead of an integer division wherever a lane needs its nodes)
-__host__ __device__ inline size_t cta_smem_bytes_pk(int N, int rows) { return cta_table_bytes(N, rows) + 256 * 8; }
+// CTA-shared: sens_s [N] float4, poly_s [rows] float4, grp_s [N] int, node_s [P] float2 (grid offsets of the nodes in
+// units of the step: a table look-up instead of an integer division wherever a lane needs its nodes; P = 32 x the
+// nodes per lane, the excess zero), and the static node lists of the node-reuse kernel
+// (recon2d_pk_kernel.cuh): ident_s, todo_s, even_s [P] u8, evoff_s [P] s16, three counters
+__host__ __device__ inline size_t cta_smem_bytes_pk(int N, int rows, int npt) {
+    return cta_table_bytes(N, rows) + (size_t)(32 * npt) * (8 + 3 + 2) + 16;
+}
 
 __device__ __forceinline__ WarpSmemPk carve_pk(unsigned char *base, int N, int method, int nodes) {
     WarpSmemPk w;

@@ -22,15 +22,46 @@ __global__ void __launch_bounds__(256, (NPT <= 3 ? 3 : 2)) recon2d_pk_kernel(con
     for (int i = threadIdx.x; i < N; i += blockDim.x) { sens_s[i] = m.sens[i]; grp_s[i] = m.grp[i]; }
     for (int i = threadIdx.x; i < rows; i += blockDim.x) poly_s[i] = m.poly[i];
     float2 *node_s = reinterpret_cast<float2 *>(smem + cta_table_bytes(N, rows));
+    constexpr int slots = 32 * NPT;
     {
         const float halfg = 0.5f * (float)(p.G - 1);
-        for (int n = threadIdx.x; n < 256; n += blockDim.x) {
+        for (int n = threadIdx.x; n < slots; n += blockDim.x) {
             const int iy = n / p.G, ix = n - iy * p.G;
             node_s[n] = n < p.nodes ? make_float2((float)ix - halfg, (float)iy - halfg) : make_float2(0.f, 0.f);
         }
     }
+    // Node reuse, static part: with a previous winner far enough from the border of its grid, the nodes that coincide
+    // with old ones (both offsets from the centre even) and the ones to evaluate are the same lists in every
+    // iteration; only a winner near the border needs the lists built for it.
+    unsigned char *ident_s = reinterpret_cast<unsigned char *>(node_s + slots);     // 0, 1, 2, ...: every node
+    unsigned char *todo_s = ident_s + slots, *even_s = todo_s + slots;
+    short *evoff_s = reinterpret_cast<short *>(even_s + slots);
+    int *lists_s = reinterpret_cast<int *>(evoff_s + slots);         // {n_todo, n_even, reach of the even offsets}
+    if (REUSE)
+        for (int n = threadIdx.x; n < slots; n += blockDim.x) ident_s[n] = (unsigned char)n;
+    if (REUSE && warp == 0) {
+        const int hg = (p.G - 1) >> 1;
+        const unsigned ltm = (1u << lane) - 1u;
+        int ct = 0, ce = 0, mr = 0;
+        for (int n0 = 0; n0 < p.nodes; n0 += 32) {
+            const int n = n0 + lane, iy = n / p.G, ix = n - iy * p.G, dxn = ix - hg, dyn = iy - hg;
+            const bool valid = n < p.nodes, even = valid && !((dxn | dyn) & 1);
+            const unsigned mt = __ballot_sync(kFull, valid && !even), me = __ballot_sync(kFull, even);
+            if (valid && !even) todo_s[ct + __popc(mt & ltm)] = (unsigned char)n;
+            if (even) {
+                const int q = ce + __popc(me & ltm);
+                even_s[q] = (unsigned char)n;
+                evoff_s[q] = (short)((dyn >> 1) * p.G + (dxn >> 1));
+                mr = max(mr, max(abs(dxn >> 1), abs(dyn >> 1)));
+            }
+            ct += __popc(mt);
+            ce += __popc(me);
+        }
+        mr = __reduce_max_sync(kFull, mr);
+        if (lane == 0) { lists_s[0] = ct; lists_s[1] = ce; lists_s[2] = mr; }
+    }
     __syncthreads();
-    WarpSmemPk w = carve_pk(smem + (cta_smem_bytes_pk(N, rows) + 15) / 16 * 16 +
+    WarpSmemPk w = carve_pk(smem + (cta_smem_bytes_pk(N, rows, NPT) + 15) / 16 * 16 +
                             (size_t)warp * warp_smem_bytes_pk(N, METHOD, p.nodes), N, METHOD, p.nodes);
     const int np1 = pk_pairs(N);
     const unsigned poly_base = (unsigned)__cvta_generic_to_shared(poly_s) - ((unsigned)kMagicBits << 4);
@@ -84,41 +115,51 @@ __global__ void __launch_bounds__(256, (NPT <= 3 ? 3 : 2)) recon2d_pk_kernel(con
         const bool reuse_ok = REUSE && p.factor == 0.5f && (p.G & 1);
         float *sc_prev = w.S0, *sc_cur = w.S1;
         bool have_prev = false;
-        int prev_bi = 0, prev_mode = -1;
+        int prev_bi = 0, prev_bx = 0, prev_by = 0, prev_mode = -1;
         const unsigned lt = (1u << lane) - 1u;
 
         float h = p.h0_xy;
         for (int k = 0; k < p.K; ++k) {
             const int mode = k < p.k_diff ? 0 : 1;
             // ---- the nodes of this iteration: carried over or to be evaluated ----
-            int count = REUSE ? 0 : p.nodes;
-            if (REUSE) {
-                const bool reuse = reuse_ok && have_prev && mode == prev_mode;
-                const int by = prev_bi / p.G, bx = prev_bi - by * p.G;
-                const float off = (reuse && mode == 1) ? sc_prev[prev_bi] : 0.f;
+            int count = p.nodes;
+            const unsigned char *lst = ident_s;
+            if (REUSE && reuse_ok && have_prev && mode == prev_mode) {
+                const float off = mode == 1 ? sc_prev[prev_bi] : 0.f;
+                const int mr = lists_s[2];
+                if (prev_bx >= mr && prev_bx + mr < p.G && prev_by >= mr && prev_by + mr < p.G) {
+                    // every coinciding node lies inside the previous grid: the static lists
+                    const int n_even = lists_s[1];
+                    for (int t = lane; t < n_even; t += 32) sc_cur[even_s[t]] = sc_prev[prev_bi + evoff_s[t]] - off;
+                    count = lists_s[0];
+                    lst = todo_s;
+                } else {
+                    count = 0;
 #pragma unroll
-                for (int j = 0; j < NPT; ++j) {
-                    const int n = lane + 32 * j;
-                    bool todo = n < p.nodes;
-                    if (reuse && todo) {
-                        const float2 no = node_s[n];
-                        const int dxn = (int)no.x, dyn = (int)no.y;          // steps from the centre (G odd: integers)
-                        const int ox = bx + (dxn >> 1), oy = by + (dyn >> 1);
-                        if (!((dxn | dyn) & 1) && (unsigned)ox < (unsigned)p.G && (unsigned)oy < (unsigned)p.G) {
-                            sc_cur[n] = sc_prev[oy * p.G + ox] - off;
-                            todo = false;
+                    for (int j = 0; j < NPT; ++j) {
+                        const int n = lane + 32 * j;
+                        bool todo = n < p.nodes;
+                        if (todo) {
+                            const float2 no = node_s[n];
+                            const int dxn = (int)no.x, dyn = (int)no.y;      // steps from the centre (G odd: integers)
+                            const int ox = prev_bx + (dxn >> 1), oy = prev_by + (dyn >> 1);
+                            if (!((dxn | dyn) & 1) && (unsigned)ox < (unsigned)p.G && (unsigned)oy < (unsigned)p.G) {
+                                sc_cur[n] = sc_prev[oy * p.G + ox] - off;
+                                todo = false;
+                            }
                         }
+                        const unsigned mk = __ballot_sync(kFull, todo);
+                        if (todo) w.L[count + __popc(mk & lt)] = (unsigned char)n;
+                        count += __popc(mk);
                     }
-                    const unsigned mk = __ballot_sync(kFull, todo);
-                    if (todo) w.L[count + __popc(mk & lt)] = (unsigned char)n;
-                    count += __popc(mk);
+                    __syncwarp();
+                    lst = w.L;
                 }
-                __syncwarp();
             }
             int nid[NPT];
 #pragma unroll
             for (int j = 0; j < NPT; ++j)
-                nid[j] = !REUSE ? lane + 32 * j : lane + 32 * j < count ? (int)w.L[lane + 32 * j] : 0;
+                nid[j] = !REUSE ? lane + 32 * j : lane + 32 * j < count ? (int)lst[lane + 32 * j] : 0;
 
             float sc_node[NPT];          // scores of this lane's nodes (lower is better), +inf = invalid
             float aux_node[NPT];         // plain mode: sum L (Poisson) / A (chi2) at the node
@@ -168,6 +209,10 @@ __global__ void __launch_bounds__(256, (NPT <= 3 ? 3 : 2)) recon2d_pk_kernel(con
                 const float2 wo = node_s[bi];           // the winner's grid offsets (one broadcast load)
                 cx = fmaf(wo.x, h, cx);
                 cy = fmaf(wo.y, h, cy);
+                if (REUSE) {                            // its column and row (G odd: the offsets are integers)
+                    prev_bx = (int)wo.x + ((p.G - 1) >> 1);
+                    prev_by = (int)wo.y + ((p.G - 1) >> 1);
+                }
             }
             if (p.out_path && lane == 0) p.out_path[e * p.K + k] = found ? (uint16_t)bi : (uint16_t)0xFFFF;
             h *= p.factor;

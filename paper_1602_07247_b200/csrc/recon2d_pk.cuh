@@ -17,7 +17,7 @@
 
 namespace ants {
 
-constexpr int kPkArrays = 10;   // D0..D7, E0, E1 (float4 [Np + 1] each)
+constexpr int kPkArrays = 9;    // D0..D7 and, for the least-squares methods, E0 (float4 [Np + 1] each)
 
 struct WarpSmemPk {
     float4 *D[kPkArrays];   // per-pair records of the current iteration (plain mode uses D[0] only)

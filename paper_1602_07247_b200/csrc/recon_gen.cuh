@@ -24,9 +24,10 @@ constexpr int kNB = 3;   // nodes per lane per chunk
 
 enum LrfKind { kAxial = 1, kAxialZ = 2, kXY = 3, kComposite = 4, kSliced = 5 };
 
-// per-warp shared memory of the general kernel: prepared signals and the list of active sensors
+// per-warp shared memory of the general kernel: the least-squares weights in double, prepared signals and the list of
+// active sensors
 __host__ __device__ inline size_t warp_smem_bytes_gen(int N) {
-    return ((size_t)N * 8 + (size_t)N * 2 + 15) / 16 * 16;
+    return ((size_t)N * 8 + (size_t)N * 8 + (size_t)N * 2 + 15) / 16 * 16;
 }
 // CTA-shared tables: sens_s [N] float4, xf_s [N] float4, poly_s [rows] float4, grp_s [N] int, cxy_s [ncxy] float
 // and, when it fits (dtab), cxyd_s [ncxy] double: the FP64 evaluations then read their coefficients without a
@@ -40,11 +41,12 @@ __host__ __device__ inline size_t cta_smem_bytes_gen(int N, int rows, int ncxy, 
 // uniform cubic B-spline basis weights of the local coordinate f in [0, 1] (R7)
 template <typename T>
 __device__ __forceinline__ void basis4(T f, T b[4]) {
-    const T o = T(1) - f, f2 = f * f, f3 = f2 * f;
-    b[0] = o * o * o * T(1.0 / 6.0);
-    b[1] = (T(3) * f3 - T(6) * f2 + T(4)) * T(1.0 / 6.0);
-    b[2] = (T(-3) * f3 + T(3) * f2 + T(3) * f + T(1)) * T(1.0 / 6.0);
-    b[3] = f3 * T(1.0 / 6.0);
+    // the two middle weights mirror each other: b1(f) = 2/3 - f^2 + f^3/2, b2(f) = b1(1 - f)
+    const T o = T(1) - f, f2 = f * f, o2 = o * o;
+    b[0] = o2 * o * T(1.0 / 6.0);
+    b[1] = f2 * (T(0.5) * f - T(1)) + T(2.0 / 3.0);
+    b[2] = o2 * (T(0.5) * o - T(1)) + T(2.0 / 3.0);
+    b[3] = f2 * f * T(1.0 / 6.0);
 }
 
 // interval and local coordinate of x on [lo, lo + n / sc], clamped into the range (R5).  (A magic-number rounding
@@ -174,7 +176,8 @@ __global__ void __launch_bounds__(256, 2) recon_gen_kernel(const Params p) {
     }
     __syncthreads();
     unsigned char *wbase = smem + cta_smem_bytes_gen(N, rows, ncxy, p.gen_dtab) + (size_t)warp * warp_smem_bytes_gen(N);
-    float2 *SC = reinterpret_cast<float2 *>(wbase);                       // {S_i prepared, log2(S_i / gL_i) or 0}
+    double *Wd = reinterpret_cast<double *>(wbase);                       // least squares: w_i = 1 / max(S_i, 1)
+    float2 *SC = reinterpret_cast<float2 *>(Wd + N);                      // {S_i prepared, log2(S_i / gL_i) or 0}
     unsigned short *act = reinterpret_cast<unsigned short *>(SC + N);     // indices of the event's active sensors
 
     const int G = p.G, GG = G * G;
@@ -202,8 +205,13 @@ __global__ void __launch_bounds__(256, 2) recon_gen_kernel(const Params p) {
                 act[n_act + __popc(mk & ((1u << lane) - 1u))] = (unsigned short)i;
                 const double S = (double)SC[i].x;
                 sumSd += S;
-                if (METHOD == 0) { if (S > 0.0) SlnS += S * log(S); }
-                else wSS += S * S / fmax(S, 1.0);
+                if (METHOD == 0) {
+                    if (S > 0.0) SlnS += S * log(S);
+                } else {
+                    const double w = 1.0 / fmax(S, 1.0);
+                    Wd[i] = w;
+                    wSS += S * S * w;
+                }
             }
             n_act += __popc(mk);
         }
@@ -242,7 +250,7 @@ __global__ void __launch_bounds__(256, 2) recon_gen_kernel(const Params p) {
                         else a1 += S * log(L);
                     }
                 } else {
-                    const double w = 1.0 / fmax(S, 1.0);
+                    const double w = Wd[i];
                     a1 += w * S * L;
                     a2 += w * L * L;
                 }

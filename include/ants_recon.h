@@ -298,6 +298,28 @@ int ants_lrf_fit_gains(const float *sensor_xy, const float *knots, const float *
                        float *gains_out, double *n_used_out, void *cuda_stream);
 
 /*
+ * ants_lrf_fit_gains_static -- ants_lrf_fit_gains for callers that must not allocate (code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid cudaMalloc).  Same arguments, same reading (R24), same result
+ * (FP64 sums; the order of the final additions differs, so the gains agree to rounding, the pair counts exactly).
+ * The call makes no cudaMalloc / cudaFree and calls no allocating library routine, and uses no host heap either:
+ * the kernel's scratch -- sums, pair counters, the device copies of sensor_xy and coeffs -- is one array of
+ * ANTS_STATIC_SCRATCH_BYTES (8 KB) built into the library, which every GPU that loads the library holds until the
+ * process exits.  Hence the fixed limits: n_sensors <= ANTS_STATIC_MAX_SENSORS and n_int_r + 3 <=
+ * ANTS_STATIC_MAX_COEFFS; a larger request is refused with ANTS_ERR_UNSUPPORTED, nothing is truncated.
+ * Every call on a device uses the same array, which keeps the previous call's contents: the call clears the sums
+ * and counters and overwrites the rest before its kernel runs, and the library serialises the calls of one process
+ * with a lock and returns only after the result is in host memory -- but work that touches the array while a call is
+ * in flight on the GPU (there is none in this library) would race with it.  One kernel launch on `cuda_stream`.
+ * Errors: ANTS_ERR_INVALID, ANTS_ERR_UNSUPPORTED (beyond the limits above; device ordinal >= 64), ANTS_ERR_CUDA.
+ */
+#define ANTS_STATIC_MAX_SENSORS 128
+#define ANTS_STATIC_MAX_COEFFS 1024
+#define ANTS_STATIC_SCRATCH_BYTES 8192
+int ants_lrf_fit_gains_static(const float *sensor_xy, const float *knots, const float *coeffs, int32_t n_sensors,
+                              int32_t n_int_r, const float *signals, const float *xyzA, int64_t n_events,
+                              float *gains_out, double *n_used_out, void *cuda_stream);
+
+/*
  * ants_gains_renormalise -- relative gains are defined up to a common factor ("a scaling
  * parameter (relative gain)"); after a re-evaluation (ants_lrf_fit_gains) the iterative procedure of
  * PAPER.md:428-440 carries them on at the scale of the previous set.  Reading R29: a sensor whose new

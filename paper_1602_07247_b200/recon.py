@@ -95,6 +95,8 @@ def load():
     lib.ants_lrf_fit_axial.argtypes = [vp, vp, vp, C.c_int32, C.c_int32, C.c_int32, vp, vp, C.c_int64, vp, vp, vp]
     lib.ants_lrf_fit_gains.restype = C.c_int
     lib.ants_lrf_fit_gains.argtypes = [vp, vp, vp, C.c_int32, C.c_int32, vp, vp, C.c_int64, vp, vp, vp]
+    lib.ants_lrf_fit_gains_static.restype = C.c_int
+    lib.ants_lrf_fit_gains_static.argtypes = lib.ants_lrf_fit_gains.argtypes
     lib.ants_lrf_fit_axial_grouped.restype = C.c_int
     lib.ants_lrf_fit_axial_grouped.argtypes = [vp, vp, vp, vp, C.c_int32, C.c_int32, C.c_int32, vp, vp, C.c_int64, vp, vp, vp]
     lib.ants_lrf_fit_axial_z.restype = C.c_int
@@ -371,6 +373,26 @@ def ants_lrf_fit_gains(sensor_xy, knots, coeffs, signals, xyzA, stream=None):
         raise AntsError(rc, "ants_lrf_fit_gains")
     return gains, used
 
+
+
+def ants_lrf_fit_gains_static(sensor_xy, knots, coeffs, signals, xyzA, stream=None):
+    """ants_lrf_fit_gains without any allocation inside the library (include/ants_recon.h): scratch in a fixed 8 KB
+    device array, N <= 128, len(coeffs) <= 1024.  -> (gains float32 [N], pairs [N])."""
+    import torch
+    xy, kn, co = _f32(sensor_xy).reshape(-1, 2), _f32(knots), _f32(coeffs).reshape(-1)
+    N, E = xy.shape[0], int(signals.shape[0])
+    for t in (signals, xyzA):
+        if not (t.is_cuda and t.is_contiguous() and t.dtype == torch.float32):
+            raise ValueError("ants_lrf_fit_gains_static needs contiguous float32 CUDA tensors")
+    if signals.shape[1] != N or tuple(xyzA.shape) != (E, 4):
+        raise ValueError("ants_lrf_fit_gains_static: shape mismatch")
+    gains, used = np.zeros(N, np.float32), np.zeros(N, np.float64)
+    st = torch.cuda.current_stream().cuda_stream if stream is None else int(stream)
+    rc = load().ants_lrf_fit_gains_static(xy.ctypes.data, kn.ctypes.data, co.ctypes.data, N, co.size - 3,
+                                          signals.data_ptr(), xyzA.data_ptr(), E, gains.ctypes.data, used.ctypes.data, st)
+    if rc != 0:
+        raise AntsError(rc, "ants_lrf_fit_gains_static")
+    return gains, used
 
 def ants_destroy(handle) -> None:
     load().ants_destroy(handle)

@@ -16,7 +16,10 @@ def iterate_response(cfg, signals, n_cycles: int, score_max: float = float("nan"
                      radius_max: float = float("nan"), refit_gains: bool = False):
     """cfg: a synth.Config-like record with the starting LRFs (axial, shared or per-sensor tables, axial+z,
     XY or Composite); signals: CUDA float32 [E][N].  Yields (cycle, cfg_k, n_events_used) after every cycle, cfg_k
-    carrying the refitted coefficients (and gains when refit_gains, shared axial profile only)."""
+    carrying the refitted coefficients (and gains when refit_gains, shared axial profile only).  A table that the
+    passing events do not cover (an interval or cell without data: typical for per-sensor tables fitted over their full
+    range from a small flood batch) ends the iteration with recon.AntsError (ANTS_ERR_SINGULAR): give cfg the knot range
+    the data cover."""
     cur = copy.copy(cfg)
     for cycle in range(n_cycles):
         r = recon.Reconstructor(cur)
@@ -46,7 +49,8 @@ def iterate_response(cfg, signals, n_cycles: int, score_max: float = float("nan"
             c, _ = recon.ants_lrf_fit_axial_z(cur.sensor_xy, cur.gains, cur.knots, cur.n_int_r, cur.n_int_z, signals, xyzA)
             nxt.coeffs = c[None, :, :].astype(np.float32)
         else:
-            c, _ = recon.ants_lrf_fit_axial(cur.sensor_xy, cur.gains, cur.knots, cur.n_lrf, cur.n_int_r, signals, xyzA)
+            c, _ = recon.ants_lrf_fit_axial(cur.sensor_xy, cur.gains, cur.knots, cur.n_lrf, cur.n_int_r, signals, xyzA,
+                                            group=getattr(cur, "group", None))
             nxt.coeffs = c[:, None, :].astype(np.float32)
             if refit_gains and cur.n_lrf == 1:
                 g, _ = recon.ants_lrf_fit_gains(cur.sensor_xy, cur.knots, c[0], signals, xyzA)

@@ -547,27 +547,33 @@ __global__ void __launch_bounds__(256) lrf_fit_rz2_kernel(const FitRZParams p) {
             k_max = max(k_max, __shfl_xor_sync(0xffffffffu, k_max, o));
         }
         __syncwarp();
-        // expand: rows (kz + b1) ncr + ja, slots (dz, dr) of the 4 x 7 block and the right-hand side
+        // expand: rows (kz + b1) ncr + ja, slots (dz, dr) of the 4 x 7 block and the right-hand side.  A lane takes one
+        // (row ja, offset dr) entry of the r-part -- or the row's right-hand side -- and adds it to all (b1, dz) places
+        // it belongs to, the z-weights bz[b1] bz[b1 + dz] with compile-time indices (the lanes of a warp hit distinct
+        // addresses; only the warps of the CTA meet)
         const int n_rows = k_max - k_min + 1;
-        for (int it = lane; it < n_rows * 29; it += 32) {
-            const int s = it % 29, ja = k_min + it / 29;
-            if (s == 28) {
+        const size_t zrow = (size_t)p.ncr * 29;
+        double *zbase = rz2_smem + (size_t)kz * zrow;
+        for (int it = lane; it < n_rows * 8; it += 32) {
+            const int ja = k_min + (it >> 3), d = it & 7;
+            if (d == 7) {
                 const double rv = Rb[(size_t)ja * 5 + 4];
                 if (rv != 0.0) {
 #pragma unroll
-                    for (int b1 = 0; b1 < 4; ++b1) atomicAdd(rz2_smem + (size_t)((kz + b1) * p.ncr + ja) * 29 + 28, bz[b1] * rv);
+                    for (int b1 = 0; b1 < 4; ++b1) atomicAdd(zbase + b1 * zrow + (size_t)ja * 29 + 28, bz[b1] * rv);
                 }
             } else {
-                const int dz = s / 7, dr = s - dz * 7 - 3, jc = ja + dr;
-                if (jc < 0 || jc >= p.ncr || (dz == 0 && dr < 0)) continue;
+                const int dr = d - 3, jc = ja + dr;
+                if (jc < 0 || jc >= p.ncr) continue;
                 const double rv = Rb[(size_t)min(ja, jc) * 5 + (dr < 0 ? -dr : dr)];
                 if (rv == 0.0) continue;
+                double *q = zbase + (size_t)ja * 29 + d;
 #pragma unroll
                 for (int b1 = 0; b1 < 4; ++b1) {
-                    // b2 = b1 + dz <= 3; the weights are picked by compile-time b1 and a small select on dz
-                    if (b1 + dz > 3) continue;
-                    const double w2 = dz == 0 ? bz[b1] : dz == 1 ? bz[(b1 + 1) & 3] : dz == 2 ? bz[(b1 + 2) & 3] : bz[3];
-                    atomicAdd(rz2_smem + (size_t)((kz + b1) * p.ncr + ja) * 29 + s, bz[b1] * w2 * rv);
+                    if (dr >= 0) atomicAdd(q + b1 * zrow, bz[b1] * bz[b1] * rv);                    // dz = 0: upper triangle only
+#pragma unroll
+                    for (int dz = 1; dz < 4; ++dz)
+                        if (b1 + dz <= 3) atomicAdd(q + b1 * zrow + dz * 7, bz[b1] * bz[b1 + dz] * rv);
                 }
             }
         }

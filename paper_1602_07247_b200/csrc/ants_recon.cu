@@ -753,7 +753,7 @@ static int make_plan3d(const ants_lrf *h, const ants_grid_params_t *g, int32_t m
     // a 3-D search runs the kernel packed over pairs of z-levels; a 2-D search at fixed z the scalar one
     const bool packed = g->dim == 3;
     const int LP = (Gz + 1) / 2;
-    if (packed) gzm = G <= 4 ? 2 : 4;                     // compiled maximum of level pairs
+    if (packed) gzm = LP;                                 // the kernel is compiled for the grid's level pairs
     pl.family = packed ? 4 : 2;
     pl.cpl = cpl;
     pl.gzm = gzm;

@@ -5,7 +5,8 @@
 namespace ants {
 const void *kernel_3d_pk_m1(int cpl, int gzp) {
 #define ANTS_K3(C, Z) if (cpl == C && gzp == Z) return (const void *)recon3d_pk_kernel<C, Z, 1>
-    ANTS_K3(1, 2); ANTS_K3(2, 2); ANTS_K3(1, 4); ANTS_K3(2, 4);
+    // GZP = the grid's level pairs exactly, (G + 1) / 2; one column per lane up to G = 5, two for G = 6 .. 8
+    ANTS_K3(1, 1); ANTS_K3(1, 2); ANTS_K3(1, 3); ANTS_K3(2, 3); ANTS_K3(2, 4);
 #undef ANTS_K3
     return nullptr;
 }

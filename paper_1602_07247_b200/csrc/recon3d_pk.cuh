@@ -136,14 +136,15 @@ __device__ __forceinline__ float4 level_row(const WarpSmem3Dpk &w, int nr1, int 
     return make_float4(src[0], src[2], src[4], src[6]);
 }
 
-// CPL columns per lane, GZP compiled maximum of level PAIRS, METHOD 0 Poisson ML / 1 weighted chi-square.
+// CPL columns per lane, GZP level PAIRS of the grid ((Gz + 1) / 2: an odd Gz leaves the last half pair idle), METHOD 0 Poisson ML / 1 weighted chi-square.
 template <int CPL, int GZP, int METHOD>
 __global__ void __launch_bounds__(256, 2) recon3d_pk_kernel(const Params p) {
     extern __shared__ __align__(16) unsigned char smem[];
     const ModelDev &m = p.m;
     const int N = m.N, nr1 = m.n_r + 1;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int Gz = p.G, LP = (Gz + 1) >> 1;
+    const int Gz = p.G;
+    constexpr int LP = GZP;                 // level pairs: the host picks the instantiation with GZP = (Gz + 1) / 2
     const int ncol = p.G * p.G;
     const int rows = (m.n_z + 3) * nr1;
     const double sczd = (double)m.n_z / ((double)m.z_hi - (double)m.z_lo);

@@ -35,6 +35,7 @@ static const unsigned kCtrSlots = 1024;
 struct Plan {
     int npt = 0;             // nodes per lane (template instantiation)
     int cpl = 0, gzm = 0;    // axial+z kernel: columns per lane, compiled z-levels
+    bool cross = false;      // packed axial+z kernel: top level of an odd grid packed across the lane's two columns
     int family = 0;          // 0 recon2d_pk_kernel, 2 recon3d_kernel, 3 recon_gen_kernel (general), 4 recon3d_pk_kernel
     int warps = 0;           // warps per CTA
     int ctas_per_sm = 0;     // resident CTAs per SM (cudaOccupancyMaxActiveBlocksPerMultiprocessor, capped by the tuning knob)
@@ -653,9 +654,9 @@ const void *kernel_2d_pk_m0(int, int), *kernel_2d_pk_m1(int, int), *kernel_2d_pk
 const void *kernel_gen_m0(int), *kernel_gen_m1(int), *kernel_gen_m2(int);
 const void *kernel_3d_m0(int, int), *kernel_3d_m1(int, int);
 const void *kernel_refine(int);
-const void *kernel_3d_pk_m0(int, int), *kernel_3d_pk_m1(int, int);
-const void *kernel_3d_pk(int method, int cpl, int gzp) {
-    return method == 0 ? kernel_3d_pk_m0(cpl, gzp) : method == 1 ? kernel_3d_pk_m1(cpl, gzp) : nullptr;
+const void *kernel_3d_pk_m0(int, int, int), *kernel_3d_pk_m1(int, int, int);
+const void *kernel_3d_pk(int method, int cpl, int gzp, int cross) {
+    return method == 0 ? kernel_3d_pk_m0(cpl, gzp, cross) : method == 1 ? kernel_3d_pk_m1(cpl, gzp, cross) : nullptr;
 }
 const void *kernel_2d_pk(int method, int npt, int reuse) {
     return method == 0 ? kernel_2d_pk_m0(npt, reuse) : method == 1 ? kernel_2d_pk_m1(npt, reuse)
@@ -681,6 +682,7 @@ static int knob_warps_per_cta() { static const int v = env_knob("ANTS_WARPS_PER_
 static int env_knob_force_reuse() { static const int v = env_knob("ANTS_FORCE_NODE_REUSE"); return v; }
 static int knob_no_reuse() { static const int v = env_knob("ANTS_NO_NODE_REUSE"); return v; }
 static int knob_max_ctas_per_sm() { static const int v = env_knob("ANTS_MAX_CTAS_PER_SM"); return v; }
+static int knob_no_cross() { static const int v = env_knob("ANTS_NO_CROSS_LEVEL"); return v; }
 
 static int validate_grid(const ants_lrf *h, const ants_grid_params_t *g, int32_t method) {
     if (!h || !g) return ANTS_ERR_INVALID;
@@ -758,7 +760,9 @@ static int make_plan3d(const ants_lrf *h, const ants_grid_params_t *g, int32_t m
     pl.cpl = cpl;
     pl.gzm = gzm;
     pl.npt = cpl * Gz;
-    pl.kernel = packed ? kernel_3d_pk(method, cpl, gzm) : kernel_3d(method, cpl, gzm);
+    // an odd grid with two columns per lane packs its top level across the columns (recon3d_pk.cuh, CROSS)
+    pl.cross = packed && cpl == 2 && (Gz & 1) && !knob_no_cross();
+    pl.kernel = packed ? kernel_3d_pk(method, cpl, gzm, pl.cross) : kernel_3d(method, cpl, gzm);
     if (!pl.kernel) return ANTS_ERR_UNSUPPORTED;
     // differential from the first grid that stays within one knot interval of the centre (r and z);
     // Poisson log1p by series once |dL/L0| <= kQSeries on the whole grid
@@ -897,7 +901,8 @@ static int get_plan(const ants_lrf *hc, const ants_grid_params_t *g, int32_t met
 static void kernel_name(const Plan &pl, int32_t method, int lrf_kind, char *buf, size_t n) {
     if (pl.family == 0) std::snprintf(buf, n, "ants::recon2d_pk_kernel<%d,%d,%s>", pl.npt, (int)method, pl.reuse ? "true" : "false");
     else if (pl.family == 3) std::snprintf(buf, n, "ants::recon_gen_kernel<%d,%d>", (int)method, lrf_kind);
-    else if (pl.family == 4) std::snprintf(buf, n, "ants::recon3d_pk_kernel<%d,%d,%d>", pl.cpl, pl.gzm, (int)method);
+    else if (pl.family == 4)
+        std::snprintf(buf, n, "ants::recon3d_pk_kernel<%d,%d,%d%s>", pl.cpl, pl.gzm, (int)method, pl.cross ? ",true" : "");
     else std::snprintf(buf, n, "ants::recon3d_kernel<%d,%d,%d>", pl.cpl, pl.gzm, (int)method);
 }
 

@@ -8,8 +8,9 @@ namespace ants {
 // axial LRFs, strictly positive: sensor-pair-packed kernel (recon2d_pk.cuh).  method 0/1/2, npt in {1,2,3,4,8}
 const void *kernel_2d_pk(int method, int npt, int reuse);
 // axial+z LRFs searched in 3-D, packed over pairs of z-levels (recon3d_pk.cuh).  method 0/1,
-// (cpl, gzp) in {(1,2),(2,2),(1,4),(2,4)}
-const void *kernel_3d_pk(int method, int cpl, int gzp);
+// (cpl, gzp) in {(1,1),(1,2),(1,3),(2,3),(2,4)}; cross = 1: (2,4) with the top level of an odd grid packed across the
+// lane's two columns
+const void *kernel_3d_pk(int method, int cpl, int gzp, int cross);
 // the general kernel (recon_gen.cuh): XY, Composite and Sliced LRFs, and axial LRFs that are not positive
 // everywhere.  method 0/1/2, lrf_kind 1/3/4/5
 const void *kernel_gen(int method, int lrf_kind);

@@ -136,9 +136,16 @@ __device__ __forceinline__ float4 level_row(const WarpSmem3Dpk &w, int nr1, int 
     return make_float4(src[0], src[2], src[4], src[6]);
 }
 
-// CPL columns per lane, GZP level PAIRS of the grid ((Gz + 1) / 2: an odd Gz leaves the last half pair idle), METHOD 0 Poisson ML / 1 weighted chi-square.
-template <int CPL, int GZP, int METHOD>
+// CPL columns per lane, GZP level PAIRS of the grid ((Gz + 1) / 2), METHOD 0 Poisson ML / 1 weighted chi-square.
+// CROSS (odd Gz, two columns per lane): the top level, which has no partner within its column, is packed ACROSS the
+// lane's two columns -- one packed unit {column 0, column 1} at level Gz - 1 with the level's table entries as
+// broadcast operands and the columns' scalars packed -- instead of one half-idle pair per column: 2 (Gz - 1) / 2 + 1
+// packed units per sensor instead of Gz + 1 (7 x 7 x 7: seven instead of eight).  Its accumulators, scores and
+// auxiliaries live in the [0][GZP - 1] entries of the per-(column, pair) arrays ([1][GZP - 1] is unused), half hl =
+// column hl.  Without CROSS an odd Gz leaves the last half pair of every column idle.
+template <int CPL, int GZP, int METHOD, bool CROSS = false>
 __global__ void __launch_bounds__(256, 2) recon3d_pk_kernel(const Params p) {
+    static_assert(!CROSS || CPL == 2, "the cross-column unit pairs the two columns of a lane");
     extern __shared__ __align__(16) unsigned char smem[];
     const ModelDev &m = p.m;
     const int N = m.N, nr1 = m.n_r + 1;
@@ -213,16 +220,19 @@ __global__ void __launch_bounds__(256, 2) recon3d_pk_kernel(const Params p) {
             float bs = kInf;
             int bi = 0x7fffffff;
 #pragma unroll
-            for (int lp = 0; lp < GZP; ++lp)
+            for (int lp = 0; lp < GZP; ++lp) {
+                const bool cross = CROSS && lp == GZP - 1;       // (level Gz - 1: half hl is column hl)
 #pragma unroll
                 for (int hl = 0; hl < 2; ++hl)
 #pragma unroll
-                    for (int j = 0; j < CPL; ++j) {
+                    for (int j = 0; j < (cross ? 1 : CPL); ++j) {
                         float s_lo, s_hi;
                         upk(sc_node[j][lp], s_lo, s_hi);
                         const float s = hl ? s_hi : s_lo;
-                        if (s < bs) { bs = s; bi = ((2 * lp + hl) << 10) | (lane + 32 * j); }
+                        const int code = cross ? ((2 * lp) << 10) | (lane + 32 * hl) : ((2 * lp + hl) << 10) | (lane + 32 * j);
+                        if (s < bs) { bs = s; bi = code; }
                     }
+            }
             warp_argmin_redux(bs, bi);
             const bool found = bs < kInf;
             const int wl = bi >> 10, wc = bi & 1023;
@@ -234,11 +244,16 @@ __global__ void __launch_bounds__(256, 2) recon3d_pk_kernel(const Params p) {
                         wx = fx[j];
                         wy = fy[j];
 #pragma unroll
-                        for (int lp = 0; lp < GZP; ++lp) {
+                        for (int lp = 0; lp < (CROSS ? GZP - 1 : GZP); ++lp) {
                             float a_lo, a_hi;
                             upk(aux_node[j][lp], a_lo, a_hi);
                             if (2 * lp == wl) mine = a_lo;
                             if (2 * lp + 1 == wl) mine = a_hi;
+                        }
+                        if (CROSS) {
+                            float a_c0, a_c1;
+                            upk(aux_node[0][GZP - 1], a_c0, a_c1);
+                            if (wl == 2 * (GZP - 1)) mine = j ? a_c1 : a_c0;
                         }
                     }
                 if (plain) {

@@ -282,6 +282,13 @@ def measure_config(idx: int, args, device, rank: int, world: int, dist, steps: i
     import torch
     from paper_1602_07247_b200 import recon, synth
     cfg = synth.make_config(idx)
+    # variants of a config for kernel studies (profiles/r02_lockstep.md): another grid size or scoring method on the
+    # same detector and events; the workload name says so, and such a line is not a BASELINE.json config
+    if getattr(args, "grid_nodes", None) or getattr(args, "method", None) is not None:
+        import dataclasses
+        G = args.grid_nodes or cfg.nodes_per_axis
+        meth = cfg.method if args.method is None else args.method
+        cfg = dataclasses.replace(cfg, nodes_per_axis=G, method=meth, name=f"{cfg.name}+G{G}m{meth}")
     E = cfg.n_events // cfg.n_batches if args.events is None else args.events
     n_resident = max(2, cfg.n_batches) if args.resident is None else args.resident
     r = recon.Reconstructor(cfg)
@@ -424,7 +431,7 @@ def run_ours(args):
             line[k] = head[k]
 
     # ---- every BASELINE.json config beside the headline (N = 1 only: north_star asks for all five) -----
-    if world == 1 and not args.no_per_config and args.events is None:
+    if world == 1 and not args.no_per_config and args.events is None and not args.grid_nodes and args.method is None:
         per = []
         for idx in (1, 2, 3, 4, 5):
             m = head if idx == args.config else measure_config(
@@ -687,6 +694,9 @@ def main(argv=None):
     ap.add_argument("--no-per-config", action="store_true", help="skip the per_config entries of the other configs")
     ap.add_argument("--per-config-cpu-seconds", type=float, default=5.0)
     ap.add_argument("--events", type=int, default=None, help="events per step per GPU (default: the config's batch)")
+    ap.add_argument("--grid-nodes", type=int, default=None, help="kernel studies: nodes per axis instead of the config's")
+    ap.add_argument("--method", type=int, default=None, choices=[0, 1, 2],
+                    help="kernel studies: scoring method instead of the config's (0 Poisson ML, 1 chi-square, 2 sum-ratio LS)")
     ap.add_argument("--resident", type=int, default=None, help="distinct resident batches to rotate through")
     ap.add_argument("--e2e-chunk", type=int, default=1 << 18)
     ap.add_argument("--cpu-seconds", type=float, default=15.0)

@@ -35,6 +35,7 @@ static const unsigned kCtrSlots = 1024;
 struct Plan {
     int npt = 0;             // nodes per lane (template instantiation)
     int cpl = 0, gzm = 0;    // axial+z kernel: columns per lane, compiled z-levels
+    int lockstep = 0;        // packed 2-D kernel: CTA-wide event rounds behind a barrier
     bool cross = false;      // packed axial+z kernel: top level of an odd grid packed across the lane's two columns
     int family = 0;          // 0 recon2d_pk_kernel, 2 recon3d_kernel, 3 recon_gen_kernel (general), 4 recon3d_pk_kernel
     int warps = 0;           // warps per CTA
@@ -839,12 +840,17 @@ static int make_plan(const ants_lrf *h, const ants_grid_params_t *g, int32_t met
     if (!pl.npt) return ANTS_ERR_UNSUPPORTED;
     // strictly positive axial LRFs (the normal case): the sensor-pair-packed kernel
     pl.family = 0;
-    // node reuse (recon2d_pk_kernel.cuh): contraction 1/2, odd G, and where it was measured to pay: large arrays
-    // (config 5 +7 %), and the Poisson kernel with up to three nodes per lane at any size (configs 1, 2: +2..3 %);
-    // the chi-square kernel with four nodes per lane loses with it on a 64-sensor array (config 3: -7 %)
-    const bool pays = m.N >= 96 || (method == ANTS_POISSON_ML && pl.npt <= 3);
-    pl.reuse = g->factor == 0.5f && (g->nodes_per_axis & 1) && pays && !knob_no_reuse() ? 1 : 0;
-    if (env_knob_force_reuse()) pl.reuse = g->factor == 0.5f && (g->nodes_per_axis & 1) ? 1 : 0;
+    // node reuse (recon2d_pk_kernel.cuh): contraction 1/2 and odd G; pl.reuse = 2 adds the CTA-wide event rounds
+    // (LOCKSTEP).  Measured on every combination (profiles/r02_lockstep.md): node reuse alone gains on the Poisson kernel
+    // with up to three nodes per lane and on large arrays (config 5 +20 %), and loses with four nodes per lane on smaller
+    // arrays and in the least-squares kernels (instruction fetch); with the rounds it gains everywhere (config 3 +10 %,
+    // config 2 +2 % on top of reuse) except on large Poisson arrays, where the events of a CTA differ in cost (the clamped
+    // sensors are dropped per event) and the barrier makes the warps wait for the slowest (config 5 -4 %)
+    const bool can = g->factor == 0.5f && (g->nodes_per_axis & 1);
+    pl.reuse = method == ANTS_POISSON_ML && m.N >= 96 ? 1 : 2;
+    if (!can || knob_no_reuse()) pl.reuse = 0;
+    if (can && env_knob_force_reuse()) pl.reuse = method == ANTS_POISSON_ML ? env_knob_force_reuse() : 2;
+    pl.lockstep = pl.reuse == 2;
     pl.kernel = kernel_2d_pk(method, pl.npt, pl.reuse);
     if (!pl.kernel) return ANTS_ERR_UNSUPPORTED;
     first_diff_iter(h, g, method, pl.k_diff, pl.k_series);
@@ -899,7 +905,7 @@ static int get_plan(const ants_lrf *hc, const ants_grid_params_t *g, int32_t met
 }
 
 static void kernel_name(const Plan &pl, int32_t method, int lrf_kind, char *buf, size_t n) {
-    if (pl.family == 0) std::snprintf(buf, n, "ants::recon2d_pk_kernel<%d,%d,%s>", pl.npt, (int)method, pl.reuse ? "true" : "false");
+    if (pl.family == 0) std::snprintf(buf, n, "ants::recon2d_pk_kernel<%d,%d,%s%s>", pl.npt, (int)method, pl.reuse ? "true" : "false", pl.lockstep ? ",true" : "");
     else if (pl.family == 3) std::snprintf(buf, n, "ants::recon_gen_kernel<%d,%d>", (int)method, lrf_kind);
     else if (pl.family == 4)
         std::snprintf(buf, n, "ants::recon3d_pk_kernel<%d,%d,%d%s>", pl.cpl, pl.gzm, (int)method, pl.cross ? ",true" : "");

@@ -6,6 +6,7 @@
 namespace ants {
 
 // axial LRFs, strictly positive: sensor-pair-packed kernel (recon2d_pk.cuh).  method 0/1/2, npt in {1,2,3,4,8}
+// reuse: 0 none, 1 node reuse, 2 node reuse with the CTA's warps taking their events in rounds behind a barrier
 const void *kernel_2d_pk(int method, int npt, int reuse);
 // axial+z LRFs searched in 3-D, packed over pairs of z-levels (recon3d_pk.cuh).  method 0/1,
 // (cpl, gzp) in {(1,1),(1,2),(1,3),(2,3),(2,4)}; cross = 1: (2,4) with the top level of an odd grid packed across the

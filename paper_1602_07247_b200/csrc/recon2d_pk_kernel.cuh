@@ -7,7 +7,8 @@ namespace ants {
 // REUSE: carry the scores of coinciding nodes over from the previous grid (see below); the host picks it for large
 // arrays, where it pays (config 5: +7 %); the kernel is latency-bound, and with a round of nodes less per lane the
 // smaller arrays lose more instruction-level parallelism than they save work (config 3: -13 %).
-template <int NPT, int METHOD, bool REUSE>
+// LOCKSTEP: the CTA takes its events in rounds of one event per warp behind a barrier (see "Event distribution" below).
+template <int NPT, int METHOD, bool REUSE, bool LOCKSTEP = false>
 __global__ void __launch_bounds__(256, (NPT <= 3 ? 3 : 2)) recon2d_pk_kernel(const Params p) {
     extern __shared__ __align__(16) unsigned char smem[];
     const ModelDev &m = p.m;
@@ -71,27 +72,50 @@ __global__ void __launch_bounds__(256, (NPT <= 3 ? 3 : 2)) recon2d_pk_kernel(con
     const float half_diag_units = 1.41421356f * half;
     const f32x2 sc2 = pk1(m.sc), of2 = pk1(m.of), magic2 = pk1(kMagic), nmagic2 = pk1(-kMagic);
 
-    // the next event's signals are fetched into registers (4 per lane: N <= 128) while this one runs
+    // The next event's signals are fetched while this one runs: into registers (4 per lane: N <= 128) in the
+    // instantiations with up to three nodes per lane, into L2 only (prefetch.global.L2) in the larger ones, where four
+    // more registers held across the search cost the node loops their in-place accumulators (register copies at every
+    // loop back-edge of the chi-square node-reuse kernel).
+    constexpr bool kRegPrefetch = NPT <= 3;
     float pf[4];
     auto prefetch = [&](long long ev) {
+        if (kRegPrefetch) {
 #pragma unroll
-        for (int c = 0; c < 4; ++c) {
-            const int i = lane + 32 * c;
-            pf[c] = (ev < p.n_events && i < N) ? __ldg(p.signals + ev * N + i) : 0.f;
+            for (int c = 0; c < 4; ++c) {
+                const int i = lane + 32 * c;
+                pf[c] = (ev < p.n_events && i < N) ? __ldg(p.signals + ev * N + i) : 0.f;
+            }
+        } else if (ev < p.n_events) {
+            for (int i = lane * 32; i < N; i += 32 * 32)       // one request per 128-byte line of the row
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(p.signals + ev * N + i));
         }
     };
-    long long e_next = grab_event(p.ctr, lane);
+    // Event distribution.  Default: every warp takes its next event from the launch's counter on its own.  LOCKSTEP:
+    // the CTA takes `warps` consecutive events per round behind a barrier, so its warps walk through the phases of
+    // the search together and share the instruction caches: the kernel's code is several times their size, and the
+    // node-reuse instantiations, with two sets of node loops, stalled on instruction fetch 1.9 warps per issue slot on
+    // config 3 (0.4 without reuse).  It pays where the events of a CTA take about the same time (profiles/r02_lockstep.md).
+    __shared__ long long round_s;
+    const int warps = blockDim.x >> 5;
+    long long b_next = LOCKSTEP ? grab_round(p.ctr, warps, &round_s) : 0;
+    long long e_next = LOCKSTEP ? b_next + warp : grab_event(p.ctr, lane);
     prefetch(e_next);
-    for (long long e = e_next; e < p.n_events; e = e_next) {
-        e_next = grab_event(p.ctr, lane);
-        // ---- a1: signals (prefetched while the previous event ran), centroid / strongest-sensor start, selection
-        // (prepare_event, recon_common.cuh); the next event's row is requested before this one is searched
+    for (long long e = e_next; LOCKSTEP ? b_next < p.n_events : e < p.n_events; e = e_next) {
+        if (LOCKSTEP) {
+            b_next = grab_round(p.ctr, warps, &round_s);
+            e_next = b_next + warp;
+            if (e >= p.n_events) continue;       // (the last round may be short)
+        } else {
+            e_next = grab_event(p.ctr, lane);
+        }
+        // ---- a1: signals (requested into L2 while the previous event ran), centroid / strongest-sensor start,
+        // selection (prepare_event, recon_common.cuh); the next event's row is requested before this one is searched
         float cur[4];
 #pragma unroll
-        for (int c = 0; c < 4; ++c) cur[c] = pf[c];
+        for (int c = 0; c < 4; ++c) cur[c] = kRegPrefetch ? pf[c] : 0.f;
         prefetch(e_next);
         float sumS, cx, cy;
-        if (!prepare_event<METHOD>(p, sens_s, w.SC, e, lane, sumS, cx, cy, cur)) continue;
+        if (!prepare_event<METHOD>(p, sens_s, w.SC, e, lane, sumS, cx, cy, kRegPrefetch ? cur : nullptr)) continue;
 
         // reference energy for the plain score: A at the seed
         float A_ref;
@@ -173,8 +197,9 @@ __global__ void __launch_bounds__(256, (NPT <= 3 ? 3 : 2)) recon2d_pk_kernel(con
             }
             if (REUSE) {
 #pragma unroll
-                for (int j = 0; j < NPT; ++j)
-                    if (lane + 32 * j < count) sc_cur[nid[j]] = sc_node[j];
+                for (int j = 0; j < NPT; ++j)     // (four nodes per lane: the ids are read again rather than kept across
+                                                  // the node loops, whose accumulators need the registers)
+                    if (lane + 32 * j < count) sc_cur[NPT >= 4 ? (int)lst[lane + 32 * j] : nid[j]] = sc_node[j];
                 __syncwarp();
             }
 

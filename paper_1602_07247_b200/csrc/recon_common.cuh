@@ -171,6 +171,14 @@ __device__ __forceinline__ long long grab_event(unsigned long long *ctr, int lan
     if (lane == 0) v = atomicAdd(ctr, 1ULL);
     return (long long)__shfl_sync(kFull, v, 0);
 }
+// CTA-wide round: one thread takes `warps` consecutive events for the CTA, all threads learn the first (the two
+// barriers also keep the CTA's warps in the same phase of the search: see recon2d_pk_kernel.cuh)
+__device__ __forceinline__ long long grab_round(unsigned long long *ctr, int warps, long long *slot_s) {
+    __syncthreads();
+    if (threadIdx.x == 0) *slot_s = (long long)atomicAdd(ctr, (unsigned long long)warps);
+    __syncthreads();
+    return *slot_s;
+}
 // a warp is done: count it; the last one re-arms the counters
 __device__ __forceinline__ void retire_warp(unsigned long long *ctr, int total_warps, int lane) {
     if (lane == 0) {

@@ -1285,7 +1285,28 @@ static int fit_axial_impl(const float *sensor_xy, const float *gains, const int3
         if (priv_threads < 64) priv_threads = (int)std::min<size_t>(128, (226 * 1024 / per_thread) / 32 * 32);
         if (priv_threads < 32) priv_threads = 0;
     }
-    if (ok && n_events > 0 && priv_threads > 0) {
+    // one table per sensor (no groups) on an array of up to 128 sensors whose tables fit in shared memory: a thread
+    // owns a sensor (lrf_fit_owned_kernel), no atomics in the loop either
+    const int own_threads = (N + 31) / 32 * 32;
+    const bool owned = n_lrf == N && N > 1 && !group && N <= 128 && per_thread * own_threads <= 226 * 1024 &&
+                       !std::getenv("ANTS_FIT_ATOMIC");
+    if (ok && n_events > 0 && owned) {
+        FitParams p{};
+        p.sens_xy = d_xy; p.gains = d_g; p.group = nullptr; p.signals = signals; p.xyzA = xyzA; p.n_events = n_events;
+        p.N = N; p.n_lrf = n_lrf; p.n_int = n_int; p.nc = nc;
+        p.lo = lo; p.hi = hi; p.h = (hi - lo) / n_int;
+        p.acc = d_acc; p.n_used = d_used; p.copies = own_threads; p.lane_split = 1;
+        const size_t osmem = per_thread * own_threads;
+        int occ = 0;
+        ok = cudaFuncSetAttribute((const void *)lrf_fit_owned_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)osmem) == cudaSuccess &&
+             cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void *)lrf_fit_owned_kernel, own_threads, osmem) == cudaSuccess && occ >= 1;
+        if (ok) {
+            const int grid = (int)std::min<long long>(n_events, (long long)sms * occ);
+            void *args[] = {&p};
+            ok = cudaLaunchKernel((const void *)lrf_fit_owned_kernel, dim3(grid), dim3(own_threads), args, osmem, st) == cudaSuccess;
+            if (ok) g_launches.fetch_add(1);
+        }
+    } else if (ok && n_events > 0 && priv_threads > 0) {
         FitParams p{};
         p.sens_xy = d_xy; p.gains = d_g; p.group = nullptr; p.signals = signals; p.xyzA = xyzA; p.n_events = n_events;
         p.N = N; p.n_lrf = 1; p.n_int = n_int; p.nc = nc;

@@ -495,6 +495,92 @@ __global__ void __launch_bounds__(128) lrf_fit_shared_kernel(const FitParams p) 
 
 namespace ants {
 
+// ---- axial LRF calculation, ONE TABLE PER SENSOR (n_lrf = N, no groups), without atomics in the loop -----------------
+// lrf_fit_kernel maps a warp to an event and lanes to sensors: several warps of a CTA update the same sensor's table,
+// hence its shared-memory FP64 CAS loops.  Here a THREAD owns a sensor: thread t of every CTA takes sensor t of all the
+// events its CTA sees, and that sensor's band, 5 (n + 3) entries, sits in column t of a shared-memory array laid out
+// [entry][thread] -- the 14 updates of a pair are plain load-add-store, free of conflicts and of retries; the signals
+// of an event are one coalesced row read, its position one broadcast load.  The columns are added to the global
+// accumulators once at the end.  Needs N <= 128 and 40 (n + 3) N bytes of shared memory (the host checks; else
+// lrf_fit_kernel).
+__global__ void __launch_bounds__(128) lrf_fit_owned_kernel(const FitParams p) {
+    extern __shared__ double fo_smem[];                 // [nc * 5][blockDim.x]
+    const int T = blockDim.x, t = threadIdx.x;
+    const int entries = p.nc * 5;
+    for (int i = t; i < entries * T; i += T) fo_smem[i] = 0.0;
+    __syncthreads();
+    double *mine = fo_smem + t;
+    const bool have = t < p.N;
+    const double sx = have ? (double)p.sens_xy[2 * t] : 0.0, sy = have ? (double)p.sens_xy[2 * t + 1] : 0.0;
+    const double inv_h = 1.0 / p.h;
+    unsigned long long used = 0ULL;
+    // the position rows and the signals of the next two events wait in registers (few warps fit beside the tables)
+    constexpr int kAhead = 2;
+    float4 pe_q[kAhead + 1];
+    float sg_q[kAhead + 1];
+    auto fetch = [&](int slot, long long ev) {
+        const bool in = ev < p.n_events;
+        pe_q[slot] = in ? __ldg(reinterpret_cast<const float4 *>(p.xyzA) + ev) : make_float4(0.f, 0.f, 0.f, 0.f);
+        sg_q[slot] = (in && have) ? __ldg(p.signals + ev * p.N + t) : 0.f;
+    };
+    const long long stride = gridDim.x;
+#pragma unroll
+    for (int a = 0; a < kAhead; ++a) fetch(a, (long long)blockIdx.x + a * stride);
+    for (long long e = blockIdx.x; e < p.n_events; e += stride) {
+        fetch(kAhead, e + kAhead * stride);
+        const float4 pe = pe_q[0];
+        const double sv = (double)sg_q[0];
+#pragma unroll
+        for (int a = 0; a < kAhead; ++a) { pe_q[a] = pe_q[a + 1]; sg_q[a] = sg_q[a + 1]; }
+        const double x = (double)pe.x, y = (double)pe.y, A = (double)pe.w;
+        if (!(fabs(x) <= 1.7e308 && fabs(y) <= 1.7e308 && A > 0.0 && A <= 1.7e308)) continue;     // R22 (CTA-uniform)
+        const double dx = x - sx, dy = y - sy;
+        const double r = sqrt(dx * dx + dy * dy);
+        if (!(have && r >= p.lo && r <= p.hi)) continue;                                          // R22
+        const double yv = sv / A;                                                                  // R21 (own table: no gain)
+        const double tt = (r - p.lo) * inv_h;
+        const int k = min(max((int)floor(tt), 0), p.n_int - 1);
+        const double u = tt - (double)k, o = 1.0 - u, u2 = u * u, u3 = u2 * u;
+        const double b4[4] = {o * o * o * (1.0 / 6.0), (3.0 * u3 - 6.0 * u2 + 4.0) * (1.0 / 6.0),
+                              (-3.0 * u3 + 3.0 * u2 + 3.0 * u + 1.0) * (1.0 / 6.0), u3 * (1.0 / 6.0)};
+        double *row = mine + (size_t)k * 5 * T;
+        double v[14];
+        int n = 0;
+#pragma unroll
+        for (int a = 0; a < 4; ++a) {
+            v[n++] = row[(a * 5 + 4) * T];
+#pragma unroll
+            for (int c = a; c < 4; ++c) v[n++] = row[(a * 5 + c - a) * T];
+        }
+        n = 0;
+#pragma unroll
+        for (int a = 0; a < 4; ++a) {
+            v[n++] += b4[a] * yv;
+#pragma unroll
+            for (int c = a; c < 4; ++c) v[n++] += b4[a] * b4[c];
+        }
+        n = 0;
+#pragma unroll
+        for (int a = 0; a < 4; ++a) {
+            row[(a * 5 + 4) * T] = v[n++];
+#pragma unroll
+            for (int c = a; c < 4; ++c) row[(a * 5 + c - a) * T] = v[n++];
+        }
+        ++used;
+    }
+    if (have) {
+        if (used) atomicAdd(p.n_used + t, used);
+        for (int j = 0; j < entries; ++j) {
+            const double s = mine[(size_t)j * T];
+            if (s != 0.0) atomicAdd(p.acc + (size_t)t * entries + j, s);
+        }
+    }
+}
+
+}  // namespace ants
+
+namespace ants {
+
 // ---- axial+z tensor LRF calculation, factorised per event (round 2) ------------------------------------------------
 // All pairs of one event share the event's z, hence the same four z-basis weights bz: the event's contribution to
 // the normal equations is (bz bz^T) (x) (sum_i br_i br_i^T) and to the right-hand side bz (x) (sum_i br_i y_i).  The

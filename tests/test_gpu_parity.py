@@ -336,6 +336,39 @@ def test_status_codes():
 
 
 # ---------------------------------------------------------------------------
+# kernel variants of the packed kernels: node reuse, CTA-wide event rounds, cross-column top level
+# ---------------------------------------------------------------------------
+@pytest.mark.parametrize("idx,G,method,n,kernel", [
+    (2, 9, 0, 3001, "ants::recon2d_pk_kernel<3,0,true,true>"),      # Poisson, small array: reuse + rounds
+    (5, 9, 0, 1203, "ants::recon2d_pk_kernel<3,0,true>"),           # Poisson, 127 sensors: reuse, no rounds
+    (2, 11, 0, 2003, "ants::recon2d_pk_kernel<4,0,true,true>"),     # four nodes per lane (L2 prefetch)
+    (5, 11, 0, 803, "ants::recon2d_pk_kernel<4,0,true>"),
+    (3, 11, 1, 2005, "ants::recon2d_pk_kernel<4,1,true,true>"),     # chi-square: always with the rounds
+    (3, 9, 2, 2001, "ants::recon2d_pk_kernel<3,2,true,true>"),
+    (5, 9, 1, 1001, "ants::recon2d_pk_kernel<3,1,true,true>"),
+    (2, 8, 0, 2001, "ants::recon2d_pk_kernel<2,0,false>"),          # even G: no node coincides
+    (4, 7, 0, 1001, "ants::recon3d_pk_kernel<2,4,0,true>"),         # odd 3-D grid, two columns per lane: cross unit
+    (4, 8, 0, 601, "ants::recon3d_pk_kernel<2,4,0>"),
+    (4, 7, 1, 801, "ants::recon3d_pk_kernel<2,4,1,true>"),
+])
+def test_packed_kernel_variants_are_picked_and_in_parity(idx, G, method, n, kernel):
+    """The plan's choice among the instantiations (csrc/ants_recon.cu make_plan / make_plan3d; profiles/r02_lockstep.md)
+    and parity of each under the full rule set.  The event counts are no multiple of a CTA's warps, so the kernels
+    with CTA-wide rounds end on a short round."""
+    cfg = synth.make_config(idx)
+    cfg.nodes_per_axis, cfg.method = G, method
+    ev = synth.generate_events(cfg, n, device="cuda")
+    r = recon.Reconstructor(cfg)
+    try:
+        assert r.plan()["kernel"] == kernel
+    finally:
+        r.close()
+    xyzA, score, path = _run(cfg, ev["signals"])
+    res = parity_rules.compare(cfg, ev["signals"].cpu().numpy(), xyzA, score, path)
+    parity_rules.assert_parity(res, f"{cfg.name} G={G} method={method} {kernel}")
+
+
+# ---------------------------------------------------------------------------
 # axial+z LRF variants beyond config 4
 # ---------------------------------------------------------------------------
 @pytest.mark.parametrize("G,method", [(7, 1), (4, 0), (8, 0), (3, 1), (5, 0)])

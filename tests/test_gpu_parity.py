@@ -110,6 +110,28 @@ def test_parity_cfg5_batch_sampled():
     parity_rules.assert_parity(res, "cfg5 host-streamed")
 
 
+@pytest.mark.parametrize("idx,E,chunk", [(2, 150_001, 40_003), (3, 60_001, 25_001)])
+def test_host_streamed_path_equals_device_path_on_round_kernels(idx, E, chunk):
+    """The kernels that take their events in CTA-wide rounds, through ants_reconstruct_host with chunks that are no
+    multiple of a CTA's warps (every chunk ends on a short round, three launches in flight on three streams): bit for
+    bit the device path's result."""
+    cfg = synth.make_config(idx)
+    ev = synth.generate_events(cfg, E, device="cuda", batch=2)
+    sig_h = ev["signals"].cpu().pin_memory()
+    xyzA = torch.empty((E, 4), dtype=torch.float32).pin_memory()
+    score = torch.empty((E,), dtype=torch.float32).pin_memory()
+    r = recon.Reconstructor(cfg)
+    try:
+        assert r.plan()["kernel"].endswith(",true,true>")
+        recon.ants_reconstruct_host(r.handle, sig_h, r.grid, r.method, xyzA, score, chunk_events=chunk)
+        d_xyzA, d_score = r(ev["signals"])
+        torch.cuda.synchronize()
+    finally:
+        r.close()
+    assert torch.equal(xyzA, d_xyzA.cpu()) and torch.equal(score, d_score.cpu())
+    assert torch.isfinite(score).all()
+
+
 # ---------------------------------------------------------------------------
 # edge cases
 # ---------------------------------------------------------------------------

@@ -4,10 +4,10 @@
 namespace ants {
 
 // METHOD 0 Poisson ML, 1 weighted chi-square.  Requires every LRF strictly positive (host-checked).
-// REUSE: carry the scores of coinciding nodes over from the previous grid (see below); the host picks it for large
-// arrays, where it pays (config 5: +7 %); the kernel is latency-bound, and with a round of nodes less per lane the
-// smaller arrays lose more instruction-level parallelism than they save work (config 3: -13 %).
+// REUSE: carry the scores of coinciding nodes over from the previous grid (see "Node reuse" below).
 // LOCKSTEP: the CTA takes its events in rounds of one event per warp behind a barrier (see "Event distribution" below).
+// The host picks both (make_plan in ants_recon.cu; measured per workload in profiles/r02_lockstep.md): reuse whenever
+// the contraction factor is 1/2 and G is odd, with the rounds except for Poisson ML on large arrays.
 template <int NPT, int METHOD, bool REUSE, bool LOCKSTEP = false>
 __global__ void __launch_bounds__(256, (NPT <= 3 ? 3 : 2)) recon2d_pk_kernel(const Params p) {
     extern __shared__ __align__(16) unsigned char smem[];

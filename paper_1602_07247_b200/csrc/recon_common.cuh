@@ -65,6 +65,8 @@ struct Params {
     int tile_events;        // events staged per CTA tile (= warps_per_cta)
     int gen_dtab;           // general kernel: a double copy of the XY coefficients sits in shared memory
     int reuse;              // packed 2-D kernel: carry coinciding nodes' scores over from the previous grid
+    int lockstep;           // general kernel: the warps of a CTA take their events in rounds behind a barrier (the packed
+                            // 2-D kernel has this as a template flag)
 };
 
 __device__ __forceinline__ float sqrt_approx(float x) {

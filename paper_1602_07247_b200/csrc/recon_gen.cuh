@@ -188,9 +188,23 @@ __global__ void __launch_bounds__(256, 2) recon_gen_kernel(const Params p) {
     const double dzp = zdep ? (z_hi - z_lo) / (double)(m.n_planes - 1) : 1.0;
     const int chunks = (p.nodes + 32 * kNB - 1) / (32 * kNB);
 
-    long long e_next = grab_event(p.ctr, lane);
-    for (long long e = e_next; e < p.n_events; e = e_next) {
-        e_next = grab_event(p.ctr, lane);
+    // Event distribution: every warp on its own, or (p.lockstep, a run-time flag here) the CTA in rounds of one event per
+    // warp behind a barrier, which keeps its warps in the same phase of the search -- the FP32 and FP64 node loops of the
+    // Composite LRF are two large bodies of code (recon2d_pk_kernel.cuh explains the mechanism; config 8 +15 %, no
+    // change on the 37- and 64-sensor configs 7 and 6: the plan sets it for arrays of up to 32 sensors)
+    __shared__ long long round_s;
+    const int warps_cta = blockDim.x >> 5, warp_id = threadIdx.x >> 5;
+    const bool LOCKSTEP = p.lockstep != 0;
+    long long b_next = LOCKSTEP ? grab_round(p.ctr, warps_cta, &round_s) : 0;
+    long long e_next = LOCKSTEP ? b_next + warp_id : grab_event(p.ctr, lane);
+    for (long long e = e_next; LOCKSTEP ? b_next < p.n_events : e < p.n_events; e = e_next) {
+        if (LOCKSTEP) {
+            b_next = grab_round(p.ctr, warps_cta, &round_s);
+            e_next = b_next + warp_id;
+            if (e >= p.n_events) continue;
+        } else {
+            e_next = grab_event(p.ctr, lane);
+        }
         // ---- a1: load signals (coalesced), prepare, centroid, start position, selection ----
         float sumS, sx0, sy0;
         if (!prepare_event<METHOD>(p, sens_s, SC, e, lane, sumS, sx0, sy0)) continue;

